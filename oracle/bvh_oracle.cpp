@@ -1,0 +1,428 @@
+// oracle/bvh_oracle.cpp
+//
+// TEST INFRASTRUCTURE ONLY.  A plain, serial, slow CPU statement of what the hot path computes,
+// written from /root/reference/PAPER.md ("Revising Apetrei's bounding volume hierarchy construction
+// algorithm to allow stackless traversal") and the readings D1-D8 / G1-G21 listed in DESIGN.md.
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load
+// this file.  It shares no code, header, table or helper with the CUDA path under
+// paper_2402_00665_b200/csrc/, and neither includes the other.
+//
+// Build:  g++ -O2 -std=c++17 -ffp-contract=off -fPIC -shared   (no -ffast-math, no -march flags)
+// All floating point is fp32, round-to-nearest, one operation per statement (no contraction), the
+// precision BASELINE.json `north_star` fixes.
+//
+// What each function follows (PAPER.md line numbers):
+//   oracle_scene_bounds   D1  union of primitive boxes (frame for step 1)
+//   oracle_morton         D2  "calculate Morton indices"; formula is DESIGN.md's reading
+//   oracle_sort           D3  "sort Morton indices", stable = index tie-break
+//   oracle_hierarchy      D5  Karras' top-down split search, Karras numbering
+//   oracle_ropes          D6  skip-connection by its definition: explicit stack walk
+//   oracle_ropes_alg2     P2  Algorithm 2 closed form -- second derivation
+//   oracle_boxes          D7  step 4 "compute the bounding boxes of the internal nodes"
+//   oracle_query_*_tree   D8  range search with a STACK on {left,right}
+//   oracle_query_*_brute  D8  the plain definition: test every primitive
+//
+// Parity pins (tests/test_oracle_*.py): P1 worked example reconstructed from PAPER.md:120/166,
+// P2 Algorithm 2, P3 invariants, P4 closed forms, P5 brute force, P6 numpy stable sort, P7 Morton
+// corners and exact-grid codes, and a test-side transliteration of Algorithm 4.  No function here
+// is "parity unpinned".
+
+#include <algorithm>
+#include <cstdint>
+#include <cstring>
+#include <numeric>
+#include <utility>
+#include <vector>
+
+namespace {
+
+constexpr int32_t SENTINEL = -1;  // the paper's black diamond; G9
+
+struct Box {
+  float lo[3];
+  float hi[3];
+};
+
+// Primitive i as a box.  Points are degenerate boxes (min = max = point).
+inline Box prim_box(const float* prim, int64_t i, int is_box) {
+  Box b;
+  if (is_box) {
+    for (int a = 0; a < 3; ++a) {
+      b.lo[a] = prim[6 * i + a];
+      b.hi[a] = prim[6 * i + 3 + a];
+    }
+  } else {
+    for (int a = 0; a < 3; ++a) {
+      b.lo[a] = prim[3 * i + a];
+      b.hi[a] = prim[3 * i + a];
+    }
+  }
+  return b;
+}
+
+inline float fmin2(float a, float b) { return (b < a) ? b : a; }
+inline float fmax2(float a, float b) { return (b > a) ? b : a; }
+
+// Augmented key k'_i = (code_i, i) (reading G5).  Bit numbering: bits 32..95 are the
+// code, bits 0..31 the sorted position.
+inline int aug_bit(uint64_t code, uint32_t idx, int bit) {
+  if (bit >= 32) return (int)((code >> (bit - 32)) & 1u);
+  return (int)((idx >> bit) & 1u);
+}
+
+// Highest bit at which k'_f and k'_l differ (f != l so they differ somewhere).
+inline int highest_differing_bit(uint64_t cf, uint32_t f, uint64_t cl, uint32_t l) {
+  const uint64_t xc = cf ^ cl;
+  if (xc != 0) return 32 + (63 - __builtin_clzll(xc));  // position of the top set bit of the code XOR
+  const uint32_t xi = f ^ l;
+  if (xi != 0) return 31 - __builtin_clz(xi);
+  return -1;
+}
+
+// D8 sphere-vs-box, exact association fixed in DESIGN.md.
+inline bool sphere_hits_box(const float c[3], float r, const float lo[3], const float hi[3]) {
+  float s[3];
+  for (int a = 0; a < 3; ++a) {
+    float u = lo[a] - c[a];
+    float v = c[a] - hi[a];
+    float d = fmax2(fmax2(u, v), 0.0f);
+    s[a] = d * d;
+  }
+  float d2 = s[0] + s[1];
+  d2 = d2 + s[2];
+  float r2 = r * r;
+  return d2 <= r2;
+}
+
+// D8 box-vs-box, closed comparisons (G12).
+inline bool box_hits_box(const float qlo[3], const float qhi[3], const float lo[3], const float hi[3]) {
+  for (int a = 0; a < 3; ++a) {
+    if (!(qlo[a] <= hi[a])) return false;
+    if (!(lo[a] <= qhi[a])) return false;
+  }
+  return true;
+}
+
+struct CsrResult {
+  std::vector<int64_t> offsets;
+  std::vector<int32_t> indices;
+};
+
+}  // namespace
+
+extern "C" {
+
+// D1.  out6 = {lo.x, lo.y, lo.z, hi.x, hi.y, hi.z}.  n >= 1.
+void oracle_scene_bounds(const float* prim, int64_t n, int is_box, float* out6) {
+  Box s = prim_box(prim, 0, is_box);
+  for (int64_t i = 1; i < n; ++i) {
+    Box b = prim_box(prim, i, is_box);
+    for (int a = 0; a < 3; ++a) {
+      s.lo[a] = fmin2(s.lo[a], b.lo[a]);
+      s.hi[a] = fmax2(s.hi[a], b.hi[a]);
+    }
+  }
+  for (int a = 0; a < 3; ++a) {
+    out6[a] = s.lo[a];
+    out6[3 + a] = s.hi[a];
+  }
+}
+
+// D2.  bits = 30 (10 per axis) or 63 (21 per axis).  x is the most significant axis: bit k of
+// cell_x -> code bit 3k+2, cell_y -> 3k+1, cell_z -> 3k.  Interleave is a bit-by-bit loop.
+void oracle_morton(const float* prim, int64_t n, int is_box, const float* scene6, int bits,
+                   uint64_t* codes) {
+  const int b = bits / 3;
+  const float scale = (float)((uint32_t)1 << b);  // 2^b, exact
+  const uint32_t cell_max = ((uint32_t)1 << b) - 1u;
+  for (int64_t i = 0; i < n; ++i) {
+    Box p = prim_box(prim, i, is_box);
+    uint32_t cell[3];
+    for (int a = 0; a < 3; ++a) {
+      float sum = p.lo[a] + p.hi[a];
+      float c = sum * 0.5f;
+      float e = scene6[3 + a] - scene6[a];
+      float t = 0.0f;
+      if (e > 0.0f) {
+        float num = c - scene6[a];
+        t = num / e;
+      }
+      float scaled = t * scale;
+      uint32_t q = (uint32_t)scaled;  // truncation
+      cell[a] = (q < cell_max) ? q : cell_max;
+    }
+    uint64_t code = 0;
+    for (int k = 0; k < b; ++k) {
+      code |= (uint64_t)((cell[0] >> k) & 1u) << (3 * k + 2);
+      code |= (uint64_t)((cell[1] >> k) & 1u) << (3 * k + 1);
+      code |= (uint64_t)((cell[2] >> k) & 1u) << (3 * k + 0);
+    }
+    codes[i] = code;
+  }
+}
+
+// D3.  perm[i] = original index at sorted position i; equal codes keep ascending original index.
+void oracle_sort(const uint64_t* codes, int64_t n, uint64_t* sorted, uint32_t* perm) {
+  std::vector<uint32_t> idx((size_t)n);
+  std::iota(idx.begin(), idx.end(), 0u);
+  std::stable_sort(idx.begin(), idx.end(),
+                   [codes](uint32_t a, uint32_t b) { return codes[a] < codes[b]; });
+  for (int64_t i = 0; i < n; ++i) {
+    perm[i] = idx[(size_t)i];
+    sorted[i] = codes[idx[(size_t)i]];
+  }
+}
+
+// D5.  Karras' construction over the augmented keys (sorted[i], i).
+// Unified node index (G8): internal I_k -> k, leaf L_i -> (n-1)+i.  Outputs, all of length n-1:
+// left[k], right[k] (unified child indices), first[k], last[k] (range covered by I_k).
+// n >= 2 (n = 1 has no internal node).
+void oracle_hierarchy(const uint64_t* sorted, int64_t n, int32_t* left, int32_t* right,
+                      int32_t* first, int32_t* last) {
+  struct Item {
+    int32_t f, l, idx;
+  };
+  std::vector<Item> stack;
+  stack.push_back({0, (int32_t)(n - 1), 0});  // "The root node is assigned index 0" PAPER.md:101
+  const int32_t leaf_base = (int32_t)(n - 1);
+  while (!stack.empty()) {
+    Item it = stack.back();
+    stack.pop_back();
+    const int32_t f = it.f, l = it.l;
+    // "partitions its keys according to the highest differing bit in its range" PAPER.md:99
+    const int B = highest_differing_bit(sorted[f], (uint32_t)f, sorted[l], (uint32_t)l);
+    // gamma = last position in [f, l) whose key has bit B clear.  Keys in [f,l] agree above B and
+    // are sorted, so "bit B clear" holds on a prefix of the range: binary search for its end.
+    int32_t a = f, b = l;  // invariant: bit clear at a, bit set at b
+    while (b - a > 1) {
+      int32_t m = a + (b - a) / 2;
+      if (aug_bit(sorted[m], (uint32_t)m, B) == 0)
+        a = m;
+      else
+        b = m;
+    }
+    const int32_t gamma = a;
+    first[it.idx] = f;
+    last[it.idx] = l;
+    // "The children of an internal node with a split gamma are assigned indices gamma and gamma+1
+    //  in either the internal node array or the leaf node array" PAPER.md:101
+    if (f == gamma) {
+      left[it.idx] = leaf_base + gamma;
+    } else {
+      left[it.idx] = gamma;
+      stack.push_back({f, gamma, gamma});
+    }
+    if (gamma + 1 == l) {
+      right[it.idx] = leaf_base + gamma + 1;
+    } else {
+      right[it.idx] = gamma + 1;
+      stack.push_back({gamma + 1, l, gamma + 1});
+    }
+  }
+}
+
+// D6.  "each skip-connection points to the right child of the last internal node that a given node
+// is in the left subtree of ... the nodes on the right-most path (including the root node) ... all
+// point to the sentinel".  Pre-order walk carrying that right child down.
+// rope has 2n-1 entries (unified index).  Works for n = 1 (single leaf = node 0).
+void oracle_ropes(const int32_t* left, const int32_t* right, int64_t n, int32_t* rope) {
+  const int32_t leaf_base = (int32_t)(n - 1);
+  std::vector<std::pair<int32_t, int32_t>> stack;
+  stack.push_back({0, SENTINEL});
+  while (!stack.empty()) {
+    auto [node, r] = stack.back();
+    stack.pop_back();
+    rope[node] = r;
+    if (node < leaf_base) {
+      stack.push_back({right[node], r});           // right subtree inherits the rope
+      stack.push_back({left[node], right[node]});  // left subtree escapes to the right child
+    }
+  }
+}
+
+// P2.  Algorithm 2 with delta* read as the XOR magnitude of adjacent augmented
+// keys (G1): larger = less similar.  Comparing two XOR values of adjacent sorted pairs is done here
+// through their highest set bit (position in the 96-bit augmented key), an independent route from
+// the CUDA path's packed integer compare.
+void oracle_ropes_alg2(const uint64_t* sorted, const int32_t* first, const int32_t* last, int64_t n,
+                       int32_t* rope) {
+  (void)first;
+  const int32_t leaf_base = (int32_t)(n - 1);
+  auto dstar = [&](int64_t i) -> int {  // highest differing bit of k'_i, k'_{i+1}; 1000 = +inf
+    if (i < 0 || i >= n - 1) return 1000;
+    return highest_differing_bit(sorted[i], (uint32_t)i, sorted[i + 1], (uint32_t)(i + 1));
+  };
+  auto skip_for_right_bound = [&](int32_t e) -> int32_t {
+    if (e == n - 1) return SENTINEL;                        // Alg. 2 L1-2
+    const int32_t r = e + 1;                                // L4
+    if (dstar(r - 1) < dstar(r)) return leaf_base + r;      // L5-6  L_r
+    return r;                                               // L8    I_r
+  };
+  for (int32_t k = 0; k < n - 1; ++k) rope[k] = skip_for_right_bound(last[k]);
+  for (int32_t i = 0; i < n; ++i) rope[leaf_base + i] = skip_for_right_bound(i);
+}
+
+// D7.  aabb[node][6] = {lo.xyz, hi.xyz}.  Leaf (n-1)+i = box of primitive perm[i]; internal =
+// component-wise min / max of its two children, post-order.
+void oracle_boxes(const float* prim, int is_box, const uint32_t* perm, const int32_t* left,
+                  const int32_t* right, int64_t n, float* aabb) {
+  const int32_t leaf_base = (int32_t)(n - 1);
+  for (int64_t i = 0; i < n; ++i) {
+    Box b = prim_box(prim, perm[i], is_box);
+    for (int a = 0; a < 3; ++a) {
+      aabb[6 * (leaf_base + i) + a] = b.lo[a];
+      aabb[6 * (leaf_base + i) + 3 + a] = b.hi[a];
+    }
+  }
+  if (n < 2) return;
+  std::vector<std::pair<int32_t, int>> stack;  // (node, children_done)
+  stack.push_back({0, 0});
+  while (!stack.empty()) {
+    auto [node, done] = stack.back();
+    stack.pop_back();
+    if (!done) {
+      stack.push_back({node, 1});
+      if (right[node] < leaf_base) stack.push_back({right[node], 0});
+      if (left[node] < leaf_base) stack.push_back({left[node], 0});
+    } else {
+      const float* L = aabb + 6 * (int64_t)left[node];
+      const float* R = aabb + 6 * (int64_t)right[node];
+      float* O = aabb + 6 * (int64_t)node;
+      for (int a = 0; a < 3; ++a) {
+        O[a] = fmin2(L[a], R[a]);
+        O[3 + a] = fmax2(L[3 + a], R[3 + a]);
+      }
+    }
+  }
+}
+
+// Whole build, D1-D7.  Output arrays: sorted[n], perm[n], left_child[2n-1] (leaf entries = perm,
+// the leaf payload convention of the boundary), rope[2n-1], aabb[2n-1][6], scene6[6];
+// right_child[n-1] is oracle-private and optional (may be null).
+void oracle_build(const float* prim, int64_t n, int is_box, int bits, uint64_t* sorted,
+                  uint32_t* perm, int32_t* left_child, int32_t* rope, float* aabb, float* scene6,
+                  int32_t* right_child) {
+  if (n <= 0) return;
+  oracle_scene_bounds(prim, n, is_box, scene6);
+  std::vector<uint64_t> codes((size_t)n);
+  oracle_morton(prim, n, is_box, scene6, bits, codes.data());
+  oracle_sort(codes.data(), n, sorted, perm);
+  std::vector<int32_t> left((size_t)std::max<int64_t>(n - 1, 0)), right(left.size()),
+      first(left.size()), last(left.size());
+  if (n >= 2) oracle_hierarchy(sorted, n, left.data(), right.data(), first.data(), last.data());
+  oracle_ropes(left.data(), right.data(), n, rope);
+  oracle_boxes(prim, is_box, perm, left.data(), right.data(), n, aabb);
+  for (int64_t k = 0; k < n - 1; ++k) left_child[k] = left[(size_t)k];
+  for (int64_t i = 0; i < n; ++i) left_child[(n - 1) + i] = (int32_t)perm[i];
+  if (right_child)
+    for (int64_t k = 0; k < n - 1; ++k) right_child[k] = right[(size_t)k];
+}
+
+// ---- D8 queries ---------------------------------------------------------------------------------
+// Tree versions walk the oracle's own {left, right} tree with an explicit stack (the
+// technique the paper replaces) and report original primitive indices (leaf payload) in the order
+// found.  They return a handle; read it with oracle_result_*.
+
+static void* query_tree(int kind, const float* aabb, const int32_t* left_child,
+                        const int32_t* right_child, int64_t n, const float* queries, int64_t q) {
+  auto* res = new CsrResult();
+  res->offsets.assign((size_t)q + 1, 0);
+  const int32_t leaf_base = (int32_t)(n - 1);
+  std::vector<int32_t> stack;
+  for (int64_t j = 0; j < q; ++j) {
+    if (n > 0) {
+      stack.clear();
+      stack.push_back(0);
+      while (!stack.empty()) {
+        int32_t node = stack.back();
+        stack.pop_back();
+        const float* b = aabb + 6 * (int64_t)node;
+        bool hit;
+        if (kind == 0)
+          hit = sphere_hits_box(queries + 4 * j, queries[4 * j + 3], b, b + 3);
+        else
+          hit = box_hits_box(queries + 6 * j, queries + 6 * j + 3, b, b + 3);
+        if (!hit) continue;
+        if (node >= leaf_base) {
+          res->indices.push_back(left_child[node]);
+        } else {
+          stack.push_back(right_child[node]);
+          stack.push_back(left_child[node]);
+        }
+      }
+    }
+    res->offsets[(size_t)j + 1] = (int64_t)res->indices.size();
+  }
+  return res;
+}
+
+void* oracle_query_spheres_tree(const float* aabb, const int32_t* left_child,
+                                const int32_t* right_child, int64_t n, const float* xyzr, int64_t q) {
+  return query_tree(0, aabb, left_child, right_child, n, xyzr, q);
+}
+
+void* oracle_query_boxes_tree(const float* aabb, const int32_t* left_child,
+                              const int32_t* right_child, int64_t n, const float* minmax, int64_t q) {
+  return query_tree(1, aabb, left_child, right_child, n, minmax, q);
+}
+
+// Brute force: the plain definition of range search: every primitive is tested.
+// Reports original primitive indices in ascending order.
+static void* query_brute(int kind, const float* prim, int64_t n, int is_box, const float* queries,
+                         int64_t q) {
+  auto* res = new CsrResult();
+  res->offsets.assign((size_t)q + 1, 0);
+  for (int64_t j = 0; j < q; ++j) {
+    for (int64_t i = 0; i < n; ++i) {
+      Box b = prim_box(prim, i, is_box);
+      bool hit;
+      if (kind == 0)
+        hit = sphere_hits_box(queries + 4 * j, queries[4 * j + 3], b.lo, b.hi);
+      else
+        hit = box_hits_box(queries + 6 * j, queries + 6 * j + 3, b.lo, b.hi);
+      if (hit) res->indices.push_back((int32_t)i);
+    }
+    res->offsets[(size_t)j + 1] = (int64_t)res->indices.size();
+  }
+  return res;
+}
+
+void* oracle_query_spheres_brute(const float* prim, int64_t n, int is_box, const float* xyzr,
+                                 int64_t q) {
+  return query_brute(0, prim, n, is_box, xyzr, q);
+}
+
+void* oracle_query_boxes_brute(const float* prim, int64_t n, int is_box, const float* minmax,
+                               int64_t q) {
+  return query_brute(1, prim, n, is_box, minmax, q);
+}
+
+int64_t oracle_result_nnz(void* h) { return (int64_t) static_cast<CsrResult*>(h)->indices.size(); }
+
+void oracle_result_copy(void* h, int64_t* offsets, int32_t* indices) {
+  auto* r = static_cast<CsrResult*>(h);
+  std::memcpy(offsets, r->offsets.data(), r->offsets.size() * sizeof(int64_t));
+  if (!r->indices.empty())
+    std::memcpy(indices, r->indices.data(), r->indices.size() * sizeof(int32_t));
+}
+
+void oracle_result_free(void* h) { delete static_cast<CsrResult*>(h); }
+
+// Algorithm 1 (reading G3) run with an always-true predicate on a
+// {left_child, rope} hierarchy: writes the visit order (unified indices) and returns its length,
+// or -1 if more than max_visits nodes are visited (a cycle).  Used to check P3 on any hierarchy.
+int64_t oracle_walk_all(const int32_t* left_child, const int32_t* rope, int64_t n, int32_t* order,
+                        int64_t max_visits) {
+  if (n <= 0) return 0;
+  const int32_t leaf_base = (int32_t)(n - 1);
+  int64_t k = 0;
+  int32_t node = 0;
+  do {
+    if (k >= max_visits) return -1;
+    order[k++] = node;
+    node = (node >= leaf_base) ? rope[node] : left_child[node];
+  } while (node != SENTINEL);
+  return k;
+}
+
+}  // extern "C"
