@@ -1,0 +1,105 @@
+/* bvh_b200.h -- C ABI of libbvh_b200.so: linear-BVH construction with skip-connections in a single
+ * bottom-up pass, and stackless range queries, on one NVIDIA B200 (sm_100a).
+ *
+ * Method: "Revising Apetrei's bounding volume hierarchy construction algorithm to allow stackless
+ * traversal" (arXiv 2402.00665).  "PAPER.md:N" cites line N of the paper's text; "G#"/"D#" cite the
+ * readings and definitions listed in DESIGN.md where the paper is silent or garbled.
+ *
+ * Conventions for EVERY entry point
+ *  - All data pointers are DEVICE pointers (cudaMalloc / torch CUDA memory), 16-byte aligned, owned
+ *    by the caller.  The only host pointers are the `size_t*` outputs of the *_sizes functions.
+ *  - The library never allocates, frees or synchronises; it holds no global state and is re-entrant
+ *    across streams.  Every call only enqueues work on `stream` (a cudaStream_t passed as void*;
+ *    NULL = the legacy default stream) and returns.
+ *  - `scratch` of a build must stay alive until that build's stream work is complete; it also
+ *    holds the sorted codes and permutation that bvh_export reads.  `nodes` must stay alive until
+ *    the last query that uses it is complete.
+ *  - Return value: BVH_OK (0) or a negative BVH_ERR_* code.  Nothing is enqueued when an argument
+ *    check fails.  Asynchronous kernel faults surface at the caller's next synchronisation.
+ *  - Inputs must not contain NaN; radii must be >= 0; boxes must have min <= max.  Not checked.
+ *
+ * Node addressing (G8).  A hierarchy over n primitives has n leaves and n-1 internal nodes
+ * in ONE index space of 2n-1 nodes: internal node I_k -> k (k in [0, n-2], Karras
+ * numbering: siblings at consecutive indices, root = 0), leaf L_i -> (n-1)+i where
+ * i is the position in Morton order.  The sentinel is -1.  For n = 1 the single
+ * leaf is node 0.  `nodes` is an opaque array of (2n-1) 32-byte records
+ *     { float min[3]; int32 left_child;  float max[3]; int32 rope; }
+ * For an internal node `left_child` is its left child (PAPER.md:46 N_left); for a leaf it is the
+ * ORIGINAL index of the primitive stored there.  `rope` is the skip-connection N_skip.
+ */
+#ifndef BVH_B200_H
+#define BVH_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BVH_OK 0
+#define BVH_ERR_INVALID_ARGUMENT (-1) /* null pointer, negative count, misaligned pointer            */
+#define BVH_ERR_MORTON_BITS (-2)      /* morton_bits is not 30 or 63                                   */
+#define BVH_ERR_TOO_LARGE (-3)        /* n >= 2^30 (node indices and sort counters are 32-bit)         */
+#define BVH_ERR_SCRATCH (-4)          /* scratch_bytes smaller than bvh_sizes / bvh_scan_sizes report  */
+#define BVH_ERR_CUDA (-5)             /* a kernel launch failed (cudaGetLastError)                     */
+
+/* Library version, for the binding's sanity check. */
+int bvh_version(void);
+
+/* Bytes the caller must provide for a hierarchy over n primitives: node_bytes = 32*(2n-1) (32 when
+ * n = 0), scratch_bytes = codes + permutation ping-pong buffers, radix-sort histograms and tile
+ * status words, the `store` array of Algorithm 4 and the scene bounds.  Host call. */
+int bvh_sizes(int64_t n, int morton_bits, size_t* node_bytes, size_t* scratch_bytes);
+
+/* Build (PAPER.md:83-93 with steps 3-4 replaced by Algorithm 4).
+ *   1. scene bounds (D1)  2. Morton index of each primitive's centroid, 10 or 21 bits per axis (D2,
+ *   PAPER.md:85)  3. stable LSD radix sort of (code, index) (ties by index)
+ *   4. one bottom-up pass from the leaves that merges ranges through ATOMICCAS on `store`, numbers
+ *   each parent with its Karras index q, writes its left child and
+ *   skip-connection (Alg. 4 L21-26, Algorithm 2) and the union of its children's boxes (G10).
+ * xyz: n*3 floats (points; a point is the box min = max = point).  minmax: n*6 floats
+ * {min.xyz, max.xyz}.  n = 0 is valid and enqueues nothing.  Output: `nodes` (node_bytes). */
+int bvh_build_points(const float* xyz, int64_t n, int morton_bits, void* nodes, void* scratch,
+                     size_t scratch_bytes, void* stream);
+int bvh_build_boxes(const float* minmax, int64_t n, int morton_bits, void* nodes, void* scratch,
+                    size_t scratch_bytes, void* stream);
+
+/* Range search by Algorithm 1: stackless traversal over
+ * {left_child, rope}.  Count pass: counts[j] = number of primitives whose box satisfies query j.
+ * Sphere query {x,y,z,r}: squared distance from the centre to the box <= r*r, fp32 round-to-nearest,
+ * association of D8.  Box query {min.xyz,max.xyz}: closed-interval overlap on every axis (G12).
+ * q = 0 or n = 0: counts (if q > 0) are set to 0. */
+int bvh_query_spheres_count(const void* nodes, int64_t n, const float* xyzr, int64_t q,
+                            int32_t* counts, void* stream);
+int bvh_query_boxes_count(const void* nodes, int64_t n, const float* minmax, int64_t q,
+                          int32_t* counts, void* stream);
+
+/* Exclusive prefix sum of counts into 64-bit CSR offsets: offsets[0] = 0, offsets[q] = nnz (G21).
+ * bvh_scan_sizes is a host call giving the scratch the scan needs. */
+int bvh_scan_sizes(int64_t q, size_t* scratch_bytes);
+int bvh_scan_counts(const int32_t* counts, int64_t q, int64_t* offsets, void* scratch,
+                    size_t scratch_bytes, void* stream);
+
+/* Fill pass: the same traversal again; row j of the CSR, indices[offsets[j] .. offsets[j+1]), gets
+ * the ORIGINAL indices of the primitives hit, in traversal order (ascending Morton position; PAPER.md:56
+ * "Store the result").  The caller reads offsets[q] to size `indices` (the one device->host sync
+ * of the path, and it is the caller's). */
+int bvh_query_spheres_fill(const void* nodes, int64_t n, const float* xyzr, int64_t q,
+                           const int64_t* offsets, int32_t* indices, void* stream);
+int bvh_query_boxes_fill(const void* nodes, int64_t n, const float* minmax, int64_t q,
+                         const int64_t* offsets, int32_t* indices, void* stream);
+
+/* Parity export: the canonical arrays of a finished build, for bit-exact comparison.
+ * sorted_codes: uint32[n] when morton_bits = 30, uint64[n] when 63.  perm: uint32[n], original
+ * index at each Morton position.  left_child, rope: int32[2n-1].  aabb: float[2n-1][6]
+ * {min.xyz,max.xyz}.  scene_bounds: float[6].  Any output pointer may be NULL to skip it.
+ * `scratch` is the one the build used, untouched since. */
+int bvh_export(const void* nodes, const void* scratch, int64_t n, int morton_bits, void* sorted_codes,
+               uint32_t* perm, int32_t* left_child, int32_t* rope, float* aabb, float* scene_bounds,
+               void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BVH_B200_H */

@@ -1,0 +1,220 @@
+"""Thin Python binding over the C ABI of ``libbvh_b200.so`` (include/bvh_b200.h).
+
+Argument marshalling only: every function has the name and the argument list of its C entry point,
+takes torch CUDA tensors (device memory) and passes their ``data_ptr()`` plus the current torch CUDA
+stream.  No step of the path runs here.  There is NO CPU fallback: if the library is missing or
+cannot be loaded, every call raises.
+
+On top of the 1:1 functions, :class:`Bvh` and the ``query_*`` helpers chain the calls the way a user
+would (sizes -> allocate with torch -> build; count -> scan -> read nnz -> allocate -> fill).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import c_int, c_int64, c_size_t, c_void_p
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libbvh_b200.so")
+
+BVH_OK = 0
+ERRORS = {
+    -1: "BVH_ERR_INVALID_ARGUMENT",
+    -2: "BVH_ERR_MORTON_BITS",
+    -3: "BVH_ERR_TOO_LARGE",
+    -4: "BVH_ERR_SCRATCH",
+    -5: "BVH_ERR_CUDA",
+}
+
+# every symbol include/bvh_b200.h declares: (name, argtypes)
+_P = c_void_p
+SYMBOLS = {
+    "bvh_version": [],
+    "bvh_sizes": [c_int64, c_int, ctypes.POINTER(c_size_t), ctypes.POINTER(c_size_t)],
+    "bvh_build_points": [_P, c_int64, c_int, _P, _P, c_size_t, _P],
+    "bvh_build_boxes": [_P, c_int64, c_int, _P, _P, c_size_t, _P],
+    "bvh_query_spheres_count": [_P, c_int64, _P, c_int64, _P, _P],
+    "bvh_query_boxes_count": [_P, c_int64, _P, c_int64, _P, _P],
+    "bvh_scan_sizes": [c_int64, ctypes.POINTER(c_size_t)],
+    "bvh_scan_counts": [_P, c_int64, _P, _P, c_size_t, _P],
+    "bvh_query_spheres_fill": [_P, c_int64, _P, c_int64, _P, _P, _P],
+    "bvh_query_boxes_fill": [_P, c_int64, _P, c_int64, _P, _P, _P],
+    "bvh_export": [_P, _P, c_int64, c_int, _P, _P, _P, _P, _P, _P, _P],
+}
+
+
+class BvhError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """Load the C-ABI library (fails loudly if it has not been built: ``python -m paper_2402_00665_b200.build``)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise BvhError(f"{LIB_PATH} is missing: build it with `python -m paper_2402_00665_b200.build` "
+                           "(there is no CPU fallback)")
+        lib = ctypes.CDLL(LIB_PATH)
+        for name, argtypes in SYMBOLS.items():
+            fn = getattr(lib, name)
+            fn.argtypes = argtypes
+            fn.restype = c_int
+        _lib = lib
+    return _lib
+
+
+def _check(code: int, what: str) -> None:
+    if code != BVH_OK:
+        raise BvhError(f"{what} failed: {ERRORS.get(code, code)}")
+
+
+def _ptr(t: torch.Tensor | None) -> int | None:
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise BvhError("the C ABI takes device memory: pass CUDA tensors (there is no CPU path)")
+    if not t.is_contiguous():
+        raise BvhError("tensors must be contiguous")
+    return t.data_ptr()
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+# ---- 1:1 with the C ABI -------------------------------------------------------------------------------
+
+def bvh_version() -> int:
+    return load_library().bvh_version()
+
+
+def bvh_sizes(n: int, morton_bits: int) -> tuple[int, int]:
+    nb, sb = c_size_t(), c_size_t()
+    _check(load_library().bvh_sizes(n, morton_bits, ctypes.byref(nb), ctypes.byref(sb)), "bvh_sizes")
+    return nb.value, sb.value
+
+
+def bvh_build_points(xyz: torch.Tensor, n: int, morton_bits: int, nodes: torch.Tensor, scratch: torch.Tensor) -> None:
+    _check(load_library().bvh_build_points(_ptr(xyz), n, morton_bits, _ptr(nodes), _ptr(scratch),
+                                           scratch.numel() * scratch.element_size(), _stream()), "bvh_build_points")
+
+
+def bvh_build_boxes(minmax: torch.Tensor, n: int, morton_bits: int, nodes: torch.Tensor, scratch: torch.Tensor) -> None:
+    _check(load_library().bvh_build_boxes(_ptr(minmax), n, morton_bits, _ptr(nodes), _ptr(scratch),
+                                          scratch.numel() * scratch.element_size(), _stream()), "bvh_build_boxes")
+
+
+def bvh_query_spheres_count(nodes, n: int, xyzr, q: int, counts) -> None:
+    _check(load_library().bvh_query_spheres_count(_ptr(nodes), n, _ptr(xyzr), q, _ptr(counts), _stream()),
+           "bvh_query_spheres_count")
+
+
+def bvh_query_boxes_count(nodes, n: int, minmax, q: int, counts) -> None:
+    _check(load_library().bvh_query_boxes_count(_ptr(nodes), n, _ptr(minmax), q, _ptr(counts), _stream()),
+           "bvh_query_boxes_count")
+
+
+def bvh_scan_sizes(q: int) -> int:
+    sb = c_size_t()
+    _check(load_library().bvh_scan_sizes(q, ctypes.byref(sb)), "bvh_scan_sizes")
+    return sb.value
+
+
+def bvh_scan_counts(counts, q: int, offsets, scratch) -> None:
+    _check(load_library().bvh_scan_counts(_ptr(counts), q, _ptr(offsets), _ptr(scratch),
+                                          scratch.numel() * scratch.element_size(), _stream()), "bvh_scan_counts")
+
+
+def bvh_query_spheres_fill(nodes, n: int, xyzr, q: int, offsets, indices) -> None:
+    _check(load_library().bvh_query_spheres_fill(_ptr(nodes), n, _ptr(xyzr), q, _ptr(offsets), _ptr(indices),
+                                                 _stream()), "bvh_query_spheres_fill")
+
+
+def bvh_query_boxes_fill(nodes, n: int, minmax, q: int, offsets, indices) -> None:
+    _check(load_library().bvh_query_boxes_fill(_ptr(nodes), n, _ptr(minmax), q, _ptr(offsets), _ptr(indices),
+                                               _stream()), "bvh_query_boxes_fill")
+
+
+def bvh_export(nodes, scratch, n: int, morton_bits: int, sorted_codes=None, perm=None, left_child=None, rope=None,
+               aabb=None, scene_bounds=None) -> None:
+    _check(load_library().bvh_export(_ptr(nodes), _ptr(scratch), n, morton_bits, _ptr(sorted_codes), _ptr(perm),
+                                     _ptr(left_child), _ptr(rope), _ptr(aabb), _ptr(scene_bounds), _stream()),
+           "bvh_export")
+
+
+# ---- the calls chained as a user would ------------------------------------------------------------------
+
+class Bvh:
+    """Device buffers of one hierarchy: ``nodes`` (the product) and ``scratch`` (kept for :meth:`export`)."""
+
+    def __init__(self, n: int, morton_bits: int, device="cuda"):
+        self.n = int(n)
+        self.morton_bits = int(morton_bits)
+        node_bytes, scratch_bytes = bvh_sizes(self.n, self.morton_bits)
+        self.nodes = torch.empty(node_bytes, dtype=torch.uint8, device=device)
+        self.scratch = torch.empty(scratch_bytes, dtype=torch.uint8, device=device)
+        self.prim_kind = None
+
+    def build(self, prims: torch.Tensor) -> "Bvh":
+        """prims: float32 CUDA tensor [n,3] (points) or [n,6] (boxes).  Asynchronous on the current stream."""
+        if prims.dtype != torch.float32 or prims.dim() != 2 or prims.shape[0] != self.n or prims.shape[1] not in (3, 6):
+            raise BvhError(f"expected float32 [{self.n},3] or [{self.n},6], got {prims.dtype} {tuple(prims.shape)}")
+        if prims.shape[1] == 3:
+            bvh_build_points(prims, self.n, self.morton_bits, self.nodes, self.scratch)
+        else:
+            bvh_build_boxes(prims, self.n, self.morton_bits, self.nodes, self.scratch)
+        self.prim_kind = "points" if prims.shape[1] == 3 else "boxes"
+        return self
+
+    def export(self) -> dict[str, torch.Tensor]:
+        n, dev = self.n, self.nodes.device
+        m = max(2 * n - 1, 0)
+        out = {
+            "sorted_codes": torch.zeros(n, dtype=torch.int32 if self.morton_bits == 30 else torch.int64, device=dev),
+            "perm": torch.zeros(n, dtype=torch.int32, device=dev),
+            "left_child": torch.zeros(m, dtype=torch.int32, device=dev),
+            "rope": torch.zeros(m, dtype=torch.int32, device=dev),
+            "aabb": torch.zeros((m, 6), dtype=torch.float32, device=dev),
+            "scene_bounds": torch.zeros(6, dtype=torch.float32, device=dev),
+        }
+        bvh_export(self.nodes, self.scratch, n, self.morton_bits, **out)
+        return out
+
+
+class QueryWorkspace:
+    """Reusable device buffers for count-then-fill over up to ``q`` queries."""
+
+    def __init__(self, q: int, device="cuda"):
+        self.q = int(q)
+        self.counts = torch.empty(max(self.q, 1), dtype=torch.int32, device=device)
+        self.offsets = torch.empty(self.q + 1, dtype=torch.int64, device=device)
+        self.scan_scratch = torch.empty(max(bvh_scan_sizes(self.q), 8), dtype=torch.uint8, device=device)
+
+
+def query(bvh: Bvh, queries: torch.Tensor, ws: QueryWorkspace | None = None, indices: torch.Tensor | None = None):
+    """Range search.  queries: float32 CUDA [q,4] spheres {x,y,z,r} or [q,6] boxes {min,max}.
+
+    Returns (offsets int64[q+1], indices int32[nnz]) on the device.  Reads nnz back once (the path's only
+    device->host sync) unless ``indices`` is passed in with enough room."""
+    if queries.dtype != torch.float32 or queries.dim() != 2 or queries.shape[1] not in (4, 6):
+        raise BvhError(f"expected float32 [q,4] or [q,6], got {queries.dtype} {tuple(queries.shape)}")
+    q = int(queries.shape[0])
+    ws = ws or QueryWorkspace(q, queries.device)
+    spheres = queries.shape[1] == 4
+    count = bvh_query_spheres_count if spheres else bvh_query_boxes_count
+    fill = bvh_query_spheres_fill if spheres else bvh_query_boxes_fill
+    count(bvh.nodes, bvh.n, queries, q, ws.counts)
+    bvh_scan_counts(ws.counts, q, ws.offsets, ws.scan_scratch)
+    if indices is None:
+        nnz = int(ws.offsets[q].item())
+        indices = torch.empty(max(nnz, 1), dtype=torch.int32, device=queries.device)
+    else:
+        nnz = None
+    fill(bvh.nodes, bvh.n, queries, q, ws.offsets, indices)
+    offsets = ws.offsets[: q + 1]
+    return offsets, (indices if nnz is None else indices[:nnz])

@@ -1,0 +1,213 @@
+// bounds_morton.cu -- K1 scene bounds (D1) and K2 Morton encoding (D2) fused with the
+// digit histograms the one-sweep sort needs.  Both are single streaming passes over the input.
+#include "common.cuh"
+
+namespace bvh {
+
+// ---------------------------------------------------------------------------------------------------
+// K1.  The input is read as a flat float array with 128-bit loads, a warp covering 96 consecutive
+// float4 (1536 B) per step with lane-contiguous addresses.  The role of a scalar (which axis; for
+// boxes also min or max) is periodic in the flat index with period 3 (points) or 6 (boxes) floats, and
+// 96 float4 = 384 floats is a multiple of both, so each (load slot j, component c) of a lane always
+// sees the same role: 12 running mins and 12 running maxes per thread, sorted into axes once at the
+// end.  Then warp shuffles, one shared-memory step per block, and one atomicMax per block and bound
+// on the order-preserving uint image of the float (min is kept as ~ord so that everything is a max
+// and the zero-initialised header is the identity).
+// ---------------------------------------------------------------------------------------------------
+constexpr int kBoundsThreads = 256;
+
+__device__ __forceinline__ void fold_role(int role, bool is_box, float mn, float mx, float lo[3], float hi[3]) {
+  // role: flat index modulo 6.  points: axis = role % 3, both bounds.  boxes: role < 3 -> min of axis role,
+  // else max of axis role - 3.
+  const int axis = role % 3;
+  const bool use_min = !is_box || role < 3;
+  const bool use_max = !is_box || role >= 3;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    if (axis == a) {
+      if (use_min) lo[a] = fminf(lo[a], mn);
+      if (use_max) hi[a] = fmaxf(hi[a], mx);
+    }
+  }
+}
+
+__global__ void __launch_bounds__(kBoundsThreads) scene_bounds_kernel(const float* __restrict__ prim, int64_t nfloats,
+                                                                      bool is_box, Header* __restrict__ header) {
+  const float inf = __int_as_float(0x7f800000);
+  float mn[3][4], mx[3][4];
+#pragma unroll
+  for (int j = 0; j < 3; ++j)
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      mn[j][c] = inf;
+      mx[j][c] = -inf;
+    }
+  const int lane = threadIdx.x & 31;
+  const int64_t warp_global = ((int64_t)blockIdx.x * kBoundsThreads + threadIdx.x) >> 5;
+  const int64_t num_warps = ((int64_t)gridDim.x * kBoundsThreads) >> 5;
+  const int64_t nvec = nfloats >> 2;          // whole float4s
+  const int64_t nchunks = nvec / 96;          // whole 96-float4 chunks
+  const float4* __restrict__ v = reinterpret_cast<const float4*>(prim);
+  for (int64_t ch = warp_global; ch < nchunks; ch += num_warps) {
+    const float4* p = v + ch * 96 + lane;
+    float4 x[3];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) x[j] = __ldcs(p + j * 32);   // streaming: read exactly once
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      mn[j][0] = fminf(mn[j][0], x[j].x); mx[j][0] = fmaxf(mx[j][0], x[j].x);
+      mn[j][1] = fminf(mn[j][1], x[j].y); mx[j][1] = fmaxf(mx[j][1], x[j].y);
+      mn[j][2] = fminf(mn[j][2], x[j].z); mx[j][2] = fmaxf(mx[j][2], x[j].z);
+      mn[j][3] = fminf(mn[j][3], x[j].w); mx[j][3] = fmaxf(mx[j][3], x[j].w);
+    }
+  }
+  float lo[3] = {inf, inf, inf}, hi[3] = {-inf, -inf, -inf};
+#pragma unroll
+  for (int j = 0; j < 3; ++j)
+#pragma unroll
+    for (int c = 0; c < 4; ++c) fold_role((4 * (j * 32 + lane) + c) % 6, is_box, mn[j][c], mx[j][c], lo, hi);
+  // tail: scalars after the last whole chunk
+  const int64_t tail0 = nchunks * 96 * 4;
+  for (int64_t e = tail0 + (int64_t)blockIdx.x * kBoundsThreads + threadIdx.x; e < nfloats;
+       e += (int64_t)gridDim.x * kBoundsThreads) {
+    const float f = prim[e];
+    fold_role((int)(e % 6), is_box, f, f, lo, hi);
+  }
+  // warp reduce
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+      lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], off));
+      hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], off));
+    }
+  }
+  __shared__ float s[kBoundsThreads / 32][6];
+  const int warp = threadIdx.x >> 5;
+  if (lane == 0) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      s[warp][a] = lo[a];
+      s[warp][3 + a] = hi[a];
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < 6) {
+    float r = s[0][threadIdx.x];
+    for (int w = 1; w < kBoundsThreads / 32; ++w)
+      r = (threadIdx.x < 3) ? fminf(r, s[w][threadIdx.x]) : fmaxf(r, s[w][threadIdx.x]);
+    // canonical zero: -0.0 and +0.0 compare equal for fminf/fmaxf; inputs carry no -0.0 (G19)
+    const uint32_t o = float_to_ordered(r);
+    atomicMax(&header->bounds_enc[threadIdx.x], threadIdx.x < 3 ? ~o : o);
+  }
+}
+
+void launch_scene_bounds(const float* prim, int n, bool is_box, Header* header, cudaStream_t stream) {
+  const int64_t nfloats = (int64_t)n * (is_box ? 6 : 3);
+  const int64_t chunks = nfloats / (96 * 4);
+  int64_t blocks = (chunks + (kBoundsThreads / 32) - 1) / (kBoundsThreads / 32);
+  const int64_t cap = (int64_t)kNumSMs * 8;
+  if (blocks > cap) blocks = cap;
+  if (blocks < 1) blocks = 1;
+  scene_bounds_kernel<<<(unsigned)blocks, kBoundsThreads, 0, stream>>>(prim, nfloats, is_box, header);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// K2.  One thread per primitive.  D2: centroid c = (min + max) * 0.5, t = (c - lo) / (hi - lo) (0 when
+// the extent is 0), cell = min(trunc(t * 2^b), 2^b - 1), all fp32 round-to-nearest with explicit
+// intrinsics so that nvcc cannot contract them.  Bits are spread with magic-number masks; x is the
+// most significant axis of each triple.  The same pass accumulates the 256-bin histogram of every
+// 8-bit digit of the code in shared memory and flushes it with one global atomic per non-empty bin
+// and block: the sort then needs no histogram pass of its own.
+// ---------------------------------------------------------------------------------------------------
+constexpr int kMortonThreads = 256;
+
+__device__ __forceinline__ uint32_t spread10(uint32_t x) {
+  x = (x | (x << 16)) & 0x030000FFu;
+  x = (x | (x << 8)) & 0x0300F00Fu;
+  x = (x | (x << 4)) & 0x030C30C3u;
+  x = (x | (x << 2)) & 0x09249249u;
+  return x;
+}
+__device__ __forceinline__ uint64_t spread21(uint32_t v) {
+  uint64_t x = v & 0x1fffffu;
+  x = (x | (x << 32)) & 0x001f00000000ffffull;
+  x = (x | (x << 16)) & 0x001f0000ff0000ffull;
+  x = (x | (x << 8)) & 0x100f00f00f00f00full;
+  x = (x | (x << 4)) & 0x10c30c30c30c30c3ull;
+  x = (x | (x << 2)) & 0x1249249249249249ull;
+  return x;
+}
+
+__device__ __forceinline__ uint32_t quantise(float lo, float hi, float slo, float shi, float scale, uint32_t cell_max) {
+  const float c = __fmul_rn(__fadd_rn(lo, hi), 0.5f);
+  const float e = __fsub_rn(shi, slo);
+  float t = 0.0f;
+  if (e > 0.0f) t = __fdiv_rn(__fsub_rn(c, slo), e);
+  const uint32_t q = __float2uint_rz(__fmul_rn(t, scale));
+  return min(q, cell_max);
+}
+
+template <typename KeyT, int PASSES, bool IS_BOX>
+__global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __restrict__ prim, int n,
+                                                                const Header* __restrict__ header,
+                                                                KeyT* __restrict__ codes, uint32_t* __restrict__ hist) {
+  __shared__ uint32_t s_hist[PASSES * 256];
+  for (int i = threadIdx.x; i < PASSES * 256; i += kMortonThreads) s_hist[i] = 0;
+  float scene[6];
+  load_scene_bounds(header, scene);
+  __syncthreads();
+  constexpr int B = (sizeof(KeyT) == 4) ? 10 : 21;
+  const float scale = (float)(1u << B);
+  const uint32_t cell_max = (1u << B) - 1u;
+  for (int64_t i = (int64_t)blockIdx.x * kMortonThreads + threadIdx.x; i < n; i += (int64_t)gridDim.x * kMortonThreads) {
+    float lo[3], hi[3];
+    if (IS_BOX) {
+      const float2* p = reinterpret_cast<const float2*>(prim + 6 * i);
+      const float2 a = __ldcs(p), b = __ldcs(p + 1), c = __ldcs(p + 2);
+      lo[0] = a.x; lo[1] = a.y; lo[2] = b.x; hi[0] = b.y; hi[1] = c.x; hi[2] = c.y;
+    } else {
+      const float* p = prim + 3 * i;
+      lo[0] = hi[0] = __ldcs(p);
+      lo[1] = hi[1] = __ldcs(p + 1);
+      lo[2] = hi[2] = __ldcs(p + 2);
+    }
+    uint32_t cell[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) cell[a] = quantise(lo[a], hi[a], scene[a], scene[3 + a], scale, cell_max);
+    KeyT code;
+    if (sizeof(KeyT) == 4)
+      code = (KeyT)((spread10(cell[0]) << 2) | (spread10(cell[1]) << 1) | spread10(cell[2]));
+    else
+      code = (KeyT)((spread21(cell[0]) << 2) | (spread21(cell[1]) << 1) | spread21(cell[2]));
+    codes[i] = code;
+#pragma unroll
+    for (int p = 0; p < PASSES; ++p) atomicAdd(&s_hist[p * 256 + (int)((code >> (8 * p)) & 0xFF)], 1u);
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < PASSES * 256; i += kMortonThreads) {
+    const uint32_t c = s_hist[i];
+    if (c) atomicAdd(&hist[i], c);
+  }
+}
+
+void launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
+                   uint32_t* hist, cudaStream_t stream) {
+  int64_t blocks = ((int64_t)n + kMortonThreads - 1) / kMortonThreads;
+  const int64_t cap = (int64_t)kNumSMs * 8;
+  if (blocks > cap) blocks = cap;
+  const unsigned g = (unsigned)blocks;
+  if (morton_bits == 30) {
+    if (is_box)
+      morton_kernel<uint32_t, 4, true><<<g, kMortonThreads, 0, stream>>>(prim, n, header, (uint32_t*)codes, hist);
+    else
+      morton_kernel<uint32_t, 4, false><<<g, kMortonThreads, 0, stream>>>(prim, n, header, (uint32_t*)codes, hist);
+  } else {
+    if (is_box)
+      morton_kernel<uint64_t, 8, true><<<g, kMortonThreads, 0, stream>>>(prim, n, header, (uint64_t*)codes, hist);
+    else
+      morton_kernel<uint64_t, 8, false><<<g, kMortonThreads, 0, stream>>>(prim, n, header, (uint64_t*)codes, hist);
+  }
+}
+
+}  // namespace bvh

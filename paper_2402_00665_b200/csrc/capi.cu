@@ -1,0 +1,217 @@
+// capi.cu -- the C ABI declared in include/bvh_b200.h: argument checks, scratch layout, and the
+// sequence of kernel launches of one build / one query pass.  No allocation, no synchronisation.
+#include "../../include/bvh_b200.h"
+#include "common.cuh"
+
+namespace bvh {
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+ScratchLayout scratch_layout(int64_t n, int morton_bits) {
+  ScratchLayout L{};
+  L.key_bytes = (morton_bits == 30) ? 4 : 8;
+  L.passes = (morton_bits == 30) ? 4 : 8;
+  const int tile = sort_tile_items(L.key_bytes);
+  L.tiles = (int)((n + tile - 1) / tile);
+  if (L.tiles < 1) L.tiles = 1;
+  size_t off = 0;
+  L.header = off;
+  off += sizeof(Header);
+  L.hist = off;
+  off += align_up((size_t)L.passes * 256 * sizeof(uint32_t), 256);
+  L.status = off;
+  off += align_up((size_t)L.passes * L.tiles * 256 * sizeof(uint32_t), 256);
+  L.zero_bytes = off;
+  const size_t nn = (size_t)(n > 0 ? n : 1);
+  L.store = off;
+  off += align_up(nn * sizeof(int32_t), 256);
+  for (int b = 0; b < 2; ++b) {
+    L.keys[b] = off;
+    off += align_up(nn * L.key_bytes, 256);
+  }
+  for (int b = 0; b < 2; ++b) {
+    L.vals[b] = off;
+    off += align_up(nn * sizeof(uint32_t), 256);
+  }
+  L.total = off;
+  return L;
+}
+
+// ---- parity export ------------------------------------------------------------------------------------
+template <typename KeyT>
+__global__ void export_kernel(const Node* __restrict__ nodes, const KeyT* __restrict__ keys,
+                              const uint32_t* __restrict__ vals, const Header* __restrict__ header, int n,
+                              KeyT* sorted_codes, uint32_t* perm, int32_t* left_child, int32_t* rope, float* aabb,
+                              float* scene_bounds) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t total = 2 * (int64_t)n - 1;
+  if (i < n) {
+    if (sorted_codes) sorted_codes[i] = keys[i];
+    if (perm) perm[i] = vals[i];
+  }
+  if (i < total) {
+    const float4 lo = nodes[i].lo, hi = nodes[i].hi;
+    if (left_child) left_child[i] = __float_as_int(lo.w);
+    if (rope) rope[i] = __float_as_int(hi.w);
+    if (aabb) {
+      float* o = aabb + 6 * i;
+      o[0] = lo.x; o[1] = lo.y; o[2] = lo.z; o[3] = hi.x; o[4] = hi.y; o[5] = hi.z;
+    }
+  }
+  if (i == 0 && scene_bounds) {
+    float s[6];
+    load_scene_bounds(header, s);
+    for (int a = 0; a < 6; ++a) scene_bounds[a] = s[a];
+  }
+}
+
+void launch_export(const Node* nodes, const void* scratch, const ScratchLayout& L, int n, void* sorted_codes,
+                   uint32_t* perm, int32_t* left_child, int32_t* rope, float* aabb, float* scene_bounds,
+                   cudaStream_t stream) {
+  const char* base = static_cast<const char*>(scratch);
+  const Header* header = reinterpret_cast<const Header*>(base + L.header);
+  const uint32_t* vals = reinterpret_cast<const uint32_t*>(base + L.vals[0]);
+  const int64_t total = 2 * (int64_t)n - 1;
+  const unsigned g = (unsigned)((total + 255) / 256);
+  if (L.key_bytes == 4)
+    export_kernel<uint32_t><<<g, 256, 0, stream>>>(nodes, reinterpret_cast<const uint32_t*>(base + L.keys[0]), vals,
+                                                   header, n, (uint32_t*)sorted_codes, perm, left_child, rope, aabb,
+                                                   scene_bounds);
+  else
+    export_kernel<uint64_t><<<g, 256, 0, stream>>>(nodes, reinterpret_cast<const uint64_t*>(base + L.keys[0]), vals,
+                                                   header, n, (uint64_t*)sorted_codes, perm, left_child, rope, aabb,
+                                                   scene_bounds);
+}
+
+__global__ void zero_counts_kernel(int32_t* counts, int64_t q) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < q) counts[i] = 0;
+}
+
+static inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+static int check_launch() { return cudaGetLastError() == cudaSuccess ? BVH_OK : BVH_ERR_CUDA; }
+
+static int build(const float* prim, bool is_box, int64_t n, int morton_bits, void* nodes, void* scratch,
+                 size_t scratch_bytes, void* stream_) {
+  if (n < 0) return BVH_ERR_INVALID_ARGUMENT;
+  if (morton_bits != 30 && morton_bits != 63) return BVH_ERR_MORTON_BITS;
+  if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
+  if (n == 0) return BVH_OK;
+  if (!prim || !nodes || !scratch) return BVH_ERR_INVALID_ARGUMENT;
+  if (misaligned(prim) || misaligned(nodes) || misaligned(scratch)) return BVH_ERR_INVALID_ARGUMENT;
+  if ((reinterpret_cast<uintptr_t>(nodes) & 31u) != 0) return BVH_ERR_INVALID_ARGUMENT;
+  const ScratchLayout L = scratch_layout(n, morton_bits);
+  if (scratch_bytes < L.total) return BVH_ERR_SCRATCH;
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  char* base = static_cast<char*>(scratch);
+  Header* header = reinterpret_cast<Header*>(base + L.header);
+  uint32_t* hist = reinterpret_cast<uint32_t*>(base + L.hist);
+  int* store = reinterpret_cast<int*>(base + L.store);
+
+  if (cudaMemsetAsync(base, 0, L.zero_bytes, stream) != cudaSuccess) return BVH_ERR_CUDA;
+  if (cudaMemsetAsync(store, 0xFF, (size_t)n * sizeof(int), stream) != cudaSuccess) return BVH_ERR_CUDA;
+  launch_scene_bounds(prim, (int)n, is_box, header, stream);
+  launch_morton(prim, (int)n, is_box, morton_bits, header, base + L.keys[0], hist, stream);
+  launch_sort(scratch, L, (int)n, stream);
+  launch_hierarchy(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
+                   store, static_cast<Node*>(nodes), (int)n, stream);
+  return check_launch();
+}
+
+static int query(const void* nodes, int64_t n, const float* queries, int64_t q, int kind, bool fill, int32_t* counts,
+                 const int64_t* offsets, int32_t* indices, void* stream_) {
+  if (n < 0 || q < 0) return BVH_ERR_INVALID_ARGUMENT;
+  if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
+  if (q == 0) return BVH_OK;
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (fill) {
+    if (!offsets) return BVH_ERR_INVALID_ARGUMENT;
+  } else {
+    if (!counts) return BVH_ERR_INVALID_ARGUMENT;
+  }
+  if (n == 0) {
+    if (!fill) {
+      zero_counts_kernel<<<(unsigned)((q + 255) / 256), 256, 0, stream>>>(counts, q);
+      return check_launch();
+    }
+    return BVH_OK;
+  }
+  if (!nodes || !queries || misaligned(nodes) || misaligned(queries)) return BVH_ERR_INVALID_ARGUMENT;
+  if (fill && !indices) return BVH_ERR_INVALID_ARGUMENT;  // nnz = 0 callers still pass a valid pointer
+  launch_traverse(static_cast<const Node*>(nodes), (int)n, queries, q, kind, fill, counts, offsets, indices, stream);
+  return check_launch();
+}
+
+}  // namespace bvh
+
+extern "C" {
+
+int bvh_version(void) { return 1; }
+
+int bvh_sizes(int64_t n, int morton_bits, size_t* node_bytes, size_t* scratch_bytes) {
+  if (n < 0 || !node_bytes || !scratch_bytes) return BVH_ERR_INVALID_ARGUMENT;
+  if (morton_bits != 30 && morton_bits != 63) return BVH_ERR_MORTON_BITS;
+  if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
+  *node_bytes = (n > 0) ? sizeof(bvh::Node) * (size_t)(2 * n - 1) : sizeof(bvh::Node);
+  *scratch_bytes = bvh::scratch_layout(n, morton_bits).total;
+  return BVH_OK;
+}
+
+int bvh_build_points(const float* xyz, int64_t n, int morton_bits, void* nodes, void* scratch, size_t scratch_bytes,
+                     void* stream) {
+  return bvh::build(xyz, false, n, morton_bits, nodes, scratch, scratch_bytes, stream);
+}
+
+int bvh_build_boxes(const float* minmax, int64_t n, int morton_bits, void* nodes, void* scratch, size_t scratch_bytes,
+                    void* stream) {
+  return bvh::build(minmax, true, n, morton_bits, nodes, scratch, scratch_bytes, stream);
+}
+
+int bvh_query_spheres_count(const void* nodes, int64_t n, const float* xyzr, int64_t q, int32_t* counts, void* stream) {
+  return bvh::query(nodes, n, xyzr, q, 0, false, counts, nullptr, nullptr, stream);
+}
+
+int bvh_query_boxes_count(const void* nodes, int64_t n, const float* minmax, int64_t q, int32_t* counts, void* stream) {
+  return bvh::query(nodes, n, minmax, q, 1, false, counts, nullptr, nullptr, stream);
+}
+
+int bvh_scan_sizes(int64_t q, size_t* scratch_bytes) {
+  if (q < 0 || !scratch_bytes) return BVH_ERR_INVALID_ARGUMENT;
+  *scratch_bytes = bvh::scan_scratch_bytes(q);
+  return BVH_OK;
+}
+
+int bvh_scan_counts(const int32_t* counts, int64_t q, int64_t* offsets, void* scratch, size_t scratch_bytes,
+                    void* stream) {
+  if (q < 0 || !offsets) return BVH_ERR_INVALID_ARGUMENT;
+  if (q > 0 && (!counts || !scratch)) return BVH_ERR_INVALID_ARGUMENT;
+  if (q > 0 && scratch_bytes < bvh::scan_scratch_bytes(q)) return BVH_ERR_SCRATCH;
+  bvh::launch_scan(counts, q, offsets, scratch, static_cast<cudaStream_t>(stream));
+  return bvh::check_launch();
+}
+
+int bvh_query_spheres_fill(const void* nodes, int64_t n, const float* xyzr, int64_t q, const int64_t* offsets,
+                           int32_t* indices, void* stream) {
+  return bvh::query(nodes, n, xyzr, q, 0, true, nullptr, offsets, indices, stream);
+}
+
+int bvh_query_boxes_fill(const void* nodes, int64_t n, const float* minmax, int64_t q, const int64_t* offsets,
+                         int32_t* indices, void* stream) {
+  return bvh::query(nodes, n, minmax, q, 1, true, nullptr, offsets, indices, stream);
+}
+
+int bvh_export(const void* nodes, const void* scratch, int64_t n, int morton_bits, void* sorted_codes, uint32_t* perm,
+               int32_t* left_child, int32_t* rope, float* aabb, float* scene_bounds, void* stream) {
+  if (n < 0) return BVH_ERR_INVALID_ARGUMENT;
+  if (morton_bits != 30 && morton_bits != 63) return BVH_ERR_MORTON_BITS;
+  if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
+  if (n == 0) return BVH_OK;
+  if (!nodes || !scratch) return BVH_ERR_INVALID_ARGUMENT;
+  const bvh::ScratchLayout L = bvh::scratch_layout(n, morton_bits);
+  bvh::launch_export(static_cast<const bvh::Node*>(nodes), scratch, L, (int)n, sorted_codes, perm, left_child, rope,
+                     aabb, scene_bounds, static_cast<cudaStream_t>(stream));
+  return bvh::check_launch();
+}
+
+}  // extern "C"

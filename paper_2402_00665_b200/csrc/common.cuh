@@ -1,0 +1,95 @@
+// common.cuh -- shared declarations of the CUDA path (sm_100a only).
+// Nothing in this directory is shared with, or included by, oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace bvh {
+
+constexpr int kSentinel = -1;   // the paper's sentinel node; reading G9
+constexpr int kInvalid = -1;    // the paper's "invalid entry value (e.g., -1)" in `store`
+constexpr int kNumSMs = 148;    // B200
+
+// 32-byte node record, read and written as two float4 (one 32-byte sector per node visit).
+//   lo = {min.x, min.y, min.z, bitcast(left_child)}   hi = {max.x, max.y, max.z, bitcast(rope)}
+struct __align__(32) Node {
+  float4 lo;
+  float4 hi;
+};
+
+// ---- scratch layout of one build (offsets in bytes from the caller's scratch pointer) ---------------
+struct ScratchLayout {
+  size_t header;        // Header (below)
+  size_t hist;          // uint32 [passes][256]   global digit histograms
+  size_t status;        // uint32 [passes][tiles][256]  onesweep tile status words
+  size_t zero_bytes;    // header + hist + status are contiguous from 0 and zero-initialised per build
+  size_t store;         // int32 [n]  Algorithm 4's `store` (n-1 used), initialised to -1
+  size_t keys[2];       // KeyT [n]   ping-pong; sorted codes end in keys[0]
+  size_t vals[2];       // uint32 [n] ping-pong; permutation ends in vals[0]
+  size_t total;
+  int passes;
+  int tiles;
+  int key_bytes;
+};
+
+struct Header {
+  uint32_t bounds_enc[8];    // [0..2] = ~ord(min.xyz), [3..5] = ord(max.xyz), maximised with atomicMax
+  uint32_t tile_counter[8];  // one dynamic tile counter per sort pass
+  uint32_t pad[48];
+};
+static_assert(sizeof(Header) == 256, "header is one 256-byte block");
+
+ScratchLayout scratch_layout(int64_t n, int morton_bits);
+int sort_tile_items(int key_bytes);
+
+// ---- order-preserving float <-> uint map (float atomic min/max through atomicMax on uint) ---------
+__host__ __device__ inline uint32_t float_to_ordered(float f) {
+#ifdef __CUDA_ARCH__
+  uint32_t b = __float_as_uint(f);
+#else
+  union { float f; uint32_t u; } c; c.f = f; uint32_t b = c.u;
+#endif
+  return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__host__ __device__ inline float ordered_to_float(uint32_t o) {
+  uint32_t b = (o & 0x80000000u) ? (o & 0x7fffffffu) : ~o;
+#ifdef __CUDA_ARCH__
+  return __uint_as_float(b);
+#else
+  union { float f; uint32_t u; } c; c.u = b; return c.f;
+#endif
+}
+
+// Scene bounds decoded from the header: {min.xyz, max.xyz}.
+__device__ inline void load_scene_bounds(const Header* h, float out[6]) {
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    out[a] = ordered_to_float(~h->bounds_enc[a]);
+    out[3 + a] = ordered_to_float(h->bounds_enc[3 + a]);
+  }
+}
+
+// ---- kernel launchers (each only enqueues on `stream`) -----------------------------------------------
+// K1: scene bounds.  is_box: prim is n*6 floats, else n*3.
+void launch_scene_bounds(const float* prim, int n, bool is_box, Header* header, cudaStream_t stream);
+// K2: Morton codes + the digit histograms of every sort pass.
+void launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
+                   uint32_t* hist, cudaStream_t stream);
+// K3: one-sweep LSD radix sort, all passes.  Result in keys[0] / vals[0] of the layout.
+void launch_sort(void* scratch, const ScratchLayout& L, int n, cudaStream_t stream);
+// K4+K5: leaf gather + modified Apetrei bottom-up pass (Algorithm 4 with boxes).
+void launch_hierarchy(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
+                      int* store, Node* nodes, int n, cudaStream_t stream);
+// K6/K8: stackless traversal.  kind 0 = spheres (xyzr), 1 = boxes (minmax).  fill: offsets/indices used.
+void launch_traverse(const Node* nodes, int n, const float* queries, int64_t q, int kind, bool fill, int32_t* counts,
+                     const int64_t* offsets, int32_t* indices, cudaStream_t stream);
+// K7: exclusive scan of int32 counts into int64 offsets[q+1].
+size_t scan_scratch_bytes(int64_t q);
+void launch_scan(const int32_t* counts, int64_t q, int64_t* offsets, void* scratch, cudaStream_t stream);
+// Parity export.
+void launch_export(const Node* nodes, const void* scratch, const ScratchLayout& L, int n, void* sorted_codes,
+                   uint32_t* perm, int32_t* left_child, int32_t* rope, float* aabb, float* scene_bounds,
+                   cudaStream_t stream);
+
+}  // namespace bvh

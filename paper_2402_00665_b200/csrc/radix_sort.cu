@@ -1,0 +1,220 @@
+// radix_sort.cu -- K3: in-house one-sweep LSD radix sort of (Morton code, index) pairs (
+// stable, so equal codes keep ascending original index: PAPER.md:172 / reading G6).
+//
+// One kernel per 8-bit digit.  Each pass reads every pair once and writes it once: a tile's position
+// in the output is known inside the pass through a chained scan with decoupled look-back over
+// per-tile digit counts, so there is no separate scan or per-pass histogram kernel (the global digit
+// histograms come from the Morton kernel).  Tiles take their id from an atomic ticket, so a tile
+// only ever waits on tiles that are already running: forward progress without co-residency
+// assumptions.
+//
+// Inside a tile: warp w owns a contiguous run of 32*ITEMS pairs, item j of lane l at offset j*32+l
+// (coalesced loads; tile order = (warp, item, lane)).  Ranks come from __match_any_sync on the digit
+// plus a per-warp 256-bin counter array in shared memory, which keeps the order of equal digits =
+// stability.  Keys and values are then permuted through shared memory into tile-sorted order and
+// written out in runs of equal digit, i.e. coalesced.
+#include "common.cuh"
+
+namespace bvh {
+
+constexpr int kSortThreads = 256;
+constexpr int kSortWarps = kSortThreads / 32;
+constexpr uint32_t kFlagPartial = 1u << 30;
+constexpr uint32_t kFlagInclusive = 2u << 30;
+constexpr uint32_t kValueMask = (1u << 30) - 1u;
+
+template <typename KeyT>
+struct SortCfg {
+  static constexpr int ITEMS = (sizeof(KeyT) == 4) ? 16 : 12;
+  static constexpr int TILE = kSortThreads * ITEMS;
+};
+
+int sort_tile_items(int key_bytes) { return key_bytes == 4 ? SortCfg<uint32_t>::TILE : SortCfg<uint64_t>::TILE; }
+
+__device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ void st_volatile_u32(uint32_t* p, uint32_t v) {
+  asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+template <typename KeyT, bool IOTA>
+__global__ void __launch_bounds__(kSortThreads, 3)
+onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_out, const uint32_t* __restrict__ vals_in,
+                     uint32_t* __restrict__ vals_out, const uint32_t* __restrict__ hist, uint32_t* status,
+                     uint32_t* tile_counter, int n, int shift) {
+  constexpr int ITEMS = SortCfg<KeyT>::ITEMS;
+  constexpr int TILE = SortCfg<KeyT>::TILE;
+  __shared__ uint32_t s_warp_hist[kSortWarps][256];
+  __shared__ uint32_t s_tile_excl[256];      // first tile-sorted position of each digit
+  __shared__ int64_t s_digit_base[256];      // global position of tile-sorted position 0 of each digit
+  __shared__ uint32_t s_scan[kSortWarps];
+  __shared__ uint32_t s_tile;
+  __shared__ KeyT s_keys[TILE];
+  __shared__ uint32_t s_vals[TILE];
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) s_tile = atomicAdd(tile_counter, 1u);
+  for (int i = tid; i < kSortWarps * 256; i += kSortThreads) (&s_warp_hist[0][0])[i] = 0;
+  __syncthreads();
+  const uint32_t tile = s_tile;
+  const int64_t tile_base = (int64_t)tile * TILE;
+  const int valid_in_tile = (int)min((int64_t)TILE, (int64_t)n - tile_base);
+
+  // ---- load (coalesced; warp-contiguous runs) -------------------------------------------------------
+  KeyT key[ITEMS];
+  uint32_t val[ITEMS];
+  const int warp_off = warp * 32 * ITEMS + lane;
+#pragma unroll
+  for (int j = 0; j < ITEMS; ++j) {
+    const int t = warp_off + j * 32;
+    if (t < valid_in_tile) {
+      key[j] = keys_in[tile_base + t];
+      val[j] = IOTA ? (uint32_t)(tile_base + t) : vals_in[tile_base + t];
+    } else {
+      key[j] = 0;
+      val[j] = 0;
+    }
+  }
+
+  // ---- rank within the warp, in tile order ---------------------------------------------------------------
+  uint32_t rank[ITEMS];
+  const uint32_t lt_mask = (1u << lane) - 1u;
+#pragma unroll
+  for (int j = 0; j < ITEMS; ++j) {
+    const bool valid = (warp_off + j * 32) < valid_in_tile;
+    const uint32_t vm = __ballot_sync(0xffffffffu, valid);
+    if (valid) {
+      const uint32_t d = (uint32_t)(key[j] >> shift) & 0xFFu;
+      const uint32_t peers = __match_any_sync(vm, d);
+      const int leader = __ffs(peers) - 1;
+      uint32_t pre = 0;
+      if (lane == leader) {
+        pre = s_warp_hist[warp][d];
+        s_warp_hist[warp][d] = pre + __popc(peers);
+      }
+      pre = __shfl_sync(peers, pre, leader);
+      rank[j] = pre + __popc(peers & lt_mask);
+    }
+    __syncwarp();
+  }
+  __syncthreads();
+
+  // ---- per digit: exclusive scan over warps, publish tile count, look back -----------------------------------
+  // kSortThreads == 256: thread d owns digit d.
+  uint32_t tile_count = 0;
+  {
+#pragma unroll
+    for (int w = 0; w < kSortWarps; ++w) {
+      const uint32_t c = s_warp_hist[w][tid];
+      s_warp_hist[w][tid] = tile_count;
+      tile_count += c;
+    }
+  }
+  uint32_t* my_status = status + (size_t)tile * 256 + tid;
+  st_volatile_u32(my_status, (tile == 0 ? kFlagInclusive : kFlagPartial) | tile_count);
+
+  // exclusive scan of tile_count over digits (tile-sorted layout) and of the global histogram over digits
+  uint32_t g = hist[tid];
+  uint32_t incl_t = tile_count, incl_g = g;
+#pragma unroll
+  for (int off = 1; off < 32; off <<= 1) {
+    const uint32_t a = __shfl_up_sync(0xffffffffu, incl_t, off);
+    const uint32_t b = __shfl_up_sync(0xffffffffu, incl_g, off);
+    if (lane >= off) {
+      incl_t += a;
+      incl_g += b;
+    }
+  }
+  __shared__ uint32_t s_scan_g[kSortWarps];
+  if (lane == 31) {
+    s_scan[warp] = incl_t;
+    s_scan_g[warp] = incl_g;
+  }
+  __syncthreads();
+  uint32_t base_t = 0, base_g = 0;
+#pragma unroll
+  for (int w = 0; w < kSortWarps; ++w) {
+    if (w < warp) {
+      base_t += s_scan[w];
+      base_g += s_scan_g[w];
+    }
+  }
+  const uint32_t tile_excl = base_t + incl_t - tile_count;
+  const uint32_t glob_excl = base_g + incl_g - g;
+
+  // decoupled look-back over the previous tiles' counts of this digit
+  uint32_t excl = 0;
+  if (tile > 0) {
+    int64_t t = (int64_t)tile - 1;
+    while (true) {
+      const uint32_t s = ld_volatile_u32(status + (size_t)t * 256 + tid);
+      const uint32_t flag = s & ~kValueMask;
+      if (flag == 0) continue;  // not published yet: that tile is running (ticket order), spin
+      excl += s & kValueMask;
+      if (flag == kFlagInclusive) break;
+      --t;
+    }
+    st_volatile_u32(my_status, kFlagInclusive | (excl + tile_count));
+  }
+  s_tile_excl[tid] = tile_excl;
+  s_digit_base[tid] = (int64_t)glob_excl + (int64_t)excl - (int64_t)tile_excl;
+  __syncthreads();
+
+  // ---- permute through shared memory into tile-sorted order -----------------------------------------------
+#pragma unroll
+  for (int j = 0; j < ITEMS; ++j) {
+    if ((warp_off + j * 32) < valid_in_tile) {
+      const uint32_t d = (uint32_t)(key[j] >> shift) & 0xFFu;
+      const uint32_t pos = s_tile_excl[d] + s_warp_hist[warp][d] + rank[j];
+      s_keys[pos] = key[j];
+      s_vals[pos] = val[j];
+    }
+  }
+  __syncthreads();
+
+  // ---- write out: consecutive tile-sorted positions of one digit are consecutive in global memory -------
+#pragma unroll
+  for (int j = 0; j < ITEMS; ++j) {
+    const int pos = tid + j * kSortThreads;
+    if (pos < valid_in_tile) {
+      const KeyT k = s_keys[pos];
+      const uint32_t d = (uint32_t)(k >> shift) & 0xFFu;
+      const int64_t dst = s_digit_base[d] + pos;
+      keys_out[dst] = k;
+      vals_out[dst] = s_vals[pos];
+    }
+  }
+}
+
+template <typename KeyT>
+static void sort_all(void* scratch, const ScratchLayout& L, int n, cudaStream_t stream) {
+  char* base = static_cast<char*>(scratch);
+  Header* header = reinterpret_cast<Header*>(base + L.header);
+  uint32_t* hist = reinterpret_cast<uint32_t*>(base + L.hist);
+  uint32_t* status = reinterpret_cast<uint32_t*>(base + L.status);
+  KeyT* keys[2] = {reinterpret_cast<KeyT*>(base + L.keys[0]), reinterpret_cast<KeyT*>(base + L.keys[1])};
+  uint32_t* vals[2] = {reinterpret_cast<uint32_t*>(base + L.vals[0]), reinterpret_cast<uint32_t*>(base + L.vals[1])};
+  const int tiles = L.tiles;
+  for (int p = 0; p < L.passes; ++p) {
+    const int in = p & 1, out = in ^ 1;
+    uint32_t* st = status + (size_t)p * tiles * 256;
+    if (p == 0)
+      onesweep_pass_kernel<KeyT, true><<<tiles, kSortThreads, 0, stream>>>(
+          keys[in], keys[out], nullptr, vals[out], hist + p * 256, st, &header->tile_counter[p], n, 8 * p);
+    else
+      onesweep_pass_kernel<KeyT, false><<<tiles, kSortThreads, 0, stream>>>(
+          keys[in], keys[out], vals[in], vals[out], hist + p * 256, st, &header->tile_counter[p], n, 8 * p);
+  }
+}
+
+void launch_sort(void* scratch, const ScratchLayout& L, int n, cudaStream_t stream) {
+  if (L.key_bytes == 4)
+    sort_all<uint32_t>(scratch, L, n, stream);
+  else
+    sort_all<uint64_t>(scratch, L, n, stream);
+}
+
+}  // namespace bvh

@@ -1,0 +1,223 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, tolerance 0.
+
+Bit-exact on: scene bounds, sorted codes, permutation, left_child, rope, AABBs, CSR offsets and sorted
+rows (rows are sets, G13; the raw traversal order is additionally checked to be ascending Morton
+position).  Sizes span several sort tiles (4096 / 3072 keys) plus a ragged tail.
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from helpers import csr_rows_sorted
+from paper_2402_00665_b200 import workloads as W
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2402_00665_b200 import binding
+
+    binding.load_library()  # must exist on a GPU box: no fallback
+    return binding
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_build(B, prims, bits):
+    bvh = B.Bvh(prims.shape[0], bits)
+    bvh.build(_dev(prims))
+    torch.cuda.synchronize()
+    return bvh
+
+
+def export_np(bvh):
+    e = {k: v.cpu().numpy() for k, v in bvh.export().items()}
+    e["sorted_codes"] = e["sorted_codes"].view(np.uint32 if bvh.morton_bits == 30 else np.uint64).astype(np.uint64)
+    e["perm"] = e["perm"].view(np.uint32)
+    return e
+
+
+def assert_build_equal(e, o, ctx=""):
+    n = o.n
+    assert np.array_equal(e["scene_bounds"].view(np.uint32), o.scene_bounds.view(np.uint32)), ctx + " scene bounds"
+    assert np.array_equal(e["sorted_codes"], o.sorted_codes), ctx + " sorted codes"
+    assert np.array_equal(e["perm"], o.perm), ctx + " perm"
+    assert np.array_equal(e["left_child"], o.left_child), ctx + " left_child"
+    assert np.array_equal(e["rope"], o.rope), ctx + " rope"
+    assert np.array_equal(e["aabb"].view(np.uint32), o.aabb.view(np.uint32)), ctx + " aabb"
+    assert e["left_child"].shape[0] == 2 * n - 1
+
+
+def gpu_query(B, bvh, queries):
+    off, idx = B.query(bvh, _dev(queries))
+    torch.cuda.synchronize()
+    return off.cpu().numpy(), idx.cpu().numpy()
+
+
+def assert_query_equal(B, bvh, o, oracle_lib, queries, ctx=""):
+    goff, gidx = gpu_query(B, bvh, queries)
+    if queries.shape[1] == 4:
+        ooff, oidx = oracle_lib.query_spheres_tree(o, queries)
+    else:
+        ooff, oidx = oracle_lib.query_boxes_tree(o, queries)
+    assert np.array_equal(goff, ooff), ctx + " offsets"
+    gidx = gidx[: goff[-1]]
+    assert np.array_equal(csr_rows_sorted(goff, gidx), csr_rows_sorted(ooff, oidx)), ctx + " rows"
+    # stronger: raw order = traversal order = ascending Morton position, which is also the oracle's DFS order
+    assert np.array_equal(gidx, oidx), ctx + " raw order"
+    return goff, gidx
+
+
+CASES = [
+    # name, n, q, radius: small enough for the oracle, several sort tiles + ragged tail
+    ("C1", 4096, 4096, None),
+    ("C2", 50_000, 20_000, 0.05),
+    ("C2", 4096 * 3 + 1, 1000, 0.05),
+    ("C3", 120_001, 5_000, 0.004),
+    ("C4", 70_003, 30_000, 4e-3),
+    ("C5", 65_537, 10_000, 0.04),
+]
+
+
+@pytest.mark.parametrize("name,n,q,radius", CASES)
+def test_build_and_query_parity(B, oracle_lib, name, n, q, radius):
+    w = W.make(name, n=n, q=q, radius=radius)
+    o = oracle_lib.build_bvh(w.prims, w.morton_bits)
+    bvh = gpu_build(B, w.prims, w.morton_bits)
+    assert_build_equal(export_np(bvh), o, name)
+    goff, gidx = assert_query_equal(B, bvh, o, oracle_lib, w.queries, name)
+    assert goff[-1] > 0
+
+
+def test_c1_brute_force(B, oracle_lib):
+    """configs[0]: GPU result = O(n*q) brute force."""
+    w = W.make("C1")
+    bvh = gpu_build(B, w.prims, w.morton_bits)
+    goff, gidx = gpu_query(B, bvh, w.queries)
+    boff, bidx = oracle_lib.query_spheres_brute(w.prims, w.queries)
+    assert np.array_equal(goff, boff)
+    assert np.array_equal(csr_rows_sorted(goff, gidx[: goff[-1]]), bidx)
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 7, 31, 32, 33, 255, 256, 257, 4095, 4096, 4097])
+@pytest.mark.parametrize("bits", [30, 63])
+def test_tiny_and_boundary_sizes(B, oracle_lib, n, bits):
+    pts = W.uniform_cube(n, seed=100 + n)
+    o = oracle_lib.build_bvh(pts, bits)
+    bvh = gpu_build(B, pts, bits)
+    assert_build_equal(export_np(bvh), o, f"n={n}")
+    qs = W.spheres_at(W.uniform_cube(64, seed=7), 0.3)
+    assert_query_equal(B, bvh, o, oracle_lib, qs, f"n={n}")
+
+
+@pytest.mark.parametrize("bits", [30, 63])
+@pytest.mark.parametrize("n", [1, 2, 5, 1000, 10_000])
+def test_all_points_coincident(B, oracle_lib, n, bits):
+    """Every code equal: the tree comes from the index tie-break alone (P4); zero scene extent on every axis."""
+    pts = np.full((n, 3), 0.25, np.float32)
+    o = oracle_lib.build_bvh(pts, bits)
+    bvh = gpu_build(B, pts, bits)
+    e = export_np(bvh)
+    assert_build_equal(e, o)
+    assert np.array_equal(e["perm"], np.arange(n, dtype=np.uint32))
+    qs = np.array([[0.25, 0.25, 0.25, 0.0], [0.5, 0.25, 0.25, 0.25], [0.5, 0.25, 0.25, 0.2499]], np.float32)
+    goff, gidx = assert_query_equal(B, bvh, o, oracle_lib, qs)
+    assert list(np.diff(goff)) == [n, n, 0]
+
+
+def test_t_corner_63bit(B, oracle_lib):
+    """G14: codes 0 and 2^63-1; delta* = INT64_MAX must stay below +infinity."""
+    pts = np.array([[0, 0, 0], [1, 1, 1]], np.float32)
+    bvh = gpu_build(B, pts, 63)
+    e = export_np(bvh)
+    assert list(e["sorted_codes"]) == [0, (1 << 63) - 1]
+    assert list(e["left_child"][:1]) == [1] and list(e["rope"]) == [-1, 2, -1]
+    assert_build_equal(e, oracle_lib.build_bvh(pts, 63))
+
+
+def test_points_equal_degenerate_boxes(B):
+    w = W.make("C2", n=30_000, q=0)
+    a = export_np(gpu_build(B, w.prims, 63))
+    b = export_np(gpu_build(B, np.concatenate([w.prims, w.prims], axis=1), 63))
+    for k in a:
+        assert np.array_equal(a[k].view(np.uint8), b[k].view(np.uint8)), k
+
+
+def test_plane_and_negative_coordinates(B, oracle_lib):
+    """A zero-extent axis (no NaN from 0/0) and negative coordinates (float atomic min/max)."""
+    pts = W.uniform_cube(20_000, seed=5) * np.float32(8.0) - np.float32(6.0)
+    pts[:, 2] = np.float32(-3.5)
+    for bits in (30, 63):
+        o = oracle_lib.build_bvh(pts, bits)
+        bvh = gpu_build(B, pts, bits)
+        assert_build_equal(export_np(bvh), o)
+    boxes = W.boxes_around(pts, 0.05)
+    o = oracle_lib.build_bvh(boxes, 63)
+    bvh = gpu_build(B, boxes, 63)
+    assert_build_equal(export_np(bvh), o)
+    assert_query_equal(B, bvh, o, oracle_lib, W.boxes_around(pts[:2000] + np.float32(0.01), 0.08))
+    assert_query_equal(B, bvh, o, oracle_lib, W.spheres_at(pts[:2000], 0.1))
+
+
+def test_schedule_independence(B):
+    """P8: 20 builds of the same input give identical bytes (nodes and exported arrays)."""
+    w = W.make("C3", n=200_000, q=0)
+    d = _dev(w.prims)
+    ref = None
+    for _ in range(20):
+        bvh = B.Bvh(w.n, w.morton_bits)
+        bvh.nodes.zero_()
+        bvh.build(d)
+        torch.cuda.synchronize()
+        cur = bvh.nodes.cpu().numpy().tobytes()
+        if ref is None:
+            ref = cur
+        assert cur == ref
+
+
+def test_structural_invariants_large(B, oracle_lib):
+    """Properties that hold at any size (P3), checked on the GPU output at n = 2^20 without the oracle tree."""
+    w = W.make("C2", n=1 << 20, q=0)
+    bvh = gpu_build(B, w.prims, w.morton_bits)
+    e = export_np(bvh)
+    n, lb = w.n, w.n - 1
+    assert np.array_equal(np.sort(e["perm"]), np.arange(n, dtype=np.uint32))
+    d = np.diff(e["sorted_codes"].astype(np.int64))
+    assert np.all(d >= 0) and np.all(np.diff(e["perm"].astype(np.int64))[d == 0] > 0)
+    order = oracle_lib.walk_all(e["left_child"], e["rope"], n)
+    assert len(order) == 2 * n - 1 and np.array_equal(order[order >= lb] - lb, np.arange(n))
+    assert e["rope"][0] == -1
+    # root box = scene bounds = numpy min/max of the input
+    assert np.array_equal(e["aabb"][0, :3], w.prims.min(axis=0)) and np.array_equal(e["aabb"][0, 3:], w.prims.max(axis=0))
+    assert np.array_equal(e["scene_bounds"], e["aabb"][0])
+    assert np.array_equal(e["aabb"][lb:, :3], w.prims[e["perm"]])
+    # rope of a left child is its sibling: consecutive Karras indices
+    left = e["left_child"][:lb]
+    sib = e["rope"][left]
+    gl = np.where(left >= lb, left - lb, left)
+    gs = np.where(sib >= lb, sib - lb, sib)
+    assert np.all(gs == gl + 1)
+
+
+def test_empty_inputs(B):
+    bvh = B.Bvh(0, 30)
+    bvh.build(torch.zeros((0, 3), dtype=torch.float32, device="cuda"))
+    qs = _dev(np.array([[0.5, 0.5, 0.5, 1.0]], np.float32))
+    off, idx = B.query(bvh, qs)
+    torch.cuda.synchronize()
+    assert off.cpu().tolist() == [0, 0]
+    bvh = gpu_build(B, W.uniform_cube(100, seed=1), 30)
+    off, idx = B.query(bvh, torch.zeros((0, 4), dtype=torch.float32, device="cuda"))
+    torch.cuda.synchronize()
+    assert off.cpu().tolist() == [0]
+    # queries that hit nothing
+    off, idx = B.query(bvh, _dev(np.array([[5, 5, 5, 0.1], [-5, 0, 0, 0.1]], np.float32)))
+    torch.cuda.synchronize()
+    assert off.cpu().tolist() == [0, 0, 0]
