@@ -1,0 +1,467 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the hot path of arXiv 2402.00665 on B200.
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: linear-BVH build (scene
+bounds, Morton codes, one-sweep radix sort, modified-Apetrei bottom-up pass with ropes and boxes) followed
+by stackless sphere range search to CSR (count, scan, fill).  Workload at N=1: BASELINE.json configs[2]
+("C3": 10,000,000 Gaussian-mixture points, 30-bit Morton, 1,000,000 sphere queries of radius 0.002), the
+config `north_star` quotes its target on.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+  torchrun --nnodes=1 --nproc-per-node N ... bench.py --gpus N --steps K --warmup W
+
+`value` = build throughput (Mprims/s) with inputs resident in HBM, CUDA-event time of the build part of the
+step; the query part is reported beside it (`query`), `ms_per_step` covers both.  N > 1 runs N independent
+replicas (one per GPU, different seeds, no collective on the data path: DESIGN.md "Multi-GPU"), timed as
+the max over ranks.  `--impl reference` times the CPU oracle (oracle/) on a bounded sample: for this tier
+the oracle is the reference arm.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2402_00665_b200 import workloads  # noqa: E402  (numpy only; loads nothing native)
+
+METRIC = "bvh_build_throughput"
+UNIT = "Mprims/s"
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+NOMINAL_HBM_GBS = 8000.0   # the denominator BASELINE.json north_star names
+
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel from the
+# `ncu --set full` capture summarised in profiles/ (None until a capture for that kernel/workload exists).
+NCU_TRAFFIC_BYTES = {}
+
+
+# ---- byte model (restated in DESIGN.md "Roofline") ---------------------------------------
+
+def byte_model(n: int, q: int, nnz: int, prim_floats: int, query_floats: int, bits: int) -> dict:
+    S, K, P, Sq = 4 * prim_floats, (4 if bits == 30 else 8), (4 if bits == 30 else 8), 4 * query_floats
+    per_kernel = {
+        "init": 4 * n,                                   # store memset (status words are implementation overhead)
+        "bounds": S * n,
+        "morton": (S + K) * n,                           # + digit histograms, fused (the model's "histogram read K" is saved)
+        "sort_pass0": (K + K + 4) * n,                   # read code, write code + index (iota synthesised)
+        **{f"sort_pass{p}": 2 * (K + 4) * n for p in range(1, P)},
+        "hierarchy": (4 + S + 32 + K + 4 + 32 + 24) * n,  # perm, input, leaf record, codes, CAS, internal record, sibling box
+        "order": (Sq + 4) * q + (4 + 4 + 4) * q + 3 * 16 * q,   # query Morton codes + 4 sort passes of (code, index)
+        "count": (Sq + 4 + 4) * q,
+        "scan": (4 + 8) * q,
+        "fill": (Sq + 8 + 4) * q + 4 * nnz,
+    }
+    build_total = (3 * S + 4 * K + (2 * P - 1) * (K + 4) + 100) * n      # SURVEY.md B_build
+    query_total = (2 * Sq + 24) * q + 4 * nnz                            # SURVEY.md B_query
+    return {"per_kernel": per_kernel, "build_total": build_total, "query_total": query_total}
+
+
+def measured_peak() -> tuple[float, str]:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+# ---- clocks ---------------------------------------------------------------------------------------------------
+
+class ClockSampler:
+    """nvidia-smi sampling of SM clocks and throttle reasons while the timed region runs."""
+
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                 "-lms", "50", "-f", self.path], stdout=subprocess.DEVNULL, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        try:
+            rows = [r.split(",") for r in open(self.path).read().strip().splitlines() if r.strip()]
+            os.unlink(self.path)
+            sm = [float(r[0]) for r in rows]
+            names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+            reasons = [nm for k, nm in enumerate(names) if any(r[3 + k].strip().lower() == "active" for r in rows)]
+            if sm:
+                # "under load": the upper half of the samples (idle gaps between steps pull the clock down)
+                load = sorted(sm)[len(sm) // 2:]
+                out.update(sm_mhz=float(np.median(load)), sm_max_mhz=float(rows[0][1]), reasons=reasons,
+                           samples=len(sm), power_w_max=max(float(r[2]) for r in rows))
+        except Exception as e:  # never let telemetry kill the bench
+            out["error"] = repr(e)
+        return out
+
+
+# ---- distributed plumbing (one process per GPU; nothing on the data path) ---------------------------------------
+
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def dist_init(backend: str):
+    import torch.distributed as dist
+
+    rank, local_rank, world = dist_env()
+    if world > 1 and not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29531")
+        dist.init_process_group(backend=backend, rank=rank, world_size=world)
+    return rank, local_rank, world
+
+
+def dist_barrier(world: int, device=None):
+    if world > 1:
+        import torch.distributed as dist
+
+        if device is not None and device.type == "cuda":
+            dist.barrier(device_ids=[device.index])
+        else:
+            dist.barrier()
+
+
+def reduce_max_sum(values_max, values_sum, world: int, device):
+    """Max over ranks of `values_max` and sum over ranks of `values_sum` (lists of floats)."""
+    import torch
+
+    if world == 1:
+        return list(values_max), list(values_sum)
+    import torch.distributed as dist
+
+    tm = torch.tensor(values_max, dtype=torch.float64, device=device)
+    ts = torch.tensor(values_sum, dtype=torch.float64, device=device)
+    dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+    dist.all_reduce(ts, op=dist.ReduceOp.SUM)
+    return tm.cpu().tolist(), ts.cpu().tolist()
+
+
+# ---- the two arms ---------------------------------------------------------------------------------------------------
+
+def make_workload(args, rank: int):
+    n = args.n if args.n else None
+    q = args.q if args.q else None
+    w = workloads.make(args.workload, n=n, q=q, seed_offset=rank)
+    return w
+
+
+def config_dict(args, w, world: int, extra=None) -> dict:
+    c = {
+        "workload": f"{w.name}: {w.n} {w.prim_kind} ({w.note}), {w.morton_bits}-bit Morton; {w.q} {w.query_kind} queries"
+                    + (" [BASELINE.json configs[2]]" if (w.name == "C3" and not args.n and not args.q) else " [non-default size]"),
+        "n": w.n, "q": w.q, "morton_bits": w.morton_bits, "replicas": world,
+        "l2": "flushed between timed steps (512 MiB device write) and step working set >> 126 MB L2",
+    }
+    if extra:
+        c.update(extra)
+    return c
+
+
+def run_ours(args) -> dict | None:
+    import torch
+
+    from paper_2402_00665_b200 import binding
+
+    rank, local_rank, world = dist_init("nccl")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU path); use --impl reference for the oracle")
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    binding.load_library()
+
+    w = make_workload(args, rank)
+    n, q, bits = w.n, w.q, w.morton_bits
+    is_box = int(w.prim_kind == "boxes")
+    spheres = w.query_kind == "spheres"
+    h_prims = torch.from_numpy(w.prims).pin_memory()
+    h_queries = torch.from_numpy(w.queries).pin_memory()
+    d_prims = h_prims.to(device)
+    d_queries = h_queries.to(device)
+    bvh = binding.Bvh(n, bits, device)
+    ws = binding.QueryWorkspace(q, device)
+    order_fn = binding.bvh_query_order_spheres if spheres else binding.bvh_query_order_boxes
+    count_fn = binding.bvh_query_spheres_count if spheres else binding.bvh_query_boxes_count
+    fill_fn = binding.bvh_query_spheres_fill if spheres else binding.bvh_query_boxes_fill
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)
+
+    # one untimed pass to learn nnz (same inputs every step -> same nnz) and size the result buffer
+    bvh.build(d_prims)
+    order_fn(bvh.nodes, n, d_queries, q, ws.order, ws.order_scratch)
+    count_fn(bvh.nodes, n, d_queries, q, ws.order, ws.counts)
+    binding.bvh_scan_counts(ws.counts, q, ws.offsets, ws.scan_scratch)
+    nnz = int(ws.offsets[q].item())
+    d_indices = torch.empty(max(nnz, 1), dtype=torch.int32, device=device)
+
+    def ev():
+        e = torch.cuda.Event(enable_timing=True)
+        e.record()  # materialise the cudaEvent_t so its handle can cross the C ABI
+        return e
+
+    stage = [ev() for _ in range(binding.NUM_STAGE_EVENTS)]
+    e_order, e_count, e_scan, e_fill = ev(), ev(), ev(), ev()
+    P = 4 if bits == 30 else 8
+    stage_for_call = [stage[k] if (k < 4 + P or k == 12) else None for k in range(binding.NUM_STAGE_EVENTS)]
+
+    def step():
+        binding.bvh_build_staged(d_prims, is_box, n, bits, bvh.nodes, bvh.scratch, stage_for_call)
+        order_fn(bvh.nodes, n, d_queries, q, ws.order, ws.order_scratch)
+        e_order.record()
+        count_fn(bvh.nodes, n, d_queries, q, ws.order, ws.counts)
+        e_count.record()
+        binding.bvh_scan_counts(ws.counts, q, ws.offsets, ws.scan_scratch)
+        e_scan.record()
+        fill_fn(bvh.nodes, n, d_queries, q, ws.order, ws.offsets, d_indices)
+        e_fill.record()
+
+    names = ["init", "bounds", "morton"] + [f"sort_pass{p}" for p in range(P)] + ["hierarchy", "order", "count", "scan", "fill"]
+    launches_per_step = {"init": 0, "bounds": 1, "morton": 1, **{f"sort_pass{p}": 1 for p in range(P)},
+                         "hierarchy": 1, "order": 5, "count": 1, "scan": 3, "fill": 1}
+
+    def read_times() -> dict:
+        t = {"init": stage[0].elapsed_time(stage[1]), "bounds": stage[1].elapsed_time(stage[2]),
+             "morton": stage[2].elapsed_time(stage[3])}
+        prev = stage[3]
+        for p in range(P):
+            t[f"sort_pass{p}"] = prev.elapsed_time(stage[4 + p])
+            prev = stage[4 + p]
+        t["hierarchy"] = prev.elapsed_time(stage[12])
+        t["order"] = stage[12].elapsed_time(e_order)
+        t["count"] = e_order.elapsed_time(e_count)
+        t["scan"] = e_count.elapsed_time(e_scan)
+        t["fill"] = e_scan.elapsed_time(e_fill)
+        t["_build"] = stage[0].elapsed_time(stage[12])
+        t["_query"] = stage[12].elapsed_time(e_fill)
+        t["_step"] = stage[0].elapsed_time(e_fill)
+        return t
+
+    for _ in range(args.warmup):
+        flush.fill_(1)
+        step()
+    torch.cuda.synchronize()
+
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    dist_barrier(world, device)
+    torch.cuda.synchronize()
+    acc = {}
+    per_step_build = []
+    for _ in range(args.steps):
+        flush.fill_(1)          # evict L2 between timed steps (outside the events)
+        step()
+        torch.cuda.synchronize()
+        t = read_times()
+        per_step_build.append(t["_build"])
+        for k, v in t.items():
+            acc[k] = acc.get(k, 0.0) + v
+    torch.cuda.synchronize()
+    dist_barrier(world, device)
+    clocks = sampler.stop() if rank == 0 else None
+
+    # ---- end to end: pinned host inputs -> device -> build -> query -> CSR back on the host, public API ----------
+    e2e_steps = max(1, min(args.steps, 5))
+    h_offsets = torch.empty(q + 1, dtype=torch.int64).pin_memory()
+    h_indices = torch.empty(max(nnz, 1), dtype=torch.int32).pin_memory()
+    h_root = torch.empty(32, dtype=torch.uint8).pin_memory()
+
+    def e2e_step():
+        t0 = time.perf_counter()
+        dp = h_prims.to(device, non_blocking=True)
+        bvh.build(dp)
+        h_root.copy_(bvh.nodes[:32], non_blocking=True)
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        dq = h_queries.to(device, non_blocking=True)
+        off, idx = binding.query(bvh, dq, ws)      # reads nnz back, allocates, fills
+        h_offsets.copy_(off, non_blocking=True)
+        h_indices[: idx.numel()].copy_(idx, non_blocking=True)
+        torch.cuda.synchronize()
+        t2 = time.perf_counter()
+        return t1 - t0, t2 - t1
+
+    e2e_step()
+    dist_barrier(world, device)
+    e2e_b, e2e_q = 0.0, 0.0
+    for _ in range(e2e_steps):
+        b, qq = e2e_step()
+        e2e_b += b
+        e2e_q += qq
+    dist_barrier(world, device)
+
+    # ---- reduce over ranks: time = max, units = sum -----------------------------------------------------------------
+    keys = sorted(acc)
+    mx, sm = reduce_max_sum([acc[k] for k in keys] + [e2e_b, e2e_q], [float(n), float(q), float(nnz)], world, device)
+    acc = dict(zip(keys, mx[: len(keys)]))
+    e2e_b, e2e_q = mx[len(keys)], mx[len(keys) + 1]
+    n_all, q_all, nnz_all = sm
+    if rank != 0:
+        return None
+
+    K = args.steps
+    ms = {k: v / K for k, v in acc.items()}
+    model = byte_model(n, q, nnz, w.prims.shape[1], w.queries.shape[1], bits)
+    peak, peak_src = measured_peak()
+    kernels = {}
+    for k in names:
+        b = model["per_kernel"][k]
+        gbs = b / (ms[k] * 1e-3) / 1e9 if ms[k] > 0 else 0.0
+        kernels[k] = {"ms": round(ms[k], 5), "alg_bytes": int(b), "gbs": round(gbs, 1), "frac": round(gbs / peak, 4),
+                      "launches": launches_per_step[k]}
+    dominant = max((k for k in names if launches_per_step[k] == 1), key=lambda k: ms[k])
+    dk = kernels[dominant]
+    build_gbs = model["build_total"] / (ms["_build"] * 1e-3) / 1e9
+    query_gbs = model["query_total"] / (ms["_query"] * 1e-3) / 1e9
+    value = n_all / (ms["_build"] * 1e-3) / 1e6
+    line = {
+        "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+        "ms_per_step": round(ms["_step"], 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u32 Morton codes / f32 boxes" if bits == 30 else "u64 Morton codes / f32 boxes", "data": "synthetic",
+        "config": config_dict(args, w, world, {"hits_per_query": round(nnz / max(q, 1), 2), "nnz": nnz}),
+        "build": {"ms": round(ms["_build"], 4), "mprims_per_s": round(value, 2), "alg_bytes": int(model["build_total"]),
+                  "gbs": round(build_gbs, 1), "frac_of_measured_peak": round(build_gbs / peak, 4),
+                  "frac_of_8TBs": round(build_gbs / NOMINAL_HBM_GBS, 4),
+                  "ms_min": round(min(per_step_build), 4), "ms_median": round(float(np.median(per_step_build)), 4)},
+        "query": {"ms": round(ms["_query"], 4), "mqueries_per_s": round(q_all / (ms["_query"] * 1e-3) / 1e6, 3),
+                  "alg_bytes": int(model["query_total"]), "gbs": round(query_gbs, 1),
+                  "frac_of_measured_peak": round(query_gbs / peak, 4), "frac_of_8TBs": round(query_gbs / NOMINAL_HBM_GBS, 4),
+                  "excluded": "nnz read-back and indices allocation (included in e2e)"},
+        "roofline": {"bound": "hbm", "kernel": dominant, "achieved": dk["gbs"], "peak": peak, "unit": "GB/s",
+                     "frac": dk["frac"], "traffic": NCU_TRAFFIC_BYTES.get(dominant), "peak_source": peak_src,
+                     "alg_bytes_per_launch": dk["alg_bytes"], "ms_per_launch": dk["ms"]},
+        "kernels": kernels,
+        "gpu_launches": K * sum(launches_per_step.values()),
+        "e2e": {"value": round(n_all / (e2e_b / e2e_steps) / 1e6, 2), "unit": UNIT,
+                "h2d_bytes_per_step": int(h_prims.numel() * 4 + h_queries.numel() * 4),
+                "d2h_bytes_per_step": int(32 + 8 + (q + 1) * 8 + nnz * 4), "steps": e2e_steps,
+                "build_ms": round(e2e_b / e2e_steps * 1e3, 3), "query_ms": round(e2e_q / e2e_steps * 1e3, 3),
+                "query_mqueries_per_s": round(q_all / (e2e_q / e2e_steps) / 1e6, 3),
+                "what": "pinned host prims -> H2D -> build -> root record D2H | pinned queries -> H2D -> count, scan, "
+                        "nnz read-back, alloc, fill -> CSR offsets+indices D2H; wall clock, through binding.Bvh/query"},
+        "clocks": clocks,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(w)
+    return line
+
+
+def cpu_baseline(w) -> dict:
+    """The oracle as it stands, one core, on a bounded sample of the same workload."""
+    import oracle
+
+    oracle.build()
+    qs = min(w.q, 50_000)
+    t0 = time.perf_counter()
+    o = oracle.build_bvh(w.prims, w.morton_bits)
+    t1 = time.perf_counter()
+    if w.query_kind == "spheres":
+        off, _ = oracle.query_spheres_tree(o, w.queries[:qs])
+    else:
+        off, _ = oracle.query_boxes_tree(o, w.queries[:qs])
+    t2 = time.perf_counter()
+    return {"value": round(w.n / (t1 - t0) / 1e6, 3), "unit": UNIT, "cores": 1, "kind": "oracle",
+            "host_cores": os.cpu_count(),
+            "sample": f"build: all {w.n} primitives once ({t1 - t0:.2f} s); queries: first {qs} of {w.q} against that tree "
+                      f"({t2 - t1:.2f} s, {int(off[-1])} hits)",
+            "query_mqueries_per_s": round(qs / (t2 - t1) / 1e6, 4)}
+
+
+def run_reference(args) -> dict | None:
+    """Reference arm for this tier = the CPU oracle, timed as it stands on the host cores (rank 0 only)."""
+    rank, _, world = dist_env()
+    if rank != 0:
+        return None
+    import oracle
+
+    oracle.build()
+    w = make_workload(args, 0)
+    ns, qs = min(w.n, 2_500_000), min(w.q, 10_000)
+    prims, queries = w.prims[:ns], w.queries[:qs]
+
+    def step():
+        t0 = time.perf_counter()
+        o = oracle.build_bvh(prims, w.morton_bits)
+        t1 = time.perf_counter()
+        if w.query_kind == "spheres":
+            oracle.query_spheres_tree(o, queries)
+        else:
+            oracle.query_boxes_tree(o, queries)
+        return t1 - t0, time.perf_counter() - t1
+
+    for _ in range(args.warmup):
+        step()
+    tb = tq = 0.0
+    for _ in range(args.steps):
+        b, qq = step()
+        tb += b
+        tq += qq
+    value = round(ns / (tb / args.steps) / 1e6, 3)
+    sample = (f"each step: oracle build of the first {ns} of {w.n} primitives + first {qs} of {w.q} queries on that tree; "
+              f"serial, 1 of {os.cpu_count()} host cores")
+    return {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": round((tb + tq) / args.steps * 1e3, 3), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u64 Morton codes / f32 boxes", "data": "synthetic",
+        "config": config_dict(args, w, world, {"sample": sample}),
+        "query": {"mqueries_per_s": round(qs / (tq / args.steps) / 1e6, 4)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--workload", default="C3", choices=sorted(workloads.FULL_SIZES))
+    ap.add_argument("--n", type=int, default=0, help="override the primitive count (non-default: for quick checks)")
+    ap.add_argument("--q", type=int, default=0, help="override the query count")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args(argv)
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    line = run_reference(args) if args.impl == "reference" else run_ours(args)
+    if line is not None:
+        print(json.dumps(line), flush=True)
+    try:
+        import torch.distributed as dist
+
+        if dist.is_available() and dist.is_initialized():
+            dist.destroy_process_group()
+    except Exception:
+        pass
+
+
+if __name__ == "__main__":
+    main()

@@ -65,14 +65,37 @@ int bvh_build_points(const float* xyz, int64_t n, int morton_bits, void* nodes, 
 int bvh_build_boxes(const float* minmax, int64_t n, int morton_bits, void* nodes, void* scratch,
                     size_t scratch_bytes, void* stream);
 
+/* The same build with stage boundaries marked for measurement: after stage k the library records
+ * stage_events[k] (a cudaEvent_t created by the caller, passed as void*) on `stream` -- recording is
+ * asynchronous, nothing is created or synchronised.  NULL entries are skipped.  Stages:
+ *   [0] start  [1] scratch initialised  [2] scene bounds  [3] Morton codes + digit histograms
+ *   [4+p] sort pass p (p < 4 for 30-bit, p < 8 for 63-bit)  [12] bottom-up pass (Algorithm 4)
+ * stage_events must hold BVH_NUM_STAGE_EVENTS entries.  prim_is_box: 0 = xyz points, 1 = minmax boxes. */
+#define BVH_NUM_STAGE_EVENTS 13
+int bvh_build_staged(const float* prim, int prim_is_box, int64_t n, int morton_bits, void* nodes, void* scratch,
+                     size_t scratch_bytes, void* stream, void* const* stage_events);
+
+/* Query scheduling (optional; "data divergence").  Computes a Morton order of the queries
+ * in the frame of the hierarchy's root box: order[t] = index of the query at position t along the curve
+ * (30-bit code of the sphere centre / box centroid, clamped into the frame; same kernels as the build's
+ * steps 1-2).  Passing `order` to the count and fill calls makes thread t serve query order[t], so that
+ * neighbouring threads walk nearly the same nodes.  Results are unaffected: row j of the CSR still
+ * belongs to query j.  order: uint32[q].  bvh_query_order_sizes is a host call. */
+int bvh_query_order_sizes(int64_t q, size_t* scratch_bytes);
+int bvh_query_order_spheres(const void* nodes, int64_t n, const float* xyzr, int64_t q, uint32_t* order,
+                            void* scratch, size_t scratch_bytes, void* stream);
+int bvh_query_order_boxes(const void* nodes, int64_t n, const float* minmax, int64_t q, uint32_t* order,
+                          void* scratch, size_t scratch_bytes, void* stream);
+
 /* Range search by Algorithm 1: stackless traversal over
  * {left_child, rope}.  Count pass: counts[j] = number of primitives whose box satisfies query j.
  * Sphere query {x,y,z,r}: squared distance from the centre to the box <= r*r, fp32 round-to-nearest,
  * association of D8.  Box query {min.xyz,max.xyz}: closed-interval overlap on every axis (G12).
+ * order: NULL (thread t serves query t) or a permutation of [0,q) from bvh_query_order_*.
  * q = 0 or n = 0: counts (if q > 0) are set to 0. */
-int bvh_query_spheres_count(const void* nodes, int64_t n, const float* xyzr, int64_t q,
+int bvh_query_spheres_count(const void* nodes, int64_t n, const float* xyzr, int64_t q, const uint32_t* order,
                             int32_t* counts, void* stream);
-int bvh_query_boxes_count(const void* nodes, int64_t n, const float* minmax, int64_t q,
+int bvh_query_boxes_count(const void* nodes, int64_t n, const float* minmax, int64_t q, const uint32_t* order,
                           int32_t* counts, void* stream);
 
 /* Exclusive prefix sum of counts into 64-bit CSR offsets: offsets[0] = 0, offsets[q] = nnz (G21).
@@ -85,9 +108,9 @@ int bvh_scan_counts(const int32_t* counts, int64_t q, int64_t* offsets, void* sc
  * the ORIGINAL indices of the primitives hit, in traversal order (ascending Morton position; PAPER.md:56
  * "Store the result").  The caller reads offsets[q] to size `indices` (the one device->host sync
  * of the path, and it is the caller's). */
-int bvh_query_spheres_fill(const void* nodes, int64_t n, const float* xyzr, int64_t q,
+int bvh_query_spheres_fill(const void* nodes, int64_t n, const float* xyzr, int64_t q, const uint32_t* order,
                            const int64_t* offsets, int32_t* indices, void* stream);
-int bvh_query_boxes_fill(const void* nodes, int64_t n, const float* minmax, int64_t q,
+int bvh_query_boxes_fill(const void* nodes, int64_t n, const float* minmax, int64_t q, const uint32_t* order,
                          const int64_t* offsets, int32_t* indices, void* stream);
 
 /* Parity export: the canonical arrays of a finished build, for bit-exact comparison.

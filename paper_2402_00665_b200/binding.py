@@ -35,12 +35,16 @@ SYMBOLS = {
     "bvh_sizes": [c_int64, c_int, ctypes.POINTER(c_size_t), ctypes.POINTER(c_size_t)],
     "bvh_build_points": [_P, c_int64, c_int, _P, _P, c_size_t, _P],
     "bvh_build_boxes": [_P, c_int64, c_int, _P, _P, c_size_t, _P],
-    "bvh_query_spheres_count": [_P, c_int64, _P, c_int64, _P, _P],
-    "bvh_query_boxes_count": [_P, c_int64, _P, c_int64, _P, _P],
+    "bvh_build_staged": [_P, c_int, c_int64, c_int, _P, _P, c_size_t, _P, ctypes.POINTER(c_void_p)],
+    "bvh_query_order_sizes": [c_int64, ctypes.POINTER(c_size_t)],
+    "bvh_query_order_spheres": [_P, c_int64, _P, c_int64, _P, _P, c_size_t, _P],
+    "bvh_query_order_boxes": [_P, c_int64, _P, c_int64, _P, _P, c_size_t, _P],
+    "bvh_query_spheres_count": [_P, c_int64, _P, c_int64, _P, _P, _P],
+    "bvh_query_boxes_count": [_P, c_int64, _P, c_int64, _P, _P, _P],
     "bvh_scan_sizes": [c_int64, ctypes.POINTER(c_size_t)],
     "bvh_scan_counts": [_P, c_int64, _P, _P, c_size_t, _P],
-    "bvh_query_spheres_fill": [_P, c_int64, _P, c_int64, _P, _P, _P],
-    "bvh_query_boxes_fill": [_P, c_int64, _P, c_int64, _P, _P, _P],
+    "bvh_query_spheres_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
+    "bvh_query_boxes_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
     "bvh_export": [_P, _P, c_int64, c_int, _P, _P, _P, _P, _P, _P, _P],
 }
 
@@ -109,13 +113,45 @@ def bvh_build_boxes(minmax: torch.Tensor, n: int, morton_bits: int, nodes: torch
                                           scratch.numel() * scratch.element_size(), _stream()), "bvh_build_boxes")
 
 
-def bvh_query_spheres_count(nodes, n: int, xyzr, q: int, counts) -> None:
-    _check(load_library().bvh_query_spheres_count(_ptr(nodes), n, _ptr(xyzr), q, _ptr(counts), _stream()),
+NUM_STAGE_EVENTS = 13
+STAGE_NAMES = ["start", "init", "bounds", "morton"] + [f"sort_pass{p}" for p in range(8)] + ["hierarchy"]
+
+
+def bvh_build_staged(prim: torch.Tensor, prim_is_box: int, n: int, morton_bits: int, nodes: torch.Tensor,
+                     scratch: torch.Tensor, stage_events) -> None:
+    """stage_events: sequence of NUM_STAGE_EVENTS entries, each a ``torch.cuda.Event(enable_timing=True)`` that has
+    been recorded at least once (so that its cudaEvent_t exists) or None."""
+    assert len(stage_events) == NUM_STAGE_EVENTS
+    arr = (c_void_p * NUM_STAGE_EVENTS)(*[None if e is None else e.cuda_event for e in stage_events])
+    _check(load_library().bvh_build_staged(_ptr(prim), int(prim_is_box), n, morton_bits, _ptr(nodes), _ptr(scratch),
+                                           scratch.numel() * scratch.element_size(), _stream(), arr), "bvh_build_staged")
+
+
+def bvh_query_order_sizes(q: int) -> int:
+    sb = c_size_t()
+    _check(load_library().bvh_query_order_sizes(q, ctypes.byref(sb)), "bvh_query_order_sizes")
+    return sb.value
+
+
+def bvh_query_order_spheres(nodes, n: int, xyzr, q: int, order, scratch) -> None:
+    _check(load_library().bvh_query_order_spheres(_ptr(nodes), n, _ptr(xyzr), q, _ptr(order), _ptr(scratch),
+                                                  scratch.numel() * scratch.element_size(), _stream()),
+           "bvh_query_order_spheres")
+
+
+def bvh_query_order_boxes(nodes, n: int, minmax, q: int, order, scratch) -> None:
+    _check(load_library().bvh_query_order_boxes(_ptr(nodes), n, _ptr(minmax), q, _ptr(order), _ptr(scratch),
+                                                scratch.numel() * scratch.element_size(), _stream()),
+           "bvh_query_order_boxes")
+
+
+def bvh_query_spheres_count(nodes, n: int, xyzr, q: int, order, counts) -> None:
+    _check(load_library().bvh_query_spheres_count(_ptr(nodes), n, _ptr(xyzr), q, _ptr(order), _ptr(counts), _stream()),
            "bvh_query_spheres_count")
 
 
-def bvh_query_boxes_count(nodes, n: int, minmax, q: int, counts) -> None:
-    _check(load_library().bvh_query_boxes_count(_ptr(nodes), n, _ptr(minmax), q, _ptr(counts), _stream()),
+def bvh_query_boxes_count(nodes, n: int, minmax, q: int, order, counts) -> None:
+    _check(load_library().bvh_query_boxes_count(_ptr(nodes), n, _ptr(minmax), q, _ptr(order), _ptr(counts), _stream()),
            "bvh_query_boxes_count")
 
 
@@ -130,14 +166,14 @@ def bvh_scan_counts(counts, q: int, offsets, scratch) -> None:
                                           scratch.numel() * scratch.element_size(), _stream()), "bvh_scan_counts")
 
 
-def bvh_query_spheres_fill(nodes, n: int, xyzr, q: int, offsets, indices) -> None:
-    _check(load_library().bvh_query_spheres_fill(_ptr(nodes), n, _ptr(xyzr), q, _ptr(offsets), _ptr(indices),
-                                                 _stream()), "bvh_query_spheres_fill")
+def bvh_query_spheres_fill(nodes, n: int, xyzr, q: int, order, offsets, indices) -> None:
+    _check(load_library().bvh_query_spheres_fill(_ptr(nodes), n, _ptr(xyzr), q, _ptr(order), _ptr(offsets),
+                                                 _ptr(indices), _stream()), "bvh_query_spheres_fill")
 
 
-def bvh_query_boxes_fill(nodes, n: int, minmax, q: int, offsets, indices) -> None:
-    _check(load_library().bvh_query_boxes_fill(_ptr(nodes), n, _ptr(minmax), q, _ptr(offsets), _ptr(indices),
-                                               _stream()), "bvh_query_boxes_fill")
+def bvh_query_boxes_fill(nodes, n: int, minmax, q: int, order, offsets, indices) -> None:
+    _check(load_library().bvh_query_boxes_fill(_ptr(nodes), n, _ptr(minmax), q, _ptr(order), _ptr(offsets),
+                                               _ptr(indices), _stream()), "bvh_query_boxes_fill")
 
 
 def bvh_export(nodes, scratch, n: int, morton_bits: int, sorted_codes=None, perm=None, left_child=None, rope=None,
@@ -187,20 +223,24 @@ class Bvh:
 
 
 class QueryWorkspace:
-    """Reusable device buffers for count-then-fill over up to ``q`` queries."""
+    """Reusable device buffers for ordered count-then-fill over up to ``q`` queries."""
 
     def __init__(self, q: int, device="cuda"):
         self.q = int(q)
         self.counts = torch.empty(max(self.q, 1), dtype=torch.int32, device=device)
         self.offsets = torch.empty(self.q + 1, dtype=torch.int64, device=device)
         self.scan_scratch = torch.empty(max(bvh_scan_sizes(self.q), 8), dtype=torch.uint8, device=device)
+        self.order = torch.empty(max(self.q, 1), dtype=torch.int32, device=device)
+        self.order_scratch = torch.empty(bvh_query_order_sizes(self.q), dtype=torch.uint8, device=device)
 
 
-def query(bvh: Bvh, queries: torch.Tensor, ws: QueryWorkspace | None = None, indices: torch.Tensor | None = None):
+def query(bvh: Bvh, queries: torch.Tensor, ws: QueryWorkspace | None = None, indices: torch.Tensor | None = None,
+          ordered: bool = True):
     """Range search.  queries: float32 CUDA [q,4] spheres {x,y,z,r} or [q,6] boxes {min,max}.
 
-    Returns (offsets int64[q+1], indices int32[nnz]) on the device.  Reads nnz back once (the path's only
-    device->host sync) unless ``indices`` is passed in with enough room."""
+    order (Morton schedule of the queries) -> count -> scan -> fill.  Returns (offsets int64[q+1], indices
+    int32[nnz]) on the device.  Reads nnz back once (the path's only device->host sync) unless ``indices`` is
+    passed in with enough room."""
     if queries.dtype != torch.float32 or queries.dim() != 2 or queries.shape[1] not in (4, 6):
         raise BvhError(f"expected float32 [q,4] or [q,6], got {queries.dtype} {tuple(queries.shape)}")
     q = int(queries.shape[0])
@@ -208,13 +248,18 @@ def query(bvh: Bvh, queries: torch.Tensor, ws: QueryWorkspace | None = None, ind
     spheres = queries.shape[1] == 4
     count = bvh_query_spheres_count if spheres else bvh_query_boxes_count
     fill = bvh_query_spheres_fill if spheres else bvh_query_boxes_fill
-    count(bvh.nodes, bvh.n, queries, q, ws.counts)
+    order = None
+    if ordered and q > 0:
+        (bvh_query_order_spheres if spheres else bvh_query_order_boxes)(bvh.nodes, bvh.n, queries, q, ws.order,
+                                                                        ws.order_scratch)
+        order = ws.order
+    count(bvh.nodes, bvh.n, queries, q, order, ws.counts)
     bvh_scan_counts(ws.counts, q, ws.offsets, ws.scan_scratch)
     if indices is None:
         nnz = int(ws.offsets[q].item())
         indices = torch.empty(max(nnz, 1), dtype=torch.int32, device=queries.device)
     else:
         nnz = None
-    fill(bvh.nodes, bvh.n, queries, q, ws.offsets, indices)
+    fill(bvh.nodes, bvh.n, queries, q, order, ws.offsets, indices)
     offsets = ws.offsets[: q + 1]
     return offsets, (indices if nnz is None else indices[:nnz])

@@ -148,24 +148,35 @@ __device__ __forceinline__ uint32_t quantise(float lo, float hi, float slo, floa
   return min(q, cell_max);
 }
 
-template <typename KeyT, int PASSES, bool IS_BOX>
+// PRIM_FLOATS: 3 = points, 6 = boxes {min,max}, 4 = sphere queries {x,y,z,r} (centre only; used to order queries).
+// FROM_ROOT: the frame is the root node's box (a finished hierarchy) instead of the build header.
+template <typename KeyT, int PASSES, int PRIM_FLOATS, bool FROM_ROOT>
 __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __restrict__ prim, int n,
                                                                 const Header* __restrict__ header,
+                                                                const Node* __restrict__ root,
                                                                 KeyT* __restrict__ codes, uint32_t* __restrict__ hist) {
   __shared__ uint32_t s_hist[PASSES * 256];
   for (int i = threadIdx.x; i < PASSES * 256; i += kMortonThreads) s_hist[i] = 0;
   float scene[6];
-  load_scene_bounds(header, scene);
+  if (FROM_ROOT) {
+    const float4 lo4 = root->lo, hi4 = root->hi;
+    scene[0] = lo4.x; scene[1] = lo4.y; scene[2] = lo4.z; scene[3] = hi4.x; scene[4] = hi4.y; scene[5] = hi4.z;
+  } else {
+    load_scene_bounds(header, scene);
+  }
   __syncthreads();
   constexpr int B = (sizeof(KeyT) == 4) ? 10 : 21;
   const float scale = (float)(1u << B);
   const uint32_t cell_max = (1u << B) - 1u;
   for (int64_t i = (int64_t)blockIdx.x * kMortonThreads + threadIdx.x; i < n; i += (int64_t)gridDim.x * kMortonThreads) {
     float lo[3], hi[3];
-    if (IS_BOX) {
+    if (PRIM_FLOATS == 6) {
       const float2* p = reinterpret_cast<const float2*>(prim + 6 * i);
       const float2 a = __ldcs(p), b = __ldcs(p + 1), c = __ldcs(p + 2);
       lo[0] = a.x; lo[1] = a.y; lo[2] = b.x; hi[0] = b.y; hi[1] = c.x; hi[2] = c.y;
+    } else if (PRIM_FLOATS == 4) {
+      const float4 v = __ldg(reinterpret_cast<const float4*>(prim) + i);
+      lo[0] = hi[0] = v.x; lo[1] = hi[1] = v.y; lo[2] = hi[2] = v.z;
     } else {
       const float* p = prim + 3 * i;
       lo[0] = hi[0] = __ldcs(p);
@@ -174,7 +185,13 @@ __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __r
     }
     uint32_t cell[3];
 #pragma unroll
-    for (int a = 0; a < 3; ++a) cell[a] = quantise(lo[a], hi[a], scene[a], scene[3 + a], scale, cell_max);
+    for (int a = 0; a < 3; ++a) {
+      if (FROM_ROOT) {  // queries may lie outside the frame: clamp the centroid into it (ordering heuristic only)
+        const float c = __fmul_rn(__fadd_rn(lo[a], hi[a]), 0.5f);
+        lo[a] = hi[a] = fminf(fmaxf(c, scene[a]), scene[3 + a]);
+      }
+      cell[a] = quantise(lo[a], hi[a], scene[a], scene[3 + a], scale, cell_max);
+    }
     KeyT code;
     if (sizeof(KeyT) == 4)
       code = (KeyT)((spread10(cell[0]) << 2) | (spread10(cell[1]) << 1) | spread10(cell[2]));
@@ -191,23 +208,36 @@ __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __r
   }
 }
 
-void launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
-                   uint32_t* hist, cudaStream_t stream) {
+static unsigned morton_grid(int n) {
   int64_t blocks = ((int64_t)n + kMortonThreads - 1) / kMortonThreads;
   const int64_t cap = (int64_t)kNumSMs * 8;
   if (blocks > cap) blocks = cap;
-  const unsigned g = (unsigned)blocks;
+  return (unsigned)blocks;
+}
+
+void launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
+                   uint32_t* hist, cudaStream_t stream) {
+  const unsigned g = morton_grid(n);
   if (morton_bits == 30) {
     if (is_box)
-      morton_kernel<uint32_t, 4, true><<<g, kMortonThreads, 0, stream>>>(prim, n, header, (uint32_t*)codes, hist);
+      morton_kernel<uint32_t, 4, 6, false><<<g, kMortonThreads, 0, stream>>>(prim, n, header, nullptr, (uint32_t*)codes, hist);
     else
-      morton_kernel<uint32_t, 4, false><<<g, kMortonThreads, 0, stream>>>(prim, n, header, (uint32_t*)codes, hist);
+      morton_kernel<uint32_t, 4, 3, false><<<g, kMortonThreads, 0, stream>>>(prim, n, header, nullptr, (uint32_t*)codes, hist);
   } else {
     if (is_box)
-      morton_kernel<uint64_t, 8, true><<<g, kMortonThreads, 0, stream>>>(prim, n, header, (uint64_t*)codes, hist);
+      morton_kernel<uint64_t, 8, 6, false><<<g, kMortonThreads, 0, stream>>>(prim, n, header, nullptr, (uint64_t*)codes, hist);
     else
-      morton_kernel<uint64_t, 8, false><<<g, kMortonThreads, 0, stream>>>(prim, n, header, (uint64_t*)codes, hist);
+      morton_kernel<uint64_t, 8, 3, false><<<g, kMortonThreads, 0, stream>>>(prim, n, header, nullptr, (uint64_t*)codes, hist);
   }
+}
+
+void launch_query_morton(const float* queries, int q, int kind, const Node* root, uint32_t* codes, uint32_t* hist,
+                         cudaStream_t stream) {
+  const unsigned g = morton_grid(q);
+  if (kind == 0)
+    morton_kernel<uint32_t, 4, 4, true><<<g, kMortonThreads, 0, stream>>>(queries, q, nullptr, root, codes, hist);
+  else
+    morton_kernel<uint32_t, 4, 6, true><<<g, kMortonThreads, 0, stream>>>(queries, q, nullptr, root, codes, hist);
 }
 
 }  // namespace bvh

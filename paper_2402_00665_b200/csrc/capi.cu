@@ -93,7 +93,7 @@ static inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_
 static int check_launch() { return cudaGetLastError() == cudaSuccess ? BVH_OK : BVH_ERR_CUDA; }
 
 static int build(const float* prim, bool is_box, int64_t n, int morton_bits, void* nodes, void* scratch,
-                 size_t scratch_bytes, void* stream_) {
+                 size_t scratch_bytes, void* stream_, void* const* events = nullptr) {
   if (n < 0) return BVH_ERR_INVALID_ARGUMENT;
   if (morton_bits != 30 && morton_bits != 63) return BVH_ERR_MORTON_BITS;
   if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
@@ -109,18 +109,26 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   uint32_t* hist = reinterpret_cast<uint32_t*>(base + L.hist);
   int* store = reinterpret_cast<int*>(base + L.store);
 
+  auto mark = [&](int k) {
+    if (events && events[k]) cudaEventRecord(static_cast<cudaEvent_t>(events[k]), stream);
+  };
+  mark(0);
   if (cudaMemsetAsync(base, 0, L.zero_bytes, stream) != cudaSuccess) return BVH_ERR_CUDA;
   if (cudaMemsetAsync(store, 0xFF, (size_t)n * sizeof(int), stream) != cudaSuccess) return BVH_ERR_CUDA;
+  mark(1);
   launch_scene_bounds(prim, (int)n, is_box, header, stream);
+  mark(2);
   launch_morton(prim, (int)n, is_box, morton_bits, header, base + L.keys[0], hist, stream);
-  launch_sort(scratch, L, (int)n, stream);
+  mark(3);
+  launch_sort(sort_buffers(scratch, L), L.key_bytes, L.passes, (int)n, stream, events ? events + 4 : nullptr);
   launch_hierarchy(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
                    store, static_cast<Node*>(nodes), (int)n, stream);
+  mark(12);
   return check_launch();
 }
 
-static int query(const void* nodes, int64_t n, const float* queries, int64_t q, int kind, bool fill, int32_t* counts,
-                 const int64_t* offsets, int32_t* indices, void* stream_) {
+static int query(const void* nodes, int64_t n, const float* queries, int64_t q, int kind, bool fill,
+                 const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* indices, void* stream_) {
   if (n < 0 || q < 0) return BVH_ERR_INVALID_ARGUMENT;
   if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
   if (q == 0) return BVH_OK;
@@ -139,7 +147,39 @@ static int query(const void* nodes, int64_t n, const float* queries, int64_t q, 
   }
   if (!nodes || !queries || misaligned(nodes) || misaligned(queries)) return BVH_ERR_INVALID_ARGUMENT;
   if (fill && !indices) return BVH_ERR_INVALID_ARGUMENT;  // nnz = 0 callers still pass a valid pointer
-  launch_traverse(static_cast<const Node*>(nodes), (int)n, queries, q, kind, fill, counts, offsets, indices, stream);
+  launch_traverse(static_cast<const Node*>(nodes), (int)n, queries, q, kind, fill, order, counts, offsets, indices, stream);
+  return check_launch();
+}
+
+__global__ void iota_kernel(uint32_t* order, int64_t q) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < q) order[i] = (uint32_t)i;
+}
+
+// Query order: 30-bit Morton code of each query centre in the frame of the root box, then the same
+// one-sweep sort as the build; `order` receives the permutation (query index at each Morton position).
+static int query_order(const void* nodes, int64_t n, const float* queries, int64_t q, int kind, uint32_t* order,
+                       void* scratch, size_t scratch_bytes, void* stream_) {
+  if (n < 0 || q < 0) return BVH_ERR_INVALID_ARGUMENT;
+  if (n >= ((int64_t)1 << 30) || q >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
+  if (q == 0) return BVH_OK;
+  if (!order) return BVH_ERR_INVALID_ARGUMENT;
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (n == 0) {  // no frame: identity
+    iota_kernel<<<(unsigned)((q + 255) / 256), 256, 0, stream>>>(order, q);
+    return check_launch();
+  }
+  if (!nodes || !queries || !scratch || misaligned(nodes) || misaligned(queries) || misaligned(scratch))
+    return BVH_ERR_INVALID_ARGUMENT;
+  const ScratchLayout L = scratch_layout(q, 30);
+  if (scratch_bytes < L.total) return BVH_ERR_SCRATCH;
+  char* base = static_cast<char*>(scratch);
+  if (cudaMemsetAsync(base, 0, L.zero_bytes, stream) != cudaSuccess) return BVH_ERR_CUDA;
+  SortBuffers B = sort_buffers(scratch, L);
+  launch_query_morton(queries, (int)q, kind, static_cast<const Node*>(nodes), static_cast<uint32_t*>(B.keys[0]), B.hist,
+                      stream);
+  B.final_vals = order;
+  launch_sort(B, 4, 4, (int)q, stream, nullptr);
   return check_launch();
 }
 
@@ -168,12 +208,36 @@ int bvh_build_boxes(const float* minmax, int64_t n, int morton_bits, void* nodes
   return bvh::build(minmax, true, n, morton_bits, nodes, scratch, scratch_bytes, stream);
 }
 
-int bvh_query_spheres_count(const void* nodes, int64_t n, const float* xyzr, int64_t q, int32_t* counts, void* stream) {
-  return bvh::query(nodes, n, xyzr, q, 0, false, counts, nullptr, nullptr, stream);
+int bvh_build_staged(const float* prim, int prim_is_box, int64_t n, int morton_bits, void* nodes, void* scratch,
+                     size_t scratch_bytes, void* stream, void* const* stage_events) {
+  return bvh::build(prim, prim_is_box != 0, n, morton_bits, nodes, scratch, scratch_bytes, stream, stage_events);
 }
 
-int bvh_query_boxes_count(const void* nodes, int64_t n, const float* minmax, int64_t q, int32_t* counts, void* stream) {
-  return bvh::query(nodes, n, minmax, q, 1, false, counts, nullptr, nullptr, stream);
+int bvh_query_order_sizes(int64_t q, size_t* scratch_bytes) {
+  if (q < 0 || !scratch_bytes) return BVH_ERR_INVALID_ARGUMENT;
+  if (q >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
+  *scratch_bytes = bvh::scratch_layout(q, 30).total;
+  return BVH_OK;
+}
+
+int bvh_query_order_spheres(const void* nodes, int64_t n, const float* xyzr, int64_t q, uint32_t* order, void* scratch,
+                            size_t scratch_bytes, void* stream) {
+  return bvh::query_order(nodes, n, xyzr, q, 0, order, scratch, scratch_bytes, stream);
+}
+
+int bvh_query_order_boxes(const void* nodes, int64_t n, const float* minmax, int64_t q, uint32_t* order, void* scratch,
+                          size_t scratch_bytes, void* stream) {
+  return bvh::query_order(nodes, n, minmax, q, 1, order, scratch, scratch_bytes, stream);
+}
+
+int bvh_query_spheres_count(const void* nodes, int64_t n, const float* xyzr, int64_t q, const uint32_t* order,
+                            int32_t* counts, void* stream) {
+  return bvh::query(nodes, n, xyzr, q, 0, false, order, counts, nullptr, nullptr, stream);
+}
+
+int bvh_query_boxes_count(const void* nodes, int64_t n, const float* minmax, int64_t q, const uint32_t* order,
+                          int32_t* counts, void* stream) {
+  return bvh::query(nodes, n, minmax, q, 1, false, order, counts, nullptr, nullptr, stream);
 }
 
 int bvh_scan_sizes(int64_t q, size_t* scratch_bytes) {
@@ -191,14 +255,14 @@ int bvh_scan_counts(const int32_t* counts, int64_t q, int64_t* offsets, void* sc
   return bvh::check_launch();
 }
 
-int bvh_query_spheres_fill(const void* nodes, int64_t n, const float* xyzr, int64_t q, const int64_t* offsets,
-                           int32_t* indices, void* stream) {
-  return bvh::query(nodes, n, xyzr, q, 0, true, nullptr, offsets, indices, stream);
+int bvh_query_spheres_fill(const void* nodes, int64_t n, const float* xyzr, int64_t q, const uint32_t* order,
+                           const int64_t* offsets, int32_t* indices, void* stream) {
+  return bvh::query(nodes, n, xyzr, q, 0, true, order, nullptr, offsets, indices, stream);
 }
 
-int bvh_query_boxes_fill(const void* nodes, int64_t n, const float* minmax, int64_t q, const int64_t* offsets,
-                         int32_t* indices, void* stream) {
-  return bvh::query(nodes, n, minmax, q, 1, true, nullptr, offsets, indices, stream);
+int bvh_query_boxes_fill(const void* nodes, int64_t n, const float* minmax, int64_t q, const uint32_t* order,
+                         const int64_t* offsets, int32_t* indices, void* stream) {
+  return bvh::query(nodes, n, minmax, q, 1, true, order, nullptr, offsets, indices, stream);
 }
 
 int bvh_export(const void* nodes, const void* scratch, int64_t n, int morton_bits, void* sorted_codes, uint32_t* perm,

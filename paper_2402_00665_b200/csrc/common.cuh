@@ -76,14 +76,32 @@ void launch_scene_bounds(const float* prim, int n, bool is_box, Header* header, 
 // K2: Morton codes + the digit histograms of every sort pass.
 void launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
                    uint32_t* hist, cudaStream_t stream);
-// K3: one-sweep LSD radix sort, all passes.  Result in keys[0] / vals[0] of the layout.
-void launch_sort(void* scratch, const ScratchLayout& L, int n, cudaStream_t stream);
+// K3: one-sweep LSD radix sort of (key, index) pairs, `passes` 8-bit digits from the least significant.
+// Pass p reads keys[p&1]/vals[p&1] and writes the other buffer; with an even pass count the result is in
+// keys[0]/vals[0].  final_vals (optional) receives the last pass's values instead of vals[...].
+// hist: [passes][256] digit histograms (already counted); status: [passes][tiles][256] zeroed; tile_counters:
+// [passes] zeroed.  pass_events: optional array of cudaEvent_t (as void*), entry p recorded after pass p.
+struct SortBuffers {
+  void* keys[2];
+  uint32_t* vals[2];
+  uint32_t* hist;
+  uint32_t* status;
+  uint32_t* tile_counters;
+  uint32_t* final_vals;
+};
+SortBuffers sort_buffers(void* scratch, const ScratchLayout& L);
+void launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStream_t stream, void* const* pass_events);
+// Morton codes (30-bit) of query centres in the frame of the root box + digit histograms: orders queries.
+void launch_query_morton(const float* queries, int q, int kind, const Node* root, uint32_t* codes, uint32_t* hist,
+                         cudaStream_t stream);
 // K4+K5: leaf gather + modified Apetrei bottom-up pass (Algorithm 4 with boxes).
 void launch_hierarchy(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
                       int* store, Node* nodes, int n, cudaStream_t stream);
 // K6/K8: stackless traversal.  kind 0 = spheres (xyzr), 1 = boxes (minmax).  fill: offsets/indices used.
-void launch_traverse(const Node* nodes, int n, const float* queries, int64_t q, int kind, bool fill, int32_t* counts,
-                     const int64_t* offsets, int32_t* indices, cudaStream_t stream);
+// order (optional): thread t serves query order[t] (results still land in row order[t]).
+void launch_traverse(const Node* nodes, int n, const float* queries, int64_t q, int kind, bool fill,
+                     const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* indices,
+                     cudaStream_t stream);
 // K7: exclusive scan of int32 counts into int64 offsets[q+1].
 size_t scan_scratch_bytes(int64_t q);
 void launch_scan(const int32_t* counts, int64_t q, int64_t* offsets, void* scratch, cudaStream_t stream);

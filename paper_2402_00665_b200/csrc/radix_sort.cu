@@ -80,24 +80,30 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_o
   }
 
   // ---- rank within the warp, in tile order ---------------------------------------------------------------
+  // peers = lanes of this warp holding the same digit, from one ballot per digit bit (a fixed 8 votes per
+  // item; __match_any_sync costs one round per DISTINCT digit in the warp, ~28 on uniformly random digits).
   uint32_t rank[ITEMS];
   const uint32_t lt_mask = (1u << lane) - 1u;
 #pragma unroll
   for (int j = 0; j < ITEMS; ++j) {
     const bool valid = (warp_off + j * 32) < valid_in_tile;
-    const uint32_t vm = __ballot_sync(0xffffffffu, valid);
-    if (valid) {
-      const uint32_t d = (uint32_t)(key[j] >> shift) & 0xFFu;
-      const uint32_t peers = __match_any_sync(vm, d);
-      const int leader = __ffs(peers) - 1;
-      uint32_t pre = 0;
-      if (lane == leader) {
-        pre = s_warp_hist[warp][d];
-        s_warp_hist[warp][d] = pre + __popc(peers);
-      }
-      pre = __shfl_sync(peers, pre, leader);
-      rank[j] = pre + __popc(peers & lt_mask);
+    const uint32_t d = (uint32_t)(key[j] >> shift) & 0xFFu;
+    uint32_t peers = __ballot_sync(0xffffffffu, valid);
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+      const bool bit = (d >> b) & 1u;
+      const uint32_t bal = __ballot_sync(0xffffffffu, bit);
+      peers &= bit ? bal : ~bal;
     }
+    if (!valid) peers = 0;
+    const int leader = peers ? (__ffs(peers) - 1) : lane;
+    uint32_t pre = 0;
+    if (valid && lane == leader) {
+      pre = s_warp_hist[warp][d];
+      s_warp_hist[warp][d] = pre + __popc(peers);
+    }
+    pre = __shfl_sync(0xffffffffu, pre, leader);
+    rank[j] = pre + __popc(peers & lt_mask);
     __syncwarp();
   }
   __syncthreads();
@@ -190,31 +196,42 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_o
 }
 
 template <typename KeyT>
-static void sort_all(void* scratch, const ScratchLayout& L, int n, cudaStream_t stream) {
-  char* base = static_cast<char*>(scratch);
-  Header* header = reinterpret_cast<Header*>(base + L.header);
-  uint32_t* hist = reinterpret_cast<uint32_t*>(base + L.hist);
-  uint32_t* status = reinterpret_cast<uint32_t*>(base + L.status);
-  KeyT* keys[2] = {reinterpret_cast<KeyT*>(base + L.keys[0]), reinterpret_cast<KeyT*>(base + L.keys[1])};
-  uint32_t* vals[2] = {reinterpret_cast<uint32_t*>(base + L.vals[0]), reinterpret_cast<uint32_t*>(base + L.vals[1])};
-  const int tiles = L.tiles;
-  for (int p = 0; p < L.passes; ++p) {
+static void sort_all(const SortBuffers& B, int n, int passes, cudaStream_t stream, void* const* pass_events) {
+  const int tiles = (n + SortCfg<KeyT>::TILE - 1) / SortCfg<KeyT>::TILE;
+  KeyT* keys[2] = {static_cast<KeyT*>(B.keys[0]), static_cast<KeyT*>(B.keys[1])};
+  for (int p = 0; p < passes; ++p) {
     const int in = p & 1, out = in ^ 1;
-    uint32_t* st = status + (size_t)p * tiles * 256;
+    uint32_t* st = B.status + (size_t)p * tiles * 256;
+    uint32_t* vout = (p == passes - 1 && B.final_vals) ? B.final_vals : B.vals[out];
     if (p == 0)
       onesweep_pass_kernel<KeyT, true><<<tiles, kSortThreads, 0, stream>>>(
-          keys[in], keys[out], nullptr, vals[out], hist + p * 256, st, &header->tile_counter[p], n, 8 * p);
+          keys[in], keys[out], nullptr, vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
     else
       onesweep_pass_kernel<KeyT, false><<<tiles, kSortThreads, 0, stream>>>(
-          keys[in], keys[out], vals[in], vals[out], hist + p * 256, st, &header->tile_counter[p], n, 8 * p);
+          keys[in], keys[out], B.vals[in], vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
+    if (pass_events && pass_events[p]) cudaEventRecord(static_cast<cudaEvent_t>(pass_events[p]), stream);
   }
 }
 
-void launch_sort(void* scratch, const ScratchLayout& L, int n, cudaStream_t stream) {
-  if (L.key_bytes == 4)
-    sort_all<uint32_t>(scratch, L, n, stream);
+SortBuffers sort_buffers(void* scratch, const ScratchLayout& L) {
+  char* base = static_cast<char*>(scratch);
+  SortBuffers B{};
+  B.keys[0] = base + L.keys[0];
+  B.keys[1] = base + L.keys[1];
+  B.vals[0] = reinterpret_cast<uint32_t*>(base + L.vals[0]);
+  B.vals[1] = reinterpret_cast<uint32_t*>(base + L.vals[1]);
+  B.hist = reinterpret_cast<uint32_t*>(base + L.hist);
+  B.status = reinterpret_cast<uint32_t*>(base + L.status);
+  B.tile_counters = reinterpret_cast<Header*>(base + L.header)->tile_counter;
+  B.final_vals = nullptr;
+  return B;
+}
+
+void launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStream_t stream, void* const* pass_events) {
+  if (key_bytes == 4)
+    sort_all<uint32_t>(B, n, passes, stream, pass_events);
   else
-    sort_all<uint64_t>(scratch, L, n, stream);
+    sort_all<uint64_t>(B, n, passes, stream, pass_events);
 }
 
 }  // namespace bvh

@@ -44,9 +44,13 @@ struct BoxQuery {
 template <typename Query, bool FILL>
 __global__ void __launch_bounds__(kTravThreads)
 traverse_kernel(const Node* __restrict__ nodes, int n, const float* __restrict__ queries, int64_t q,
-                int32_t* __restrict__ counts, const int64_t* __restrict__ offsets, int32_t* __restrict__ indices) {
-  const int64_t j = (int64_t)blockIdx.x * kTravThreads + threadIdx.x;
-  if (j >= q) return;
+                const uint32_t* __restrict__ order, int32_t* __restrict__ counts, const int64_t* __restrict__ offsets,
+                int32_t* __restrict__ indices) {
+  const int64_t t = (int64_t)blockIdx.x * kTravThreads + threadIdx.x;
+  if (t >= q) return;
+  // Neighbouring threads serve queries that are neighbours on the Morton curve when `order` is given: they
+  // walk nearly the same nodes, which is what keeps the node reads in L1/L2 (PAPER.md:15-17 data divergence).
+  const int64_t j = order ? (int64_t)order[t] : t;
   Query query;
   query.load(queries, j);
   const int leaf_base = n - 1;
@@ -70,19 +74,20 @@ traverse_kernel(const Node* __restrict__ nodes, int n, const float* __restrict__
   if (!FILL) counts[j] = count;
 }
 
-void launch_traverse(const Node* nodes, int n, const float* queries, int64_t q, int kind, bool fill, int32_t* counts,
-                     const int64_t* offsets, int32_t* indices, cudaStream_t stream) {
+void launch_traverse(const Node* nodes, int n, const float* queries, int64_t q, int kind, bool fill,
+                     const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* indices,
+                     cudaStream_t stream) {
   const unsigned g = (unsigned)((q + kTravThreads - 1) / kTravThreads);
   if (kind == 0) {
     if (fill)
-      traverse_kernel<SphereQuery, true><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, counts, offsets, indices);
+      traverse_kernel<SphereQuery, true><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, order, counts, offsets, indices);
     else
-      traverse_kernel<SphereQuery, false><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, counts, offsets, indices);
+      traverse_kernel<SphereQuery, false><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, order, counts, offsets, indices);
   } else {
     if (fill)
-      traverse_kernel<BoxQuery, true><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, counts, offsets, indices);
+      traverse_kernel<BoxQuery, true><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, order, counts, offsets, indices);
     else
-      traverse_kernel<BoxQuery, false><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, counts, offsets, indices);
+      traverse_kernel<BoxQuery, false><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, order, counts, offsets, indices);
   }
 }
 

@@ -169,38 +169,41 @@ FULL_SIZES = {
 C5_RADIUS_FULL = 0.00606  # 32 = (2**24 / 0.488) * (4/3) pi r^3
 
 
-def make(name: str, n: int | None = None, q: int | None = None, radius: float | None = None) -> Workload:
+def make(name: str, n: int | None = None, q: int | None = None, radius: float | None = None,
+         seed_offset: int = 0) -> Workload:
     """Build config ``name`` ("C1".."C5").  ``n``/``q`` override the full sizes (same distribution, same
     seeds, just fewer draws), ``radius`` overrides the query radius / half-edge scale; scaled-down cases
-    are what the parity tests use.  q=0 gives a build-only workload."""
+    are what the parity tests use.  q=0 gives a build-only workload.  ``seed_offset`` r adds 10000*r to every seed
+    (independent replicas for the multi-GPU bench)."""
+    so = 10000 * int(seed_offset)
     fn, fq = FULL_SIZES[name]
     n = fn if n is None else n
     q = fq if q is None else q
     if name == "C1":
         # 4096 fp32 points uniform in [0,1)^3 (seed 0) as degenerate AABBs, 30-bit; spheres on the points.
-        pts = uniform_cube(n, seed=0)
+        pts = uniform_cube(n, seed=0 + so)
         r = 0.085 if radius is None else radius
-        centres = pts[:q] if q <= n else uniform_cube(q, seed=0)
+        centres = pts[:q] if q <= n else uniform_cube(q, seed=0 + so)
         return Workload(name, boxes_around(pts, 0.0), "boxes", 30, spheres_at(centres, r) if q else None,
                         "spheres" if q else None, "uniform cube, degenerate boxes")
     if name == "C2":
-        pts = uniform_cube(n, seed=2)
+        pts = uniform_cube(n, seed=2 + so)
         r = 0.0157 if radius is None else radius
-        return Workload(name, pts, "points", 63, spheres_at(uniform_cube(q, seed=1002), r) if q else None,
+        return Workload(name, pts, "points", 63, spheres_at(uniform_cube(q, seed=1002 + so), r) if q else None,
                         "spheres" if q else None, "uniform cube")
     if name == "C3":
-        pts = gaussian_mixture(n, seed=3, centre_seed=3)
+        pts = gaussian_mixture(n, seed=3 + so, centre_seed=3 + so)
         r = 0.002 if radius is None else radius
-        qs = spheres_at(gaussian_mixture(q, seed=1003, centre_seed=3), r) if q else None
+        qs = spheres_at(gaussian_mixture(q, seed=1003 + so, centre_seed=3 + so), r) if q else None
         return Workload(name, pts, "points", 30, qs, "spheres" if q else None, "100-component mixture, sigma 0.005")
     if name == "C4":
         h = 5e-4 if radius is None else radius
-        prims = boxes_around(sphere_surface(n, seed=4), h)
-        qs = boxes_around(sphere_surface(q, seed=1004), 2.0 * h) if q else None
+        prims = boxes_around(sphere_surface(n, seed=4 + so), h)
+        qs = boxes_around(sphere_surface(q, seed=1004 + so), 2.0 * h) if q else None
         return Workload(name, prims, "boxes", 63, qs, "boxes" if q else None, "boxes on the unit sphere surface")
     if name == "C5":
-        pts = hollow_shell(n, seed=5)
+        pts = hollow_shell(n, seed=5 + so)
         r = C5_RADIUS_FULL if radius is None else radius
-        qs = spheres_at(hollow_shell(q, seed=1005), r) if q else None
+        qs = spheres_at(hollow_shell(q, seed=1005 + so), r) if q else None
         return Workload(name, pts, "points", 63, qs, "spheres" if q else None, "hollow cube shell")
     raise KeyError(name)

@@ -31,7 +31,7 @@ def test_header_symbols_exported_and_bound(lib):
     from paper_2402_00665_b200 import binding
 
     names = _declared()
-    assert len(names) >= 11
+    assert len(names) >= 15
     for name in names:
         assert hasattr(lib, name), name
         assert name in binding.SYMBOLS, f"{name} not bound"
@@ -64,8 +64,11 @@ def test_sizes_and_errors_host_only(lib):
     assert f(None, 0, 30, None, None, 0, None) == 0             # n = 0 is a valid no-op
     assert f(ctypes.c_void_p(16), 10, 30, ctypes.c_void_p(64), ctypes.c_void_p(256), 16, None) == -4   # scratch too small
     assert f(ctypes.c_void_p(8), 10, 30, ctypes.c_void_p(64), ctypes.c_void_p(256), 1 << 30, None) == -1  # misaligned
-    assert lib.bvh_query_spheres_count(None, 5, None, -1, None, None) == -1
-    assert lib.bvh_query_spheres_count(None, 5, None, 0, None, None) == 0
+    assert lib.bvh_query_spheres_count(None, 5, None, -1, None, None, None) == -1
+    assert lib.bvh_query_spheres_count(None, 5, None, 0, None, None, None) == 0
+    assert binding.bvh_query_order_sizes(1000) >= 1000 * 16
+    assert lib.bvh_query_order_spheres(None, 5, None, 0, None, None, 0, None) == 0
+    assert lib.bvh_query_order_spheres(None, 5, None, 7, None, None, 0, None) == -1
 
 
 def test_binding_refuses_cpu_tensors(lib):

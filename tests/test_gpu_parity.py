@@ -206,6 +206,33 @@ def test_structural_invariants_large(B, oracle_lib):
     assert np.all(gs == gl + 1)
 
 
+def test_query_order_is_a_permutation_and_does_not_change_results(B):
+    w = W.make("C3", n=150_000, q=40_000, radius=0.004)
+    bvh = gpu_build(B, w.prims, w.morton_bits)
+    dq = _dev(w.queries)
+    ws = B.QueryWorkspace(w.q)
+    o1, i1 = B.query(bvh, dq, ws, ordered=True)
+    torch.cuda.synchronize()
+    order = ws.order.cpu().numpy().view(np.uint32)
+    assert np.array_equal(np.sort(order), np.arange(w.q, dtype=np.uint32))
+    o1, i1 = o1.cpu().numpy().copy(), i1.cpu().numpy().copy()
+    o2, i2 = B.query(bvh, dq, ws, ordered=False)
+    torch.cuda.synchronize()
+    assert np.array_equal(o1, o2.cpu().numpy()) and np.array_equal(i1, i2.cpu().numpy())
+    # box queries too, including queries whose centroid lies outside the scene box (clamped for ordering only)
+    wb = W.make("C4", n=60_000, q=20_000, radius=4e-3)
+    bvh = gpu_build(B, wb.prims, wb.morton_bits)
+    qs = wb.queries.copy()
+    qs[:100] += np.float32(3.0)
+    qs[100:200, 3:] += np.float32(5.0)
+    dq = _dev(qs)
+    o1, i1 = B.query(bvh, dq, ordered=True)
+    o2, i2 = B.query(bvh, dq, ordered=False)
+    torch.cuda.synchronize()
+    assert torch.equal(o1, o2) and torch.equal(i1, i2)
+    assert int(o1[100]) == 0 and int(o1[-1]) > 0
+
+
 def test_empty_inputs(B):
     bvh = B.Bvh(0, 30)
     bvh.build(torch.zeros((0, 3), dtype=torch.float32, device="cuda"))
