@@ -35,14 +35,17 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if force or _stale():
+def build(force: bool = False, verbose: bool = False, out: str | None = None, extra: list[str] | None = None) -> str:
+    """Build the library.  ``out``/``extra`` (another output path, extra nvcc flags such as -DBVH_SCAN_LEAVES=8)
+    are for tuning sweeps; the product is the default build."""
+    target = out or LIB
+    if force or out or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), *sources(), "-o", tmp]
+        tmp = target + f".tmp{os.getpid()}"
+        cmd = [nvcc, *NVCC_FLAGS, *(extra or []), *(["-Xptxas", "-v"] if verbose else []), *sources(), "-o", tmp]
         subprocess.check_call(cmd)
-        os.replace(tmp, LIB)
-    return LIB
+        os.replace(tmp, target)
+    return target
 
 
 if __name__ == "__main__":
