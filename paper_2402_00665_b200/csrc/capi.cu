@@ -33,6 +33,9 @@ ScratchLayout scratch_layout(int64_t n, int morton_bits) {
     L.vals[b] = off;
     off += align_up(nn * sizeof(uint32_t), 256);
   }
+  L.queue = off;
+  L.queue_capacity = hierarchy_queue_capacity((int)nn);
+  off += align_up((size_t)L.queue_capacity * sizeof(int2), 256);
   L.total = off;
   return L;
 }
@@ -122,7 +125,8 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   mark(3);
   launch_sort(sort_buffers(scratch, L), L.key_bytes, L.passes, (int)n, stream, events ? events + 4 : nullptr);
   launch_hierarchy(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
-                   store, static_cast<Node*>(nodes), (int)n, stream);
+                   store, static_cast<Node*>(nodes), (int)n, reinterpret_cast<int2*>(base + L.queue),
+                   &header->queue_count, stream);
   mark(12);
   return check_launch();
 }

@@ -27,7 +27,9 @@ struct ScratchLayout {
   size_t store;         // int32 [n]  Algorithm 4's `store` (n-1 used), initialised to -1
   size_t keys[2];       // KeyT [n]   ping-pong; sorted codes end in keys[0]
   size_t vals[2];       // uint32 [n] ping-pong; permutation ends in vals[0]
+  size_t queue;         // int2 [queue_capacity]  nodes handed from the block-local to the global bottom-up phase
   size_t total;
+  int queue_capacity;
   int passes;
   int tiles;
   int key_bytes;
@@ -36,7 +38,8 @@ struct ScratchLayout {
 struct Header {
   uint32_t bounds_enc[8];    // [0..2] = ~ord(min.xyz), [3..5] = ord(max.xyz), maximised with atomicMax
   uint32_t tile_counter[8];  // one dynamic tile counter per sort pass
-  uint32_t pad[48];
+  uint32_t queue_count;      // entries in the bottom-up pass's hand-over queue
+  uint32_t pad[47];
 };
 static_assert(sizeof(Header) == 256, "header is one 256-byte block");
 
@@ -96,7 +99,8 @@ void launch_query_morton(const float* queries, int q, int kind, const Node* root
                          cudaStream_t stream);
 // K4+K5: leaf gather + modified Apetrei bottom-up pass (Algorithm 4 with boxes).
 void launch_hierarchy(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
-                      int* store, Node* nodes, int n, cudaStream_t stream);
+                      int* store, Node* nodes, int n, int2* queue, uint32_t* queue_count, cudaStream_t stream);
+int hierarchy_queue_capacity(int n);
 // K6/K8: stackless traversal.  kind 0 = spheres (xyzr), 1 = boxes (minmax).  fill: offsets/indices used.
 // order (optional): thread t serves query order[t] (results still land in row order[t]).
 void launch_traverse(const Node* nodes, int n, const float* queries, int64_t q, int kind, bool fill,

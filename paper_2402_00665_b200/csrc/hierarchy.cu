@@ -11,7 +11,10 @@
 
 namespace bvh {
 
-constexpr int kHierThreads = 256;
+#ifndef BVH_HIER_THREADS
+#define BVH_HIER_THREADS 512
+#endif
+constexpr int kHierThreads = BVH_HIER_THREADS;  // leaves per block = size of the shared-memory phase
 
 // delta*(i): XOR of adjacent sorted codes; equal codes fall back to the XOR of the
 // sorted positions (augmented key, readings G1/G5); +infinity outside [0, n-2].  The
@@ -43,104 +46,255 @@ __device__ __forceinline__ typename Delta<KeyT>::T delta_star(const KeyT* __rest
   return Delta<KeyT>::make(codes[i], codes[i + 1], i);
 }
 
-__device__ __forceinline__ void store_node(Node* nodes, int idx, float lo0, float lo1, float lo2, float hi0, float hi1,
-                                           float hi2, int left, int rope) {
-  float4* p = reinterpret_cast<float4*>(nodes + idx);
-  p[0] = make_float4(lo0, lo1, lo2, __int_as_float(left));
-  p[1] = make_float4(hi0, hi1, hi2, __int_as_float(rope));
+__device__ __forceinline__ void store_node(Node* nodes, int idx, const float lo[3], const float hi[3], int left, int rope) {
+  // one 256-bit store = one full 32-byte sector (STG.E.ENL2.256, sm_100)
+  asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(nodes + idx), "f"(lo[0]), "f"(lo[1]), "f"(lo[2]),
+               "f"(__int_as_float(left)), "f"(hi[0]), "f"(hi[1]), "f"(hi[2]), "f"(__int_as_float(rope))
+               : "memory");
 }
 
+// The pass runs in two phases per block of kHierThreads consecutive leaves [c0, c_last].
+//
+// Phase 1 (shared memory).  The block stages delta* of its leaves (and one neighbour on each side), its leaf
+// boxes, a private copy of `store` and a box slot per local internal node in shared memory and runs
+// Algorithm 4 there: the CAS is a shared-memory atomic, the sibling's box a shared-memory read, ordered by
+// __threadfence_block().  A thread leaves this phase when (a) it is the first to arrive at a parent (L13 /
+// L18: it may be done, or its sibling may be a node that straddles the block boundary and can only arrive
+// through global memory), or (b) its parent's split lies on the block boundary.  Internal nodes are still
+// written to global memory as they are created (each exactly once, by the thread that merged its children).
+//
+// Phase 2 (global memory), after one __syncthreads().  A thread of kind (a) whose sibling did arrive locally
+// (its `store` slot was marked) is done; every other thread that left phase 1 carries on with Algorithm 4 on
+// the global `store` exactly as the paper states it (release fence, ATOMICCAS, acquire fence, sibling box
+// through L2).  Only nodes whose range straddles a block boundary are created here: a few per block.
+// Any two children of a parent meet either both in shared memory or both in global memory, so exactly one
+// thread survives each node and the result is the same unique hierarchy.
 template <typename KeyT, bool IS_BOX>
 __global__ void __launch_bounds__(kHierThreads)
-hierarchy_kernel(const float* __restrict__ prim, const KeyT* __restrict__ codes, const uint32_t* __restrict__ perm,
-                 int* store, Node* nodes, int n) {
+hierarchy_local_kernel(const float* __restrict__ prim, const KeyT* __restrict__ codes,
+                       const uint32_t* __restrict__ perm, Node* nodes, int n, int2* __restrict__ queue,
+                       uint32_t* __restrict__ queue_count) {
   using D = typename Delta<KeyT>::T;
-  const int i0 = blockIdx.x * kHierThreads + threadIdx.x;
-  if (i0 >= n) return;
+  constexpr int C = kHierThreads;
+  __shared__ uint32_t s_wsum[C / 32];
+  __shared__ uint32_t s_qbase;
+  __shared__ D s_delta[C + 2];      // s_delta[k] = delta*(c0 - 1 + k)
+  __shared__ int s_store[C];        // s_store[p - c0]: -1 empty, >= 0 first arrival's range bound, -2 both arrived
+  __shared__ float s_leaf[6][C];    // leaf boxes, by local leaf index
+  __shared__ float s_int[6][C];     // internal boxes, by local Karras index q - c0
+
+  const int tid = threadIdx.x;
+  const int c0 = blockIdx.x * C;
+  const int c_last = min(c0 + C, n) - 1;
+  const int i = c0 + tid;
+  const bool valid = i < n;
   const int leaf_base = n - 1;
-  int i = i0;
+
+  s_delta[tid + 1] = delta_star<KeyT>(codes, i, n);
+  if (tid == 0) s_delta[0] = delta_star<KeyT>(codes, c0 - 1, n);
+  if (tid == C - 1) s_delta[C + 1] = delta_star<KeyT>(codes, c0 + C, n);
+  s_store[tid] = kInvalid;                                  // L1
+
+  // K4: leaf box = box of the primitive sorted to position i
+  float lo[3] = {0.f, 0.f, 0.f}, hi[3] = {0.f, 0.f, 0.f};
+  uint32_t orig = 0;
+  if (valid) {
+    orig = perm[i];
+    if (IS_BOX) {
+      const float2* p = reinterpret_cast<const float2*>(prim + 6 * (size_t)orig);
+      const float2 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
+      lo[0] = a.x; lo[1] = a.y; lo[2] = b.x; hi[0] = b.y; hi[1] = c.x; hi[2] = c.y;
+    } else {
+      const float* p = prim + 3 * (size_t)orig;
+      lo[0] = hi[0] = __ldg(p);
+      lo[1] = hi[1] = __ldg(p + 1);
+      lo[2] = hi[2] = __ldg(p + 2);
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      s_leaf[a][tid] = lo[a];
+      s_leaf[3 + a][tid] = hi[a];
+    }
+  }
+  __syncthreads();
 
   // L3-4
   int range_left = i, range_right = i;
-  D delta_left = delta_star<KeyT>(codes, i - 1, n);
-  D delta_right = delta_star<KeyT>(codes, i, n);
-
-  // leaf box = box of the primitive sorted to position i (K4)
-  const uint32_t orig = perm[i];
-  float lo[3], hi[3];
-  if (IS_BOX) {
-    const float2* p = reinterpret_cast<const float2*>(prim + 6 * (size_t)orig);
-    const float2 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
-    lo[0] = a.x; lo[1] = a.y; lo[2] = b.x; hi[0] = b.y; hi[1] = c.x; hi[2] = c.y;
-  } else {
-    const float* p = prim + 3 * (size_t)orig;
-    lo[0] = hi[0] = __ldg(p);
-    lo[1] = hi[1] = __ldg(p + 1);
-    lo[2] = hi[2] = __ldg(p + 2);
-  }
-  // L5-8: leaf skip-connection
-  int rope;
-  if (i == n - 1)
-    rope = kSentinel;
-  else
-    rope = (delta_right < delta_star<KeyT>(codes, i + 1, n)) ? leaf_base + i + 1 : i + 1;
-  store_node(nodes, leaf_base + i, lo[0], lo[1], lo[2], hi[0], hi[1], hi[2], (int)orig, rope);
-  if (n == 1) return;  // G11
-
-  // L9-28
-  do {
-    // the node this thread carries (leaf or internal `i`) is fully written: publish before arriving
-    __threadfence();
-    int p, sibling;
-    if (delta_right < delta_left) {       // L10: left child of its parent
-      p = range_right;                    // L11: Apetrei index
-      const int other = atomicCAS(&store[p], kInvalid, range_left);  // L12
-      if (other == kInvalid) return;      // L13: first to arrive
-      range_right = other;
-      sibling = (range_right == p + 1) ? leaf_base + p + 1 : p + 1;  // right child: L_{p+1} or I_{p+1}
-      delta_right = delta_star<KeyT>(codes, range_right, n);  // L14
-    } else {                              // right child of its parent
-      p = range_left - 1;                 // L16
-      const int other = atomicCAS(&store[p], kInvalid, range_right);  // L17
-      if (other == kInvalid) return;      // L18
-      range_left = other;
-      sibling = (range_left == p) ? leaf_base + p : p;               // left child: L_p or I_p
-      delta_left = delta_star<KeyT>(codes, range_left - 1, n);  // L19
-    }
-    __threadfence();  // acquire side: the sibling's record was written before its CAS
-    const float4 slo = __ldcg(reinterpret_cast<const float4*>(nodes + sibling));
-    const float4 shi = __ldcg(reinterpret_cast<const float4*>(nodes + sibling) + 1);
-    lo[0] = fminf(lo[0], slo.x); lo[1] = fminf(lo[1], slo.y); lo[2] = fminf(lo[2], slo.z);
-    hi[0] = fmaxf(hi[0], shi.x); hi[1] = fmaxf(hi[1], shi.y); hi[2] = fmaxf(hi[2], shi.z);
-
-    const int q = (delta_right < delta_left) ? range_right : range_left;       // L20: Karras index
-    const int left = (range_left == p) ? leaf_base + p : p;                    // L21 (reading G2)
-    if (range_right == n - 1) {                                                // L22-23
+  D delta_left = s_delta[tid], delta_right = s_delta[tid + 1];
+  bool go_global = false;
+  int pending_p = -1;
+  if (valid) {
+    // L5-8: leaf skip-connection
+    int rope;
+    if (i == n - 1)
       rope = kSentinel;
-    } else {
-      const int r = range_right + 1;                                           // L25
-      rope = (delta_right < delta_star<KeyT>(codes, r, n)) ? leaf_base + r : r;  // L26
+    else
+      rope = (delta_right < s_delta[tid + 2]) ? leaf_base + i + 1 : i + 1;
+    store_node(nodes, leaf_base + i, lo, hi, (int)orig, rope);
+
+    // ---- phase 1: L9-28 on shared memory ----
+    if (n > 1) {  // G11
+      while (true) {
+        const bool is_left = delta_right < delta_left;                    // L10
+        const int p = is_left ? range_right : range_left - 1;             // L11 / L16: Apetrei index
+        const bool interior = is_left ? (range_right < c_last) : (range_left > c0);
+        if (!interior) {
+          go_global = true;
+          break;
+        }
+        const int other = atomicCAS(&s_store[p - c0], kInvalid, is_left ? range_left : range_right);  // L12 / L17
+        if (other == kInvalid) {                                          // L13 / L18: first to arrive here
+          pending_p = p;
+          break;
+        }
+        s_store[p - c0] = -2;
+        bool sib_leaf;
+        int sib;
+        if (is_left) {
+          range_right = other;
+          sib_leaf = (range_right == p + 1);
+          sib = p + 1 - c0;
+          delta_right = s_delta[range_right - c0 + 1];                    // L14
+        } else {
+          range_left = other;
+          sib_leaf = (range_left == p);
+          sib = p - c0;
+          delta_left = s_delta[range_left - c0];                          // L19
+        }
+        __threadfence_block();
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+          lo[a] = fminf(lo[a], sib_leaf ? s_leaf[a][sib] : s_int[a][sib]);
+          hi[a] = fmaxf(hi[a], sib_leaf ? s_leaf[3 + a][sib] : s_int[3 + a][sib]);
+        }
+        const int q = (delta_right < delta_left) ? range_right : range_left;   // L20: Karras index
+        const int left = (range_left == p) ? leaf_base + p : p;                // L21 (reading G2)
+        if (range_right == n - 1)                                              // L22-23
+          rope = kSentinel;
+        else                                                                   // L25-26
+          rope = (delta_right < s_delta[range_right - c0 + 2]) ? leaf_base + range_right + 1 : range_right + 1;
+        store_node(nodes, q, lo, hi, left, rope);
+        if (q == 0) break;                                                     // L28 (whole tree inside this block)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+          s_int[a][q - c0] = lo[a];
+          s_int[3 + a][q - c0] = hi[a];
+        }
+        __threadfence_block();
+      }
     }
-    store_node(nodes, q, lo[0], lo[1], lo[2], hi[0], hi[1], hi[2], left, rope);
-    i = q;                                                                     // L27
-  } while (i != 0);                                                            // L28
+  }
+  __syncthreads();
+  if (pending_p >= 0 && s_store[pending_p - c0] != -2) go_global = true;     // my sibling never came locally
+
+  // The survivors (maximal nodes of the tree inside this block: at most 2 x tree height of them) go to a
+  // compact queue; the global phase runs as its own dense kernel instead of keeping this block resident.
+  const uint32_t m = __ballot_sync(0xffffffffu, go_global);
+  const int lane = tid & 31, warp = tid >> 5;
+  if (lane == 0) s_wsum[warp] = __popc(m);
+  __syncthreads();
+  if (tid == 0) {
+    uint32_t total = 0;
+    for (int w = 0; w < C / 32; ++w) {
+      const uint32_t c = s_wsum[w];
+      s_wsum[w] = total;
+      total += c;
+    }
+    s_qbase = total ? atomicAdd(queue_count, total) : 0u;
+  }
+  __syncthreads();
+  if (go_global) queue[s_qbase + s_wsum[warp] + __popc(m & ((1u << lane) - 1u))] = make_int2(range_left, range_right);
+}
+
+// Phase 2: Algorithm 4 on global memory for the queued nodes (those whose parent straddles a block boundary).
+template <typename KeyT>
+__global__ void __launch_bounds__(256)
+hierarchy_global_kernel(const KeyT* __restrict__ codes, int* store, Node* nodes, int n, const int2* __restrict__ queue,
+                        const uint32_t* __restrict__ queue_count) {
+  using D = typename Delta<KeyT>::T;
+  const int leaf_base = n - 1;
+  const uint32_t count = *queue_count;
+  for (uint32_t item = blockIdx.x * blockDim.x + threadIdx.x; item < count; item += gridDim.x * blockDim.x) {
+    const int2 range = queue[item];
+    int range_left = range.x, range_right = range.y;
+    D delta_left = delta_star<KeyT>(codes, range_left - 1, n);
+    D delta_right = delta_star<KeyT>(codes, range_right, n);
+    // the node this item carries: a leaf, or the internal node with that range (Karras index, L20)
+    const int carried = (range_left == range_right) ? leaf_base + range_left
+                                                    : ((delta_right < delta_left) ? range_right : range_left);
+    float lo[3], hi[3];
+    {
+      const float4 a = __ldcg(reinterpret_cast<const float4*>(nodes + carried));
+      const float4 b = __ldcg(reinterpret_cast<const float4*>(nodes + carried) + 1);
+      lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; hi[0] = b.x; hi[1] = b.y; hi[2] = b.z;
+    }
+    bool first_round = true;
+    while (true) {
+      // the node this thread carries is fully written: publish before arriving (the previous kernel's writes
+      // are already visible; a fence is only needed for nodes written in this kernel)
+      if (!first_round) __threadfence();
+      first_round = false;
+      int p, sibling;
+      if (delta_right < delta_left) {       // L10: left child of its parent
+        p = range_right;                    // L11: Apetrei index
+        const int other = atomicCAS(&store[p], kInvalid, range_left);  // L12
+        if (other == kInvalid) break;       // L13: first to arrive
+        range_right = other;
+        sibling = (range_right == p + 1) ? leaf_base + p + 1 : p + 1;  // right child: L_{p+1} or I_{p+1}
+        delta_right = delta_star<KeyT>(codes, range_right, n);  // L14
+      } else {                              // right child of its parent
+        p = range_left - 1;                 // L16
+        const int other = atomicCAS(&store[p], kInvalid, range_right);  // L17
+        if (other == kInvalid) break;       // L18
+        range_left = other;
+        sibling = (range_left == p) ? leaf_base + p : p;               // left child: L_p or I_p
+        delta_left = delta_star<KeyT>(codes, range_left - 1, n);  // L19
+      }
+      __threadfence();  // acquire side: the sibling's record was written before its CAS
+      const float4 slo = __ldcg(reinterpret_cast<const float4*>(nodes + sibling));
+      const float4 shi = __ldcg(reinterpret_cast<const float4*>(nodes + sibling) + 1);
+      lo[0] = fminf(lo[0], slo.x); lo[1] = fminf(lo[1], slo.y); lo[2] = fminf(lo[2], slo.z);
+      hi[0] = fmaxf(hi[0], shi.x); hi[1] = fmaxf(hi[1], shi.y); hi[2] = fmaxf(hi[2], shi.z);
+
+      const int q = (delta_right < delta_left) ? range_right : range_left;       // L20: Karras index
+      const int left = (range_left == p) ? leaf_base + p : p;                    // L21 (reading G2)
+      int rope;
+      if (range_right == n - 1) {                                                // L22-23
+        rope = kSentinel;
+      } else {
+        const int r = range_right + 1;                                           // L25
+        rope = (delta_right < delta_star<KeyT>(codes, r, n)) ? leaf_base + r : r;  // L26
+      }
+      store_node(nodes, q, lo, hi, left, rope);
+      if (q == 0) break;                                                         // L27-28
+    }
+  }
+}
+
+int hierarchy_queue_capacity(int n) {
+  const int blocks = (n + kHierThreads - 1) / kHierThreads;
+  const int per_block = kHierThreads < 192 ? kHierThreads : 192;  // <= 2 x tree height (93 bits of augmented key)
+  return blocks * per_block;
 }
 
 void launch_hierarchy(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
-                      int* store, Node* nodes, int n, cudaStream_t stream) {
+                      int* store, Node* nodes, int n, int2* queue, uint32_t* queue_count, cudaStream_t stream) {
   const unsigned g = (unsigned)((n + kHierThreads - 1) / kHierThreads);
+  const unsigned g2 = kNumSMs * 4;
   if (key_bytes == 4) {
     const uint32_t* c = static_cast<const uint32_t*>(sorted_codes);
     if (is_box)
-      hierarchy_kernel<uint32_t, true><<<g, kHierThreads, 0, stream>>>(prim, c, perm, store, nodes, n);
+      hierarchy_local_kernel<uint32_t, true><<<g, kHierThreads, 0, stream>>>(prim, c, perm, nodes, n, queue, queue_count);
     else
-      hierarchy_kernel<uint32_t, false><<<g, kHierThreads, 0, stream>>>(prim, c, perm, store, nodes, n);
+      hierarchy_local_kernel<uint32_t, false><<<g, kHierThreads, 0, stream>>>(prim, c, perm, nodes, n, queue, queue_count);
+    hierarchy_global_kernel<uint32_t><<<g2, 256, 0, stream>>>(c, store, nodes, n, queue, queue_count);
   } else {
     const uint64_t* c = static_cast<const uint64_t*>(sorted_codes);
     if (is_box)
-      hierarchy_kernel<uint64_t, true><<<g, kHierThreads, 0, stream>>>(prim, c, perm, store, nodes, n);
+      hierarchy_local_kernel<uint64_t, true><<<g, kHierThreads, 0, stream>>>(prim, c, perm, nodes, n, queue, queue_count);
     else
-      hierarchy_kernel<uint64_t, false><<<g, kHierThreads, 0, stream>>>(prim, c, perm, store, nodes, n);
+      hierarchy_local_kernel<uint64_t, false><<<g, kHierThreads, 0, stream>>>(prim, c, perm, nodes, n, queue, queue_count);
+    hierarchy_global_kernel<uint64_t><<<g2, 256, 0, stream>>>(c, store, nodes, n, queue, queue_count);
   }
 }
 
