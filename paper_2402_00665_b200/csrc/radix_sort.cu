@@ -9,10 +9,13 @@
 // assumptions.
 //
 // Inside a tile: warp w owns a contiguous run of 32*ITEMS pairs, item j of lane l at offset j*32+l
-// (coalesced loads; tile order = (warp, item, lane)).  Ranks come from __match_any_sync on the digit
-// plus a per-warp 256-bin counter array in shared memory, which keeps the order of equal digits =
-// stability.  Keys and values are then permuted through shared memory into tile-sorted order and
-// written out in runs of equal digit, i.e. coalesced.
+// (coalesced loads; tile order = (warp, item, lane)).  Ranks come from one ballot per digit bit plus a
+// per-warp 256-bin counter array in shared memory, which keeps the order of equal digits = stability.
+// Keys and values are then permuted through shared memory into tile-sorted order and written out in
+// runs of equal digit, i.e. coalesced.  On B200 this kernel is bound by instruction issue, not by HBM
+// (profiles/): the code below is written to keep the per-pair instruction count down -- full tiles take
+// a path without bounds predicates, positions are 32-bit, values are loaded after the ranking so that
+// fewer registers are live (4 CTAs of 256 threads per SM).
 #include "common.cuh"
 
 namespace bvh {
@@ -40,90 +43,106 @@ __device__ __forceinline__ void st_volatile_u32(uint32_t* p, uint32_t v) {
   asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-template <typename KeyT, bool IOTA>
-__global__ void __launch_bounds__(kSortThreads, 3)
-onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_out, const uint32_t* __restrict__ vals_in,
-                     uint32_t* __restrict__ vals_out, const uint32_t* __restrict__ hist, uint32_t* status,
-                     uint32_t* tile_counter, int n, int shift) {
+template <typename KeyT>
+struct SortSmem {
+  uint32_t warp_hist[kSortWarps][256];
+  uint32_t tile_excl[256];     // first tile-sorted position of each digit
+  uint32_t digit_base[256];    // global position of tile-sorted position 0 of each digit (mod 2^32; n < 2^30)
+  uint32_t scan[2][kSortWarps];
+  uint32_t tile;
+  KeyT keys[SortCfg<KeyT>::TILE];
+  uint32_t vals[SortCfg<KeyT>::TILE];
+};
+
+// Lanes of the warp whose digit equals this lane's: AND over the 8 digit bits of (ballot of the bit) or its
+// complement.  `peers` enters as the mask of participating lanes.
+__device__ __forceinline__ uint32_t match_digit(uint32_t d, uint32_t peers) {
+#pragma unroll
+  for (int b = 0; b < 8; ++b) {
+    // four SASS instructions per bit: bit test -> predicate, VOTE, and one predicated LOP3 per polarity
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        ".reg .b32 t, bal;\n\t"
+        "and.b32 t, %1, %2;\n\t"
+        "setp.ne.u32 p, t, 0;\n\t"
+        "vote.sync.ballot.b32 bal, p, 0xffffffff;\n\t"
+        "@p and.b32 %0, %0, bal;\n\t"
+        "@!p not.b32 bal, bal;\n\t"
+        "@!p and.b32 %0, %0, bal;\n\t"
+        "}"
+        : "+r"(peers)
+        : "r"(d), "r"(1u << b));
+  }
+  return peers;
+}
+
+template <typename KeyT, bool IOTA, bool FULL>
+__device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_out,
+                                          const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ vals_out,
+                                          const uint32_t* __restrict__ hist, uint32_t* status, uint32_t tile,
+                                          uint32_t tile_base, int valid_in_tile, int shift) {
   constexpr int ITEMS = SortCfg<KeyT>::ITEMS;
-  constexpr int TILE = SortCfg<KeyT>::TILE;
-  __shared__ uint32_t s_warp_hist[kSortWarps][256];
-  __shared__ uint32_t s_tile_excl[256];      // first tile-sorted position of each digit
-  __shared__ int64_t s_digit_base[256];      // global position of tile-sorted position 0 of each digit
-  __shared__ uint32_t s_scan[kSortWarps];
-  __shared__ uint32_t s_tile;
-  __shared__ KeyT s_keys[TILE];
-  __shared__ uint32_t s_vals[TILE];
-
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  if (tid == 0) s_tile = atomicAdd(tile_counter, 1u);
-  for (int i = tid; i < kSortWarps * 256; i += kSortThreads) (&s_warp_hist[0][0])[i] = 0;
-  __syncthreads();
-  const uint32_t tile = s_tile;
-  const int64_t tile_base = (int64_t)tile * TILE;
-  const int valid_in_tile = (int)min((int64_t)TILE, (int64_t)n - tile_base);
-
-  // ---- load (coalesced; warp-contiguous runs) -------------------------------------------------------
-  KeyT key[ITEMS];
-  uint32_t val[ITEMS];
   const int warp_off = warp * 32 * ITEMS + lane;
+
+  // ---- load keys (coalesced; warp-contiguous runs) ------------------------------------------------------
+  KeyT key[ITEMS];
 #pragma unroll
   for (int j = 0; j < ITEMS; ++j) {
     const int t = warp_off + j * 32;
-    if (t < valid_in_tile) {
-      key[j] = keys_in[tile_base + t];
-      val[j] = IOTA ? (uint32_t)(tile_base + t) : vals_in[tile_base + t];
-    } else {
-      key[j] = 0;
-      val[j] = 0;
-    }
+    key[j] = (FULL || t < valid_in_tile) ? keys_in[tile_base + t] : (KeyT)0;
   }
 
   // ---- rank within the warp, in tile order ---------------------------------------------------------------
-  // peers = lanes of this warp holding the same digit, from one ballot per digit bit (a fixed 8 votes per
-  // item; __match_any_sync costs one round per DISTINCT digit in the warp, ~28 on uniformly random digits).
   uint32_t rank[ITEMS];
   const uint32_t lt_mask = (1u << lane) - 1u;
+  uint32_t* my_hist = s.warp_hist[warp];
 #pragma unroll
   for (int j = 0; j < ITEMS; ++j) {
-    const bool valid = (warp_off + j * 32) < valid_in_tile;
     const uint32_t d = (uint32_t)(key[j] >> shift) & 0xFFu;
-    uint32_t peers = __ballot_sync(0xffffffffu, valid);
-#pragma unroll
-    for (int b = 0; b < 8; ++b) {
-      const bool bit = (d >> b) & 1u;
-      const uint32_t bal = __ballot_sync(0xffffffffu, bit);
-      peers &= bit ? bal : ~bal;
+    uint32_t peers;
+    if (FULL) {
+      peers = match_digit(d, 0xffffffffu);
+    } else {
+      const bool valid = (warp_off + j * 32) < valid_in_tile;
+      peers = match_digit(d, __ballot_sync(0xffffffffu, valid));
+      if (!valid) peers = 0;
     }
-    if (!valid) peers = 0;
-    const int leader = peers ? (__ffs(peers) - 1) : lane;
-    uint32_t pre = 0;
-    if (valid && lane == leader) {
-      pre = s_warp_hist[warp][d];
-      s_warp_hist[warp][d] = pre + __popc(peers);
-    }
-    pre = __shfl_sync(0xffffffffu, pre, leader);
-    rank[j] = pre + __popc(peers & lt_mask);
+    // every peer reads the warp's running count of its digit (a broadcast), the lowest peer then bumps it
+    const uint32_t below = __popc(peers & lt_mask);
+    const uint32_t pre = my_hist[d];
     __syncwarp();
+    if (below == 0 && (FULL || peers)) my_hist[d] = pre + __popc(peers);
+    __syncwarp();
+    rank[j] = pre + below;
+  }
+
+  // values are only needed for the scatter: issue their loads now, they land during the look-back
+  uint32_t val[ITEMS];
+#pragma unroll
+  for (int j = 0; j < ITEMS; ++j) {
+    const int t = warp_off + j * 32;
+    if (IOTA)
+      val[j] = tile_base + t;
+    else
+      val[j] = (FULL || t < valid_in_tile) ? vals_in[tile_base + t] : 0u;
   }
   __syncthreads();
 
-  // ---- per digit: exclusive scan over warps, publish tile count, look back -----------------------------------
-  // kSortThreads == 256: thread d owns digit d.
+  // ---- per digit (thread d owns digit d): exclusive scan over warps, publish tile count, look back -------
   uint32_t tile_count = 0;
-  {
 #pragma unroll
-    for (int w = 0; w < kSortWarps; ++w) {
-      const uint32_t c = s_warp_hist[w][tid];
-      s_warp_hist[w][tid] = tile_count;
-      tile_count += c;
-    }
+  for (int w = 0; w < kSortWarps; ++w) {
+    const uint32_t c = s.warp_hist[w][tid];
+    s.warp_hist[w][tid] = tile_count;
+    tile_count += c;
   }
   uint32_t* my_status = status + (size_t)tile * 256 + tid;
   st_volatile_u32(my_status, (tile == 0 ? kFlagInclusive : kFlagPartial) | tile_count);
 
   // exclusive scan of tile_count over digits (tile-sorted layout) and of the global histogram over digits
-  uint32_t g = hist[tid];
+  const uint32_t g = hist[tid];
   uint32_t incl_t = tile_count, incl_g = g;
 #pragma unroll
   for (int off = 1; off < 32; off <<= 1) {
@@ -134,18 +153,17 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_o
       incl_g += b;
     }
   }
-  __shared__ uint32_t s_scan_g[kSortWarps];
   if (lane == 31) {
-    s_scan[warp] = incl_t;
-    s_scan_g[warp] = incl_g;
+    s.scan[0][warp] = incl_t;
+    s.scan[1][warp] = incl_g;
   }
   __syncthreads();
   uint32_t base_t = 0, base_g = 0;
 #pragma unroll
   for (int w = 0; w < kSortWarps; ++w) {
     if (w < warp) {
-      base_t += s_scan[w];
-      base_g += s_scan_g[w];
+      base_t += s.scan[0][w];
+      base_g += s.scan[1][w];
     }
   }
   const uint32_t tile_excl = base_t + incl_t - tile_count;
@@ -156,27 +174,27 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_o
   if (tile > 0) {
     int64_t t = (int64_t)tile - 1;
     while (true) {
-      const uint32_t s = ld_volatile_u32(status + (size_t)t * 256 + tid);
-      const uint32_t flag = s & ~kValueMask;
+      const uint32_t sw = ld_volatile_u32(status + (size_t)t * 256 + tid);
+      const uint32_t flag = sw & ~kValueMask;
       if (flag == 0) continue;  // not published yet: that tile is running (ticket order), spin
-      excl += s & kValueMask;
+      excl += sw & kValueMask;
       if (flag == kFlagInclusive) break;
       --t;
     }
     st_volatile_u32(my_status, kFlagInclusive | (excl + tile_count));
   }
-  s_tile_excl[tid] = tile_excl;
-  s_digit_base[tid] = (int64_t)glob_excl + (int64_t)excl - (int64_t)tile_excl;
+  s.tile_excl[tid] = tile_excl;
+  s.digit_base[tid] = glob_excl + excl - tile_excl;
   __syncthreads();
 
   // ---- permute through shared memory into tile-sorted order -----------------------------------------------
 #pragma unroll
   for (int j = 0; j < ITEMS; ++j) {
-    if ((warp_off + j * 32) < valid_in_tile) {
+    if (FULL || (warp_off + j * 32) < valid_in_tile) {
       const uint32_t d = (uint32_t)(key[j] >> shift) & 0xFFu;
-      const uint32_t pos = s_tile_excl[d] + s_warp_hist[warp][d] + rank[j];
-      s_keys[pos] = key[j];
-      s_vals[pos] = val[j];
+      const uint32_t pos = s.tile_excl[d] + my_hist[d] + rank[j];
+      s.keys[pos] = key[j];
+      s.vals[pos] = val[j];
     }
   }
   __syncthreads();
@@ -185,29 +203,55 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_o
 #pragma unroll
   for (int j = 0; j < ITEMS; ++j) {
     const int pos = tid + j * kSortThreads;
-    if (pos < valid_in_tile) {
-      const KeyT k = s_keys[pos];
+    if (FULL || pos < valid_in_tile) {
+      const KeyT k = s.keys[pos];
       const uint32_t d = (uint32_t)(k >> shift) & 0xFFu;
-      const int64_t dst = s_digit_base[d] + pos;
+      const uint32_t dst = s.digit_base[d] + (uint32_t)pos;
       keys_out[dst] = k;
-      vals_out[dst] = s_vals[pos];
+      vals_out[dst] = s.vals[pos];
     }
   }
+}
+
+template <typename KeyT, bool IOTA>
+__global__ void __launch_bounds__(kSortThreads, 4)
+onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_out, const uint32_t* __restrict__ vals_in,
+                     uint32_t* __restrict__ vals_out, const uint32_t* __restrict__ hist, uint32_t* status,
+                     uint32_t* tile_counter, int n, int shift) {
+  constexpr int TILE = SortCfg<KeyT>::TILE;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  SortSmem<KeyT>& s = *reinterpret_cast<SortSmem<KeyT>*>(smem_raw);
+
+  const int tid = threadIdx.x;
+  if (tid == 0) s.tile = atomicAdd(tile_counter, 1u);
+  for (int i = tid; i < kSortWarps * 256; i += kSortThreads) (&s.warp_hist[0][0])[i] = 0;
+  __syncthreads();
+  const uint32_t tile = s.tile;
+  const uint32_t tile_base = tile * (uint32_t)TILE;
+  const int valid_in_tile = min(TILE, n - (int)tile_base);
+  if (valid_in_tile == TILE)
+    sort_tile<KeyT, IOTA, true>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, TILE, shift);
+  else
+    sort_tile<KeyT, IOTA, false>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, valid_in_tile,
+                                 shift);
 }
 
 template <typename KeyT>
 static void sort_all(const SortBuffers& B, int n, int passes, cudaStream_t stream, void* const* pass_events) {
   const int tiles = (n + SortCfg<KeyT>::TILE - 1) / SortCfg<KeyT>::TILE;
   KeyT* keys[2] = {static_cast<KeyT*>(B.keys[0]), static_cast<KeyT*>(B.keys[1])};
+  const size_t smem = sizeof(SortSmem<KeyT>);
+  cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   for (int p = 0; p < passes; ++p) {
     const int in = p & 1, out = in ^ 1;
     uint32_t* st = B.status + (size_t)p * tiles * 256;
     uint32_t* vout = (p == passes - 1 && B.final_vals) ? B.final_vals : B.vals[out];
     if (p == 0)
-      onesweep_pass_kernel<KeyT, true><<<tiles, kSortThreads, 0, stream>>>(
+      onesweep_pass_kernel<KeyT, true><<<tiles, kSortThreads, smem, stream>>>(
           keys[in], keys[out], nullptr, vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
     else
-      onesweep_pass_kernel<KeyT, false><<<tiles, kSortThreads, 0, stream>>>(
+      onesweep_pass_kernel<KeyT, false><<<tiles, kSortThreads, smem, stream>>>(
           keys[in], keys[out], B.vals[in], vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
     if (pass_events && pass_events[p]) cudaEventRecord(static_cast<cudaEvent_t>(pass_events[p]), stream);
   }
