@@ -298,7 +298,7 @@ def run_ours(args) -> dict | None:
         t0 = time.perf_counter()
         dp = h_prims.to(device, non_blocking=True)
         bvh.build(dp)
-        h_root.copy_(bvh.nodes[:32], non_blocking=True)
+        h_root.copy_(bvh.nodes[64:96], non_blocking=True)   # root record (after the 64-byte header)
         torch.cuda.synchronize()
         t1 = time.perf_counter()
         dq = h_queries.to(device, non_blocking=True)

@@ -149,18 +149,21 @@ __device__ __forceinline__ uint32_t quantise(float lo, float hi, float slo, floa
 }
 
 // PRIM_FLOATS: 3 = points, 6 = boxes {min,max}, 4 = sphere queries {x,y,z,r} (centre only; used to order queries).
-// FROM_ROOT: the frame is the root node's box (a finished hierarchy) instead of the build header.
+// FROM_ROOT: the frame is the root box of a finished hierarchy (kept in its NodesHeader) instead of the build header.
 template <typename KeyT, int PASSES, int PRIM_FLOATS, bool FROM_ROOT>
 __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __restrict__ prim, int n,
                                                                 const Header* __restrict__ header,
-                                                                const Node* __restrict__ root,
+                                                                const NodesHeader* __restrict__ root,
                                                                 KeyT* __restrict__ codes, uint32_t* __restrict__ hist) {
   __shared__ uint32_t s_hist[PASSES * 256];
   for (int i = threadIdx.x; i < PASSES * 256; i += kMortonThreads) s_hist[i] = 0;
   float scene[6];
   if (FROM_ROOT) {
-    const float4 lo4 = root->lo, hi4 = root->hi;
-    scene[0] = lo4.x; scene[1] = lo4.y; scene[2] = lo4.z; scene[3] = hi4.x; scene[4] = hi4.y; scene[5] = hi4.z;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      scene[a] = root->scene_lo[a];
+      scene[3 + a] = root->scene_hi[a];
+    }
   } else {
     load_scene_bounds(header, scene);
   }
@@ -231,7 +234,7 @@ void launch_morton(const float* prim, int n, bool is_box, int morton_bits, const
   }
 }
 
-void launch_query_morton(const float* queries, int q, int kind, const Node* root, uint32_t* codes, uint32_t* hist,
+void launch_query_morton(const float* queries, int q, int kind, const NodesHeader* root, uint32_t* codes, uint32_t* hist,
                          cudaStream_t stream) {
   const unsigned g = morton_grid(q);
   if (kind == 0)

@@ -41,24 +41,50 @@ ScratchLayout scratch_layout(int64_t n, int morton_bits) {
 }
 
 // ---- parity export ------------------------------------------------------------------------------------
+// The canonical arrays of the unified index space (G8) from the internal records and the leaf records.
 template <typename KeyT>
-__global__ void export_kernel(const Node* __restrict__ nodes, const KeyT* __restrict__ keys,
+__global__ void export_kernel(const char* __restrict__ nodes, const KeyT* __restrict__ keys,
                               const uint32_t* __restrict__ vals, const Header* __restrict__ header, int n,
                               KeyT* sorted_codes, uint32_t* perm, int32_t* left_child, int32_t* rope, float* aabb,
                               float* scene_bounds) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t total = 2 * (int64_t)n - 1;
+  const int leaf_base = n - 1;
   if (i < n) {
     if (sorted_codes) sorted_codes[i] = keys[i];
     if (perm) perm[i] = vals[i];
   }
   if (i < total) {
-    const float4 lo = nodes[i].lo, hi = nodes[i].hi;
-    if (left_child) left_child[i] = __float_as_int(lo.w);
-    if (rope) rope[i] = __float_as_int(hi.w);
+    float lo[3], hi[3];
+    int left, rp;
+    if (i < leaf_base) {
+      const Node* rec = reinterpret_cast<const Node*>(nodes + kNodesHeaderBytes) + i;
+      const float4 a = rec->lo, b = rec->hi;
+      lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; hi[0] = b.x; hi[1] = b.y; hi[2] = b.z;
+      left = __float_as_int(a.w);
+      rp = __float_as_int(b.w);
+    } else {
+      const int li = (int)(i - leaf_base);
+      const char* leaves = nodes + leaf_offset_bytes(n);
+      uint32_t payload;
+      if (reinterpret_cast<const NodesHeader*>(nodes)->leaf_kind == kLeafPoints) {
+        const float4 v = reinterpret_cast<const float4*>(leaves)[li];
+        lo[0] = hi[0] = v.x; lo[1] = hi[1] = v.y; lo[2] = hi[2] = v.z;
+        payload = __float_as_uint(v.w);
+      } else {
+        const Node* rec = reinterpret_cast<const Node*>(leaves) + li;
+        const float4 a = rec->lo, b = rec->hi;
+        lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; hi[0] = b.x; hi[1] = b.y; hi[2] = b.z;
+        payload = __float_as_uint(a.w);
+      }
+      left = (int)(payload & kLeafPrimMask);
+      rp = (li == n - 1) ? kSentinel : ((payload & kLeafRopeInternal) ? li + 1 : leaf_base + li + 1);
+    }
+    if (left_child) left_child[i] = left;
+    if (rope) rope[i] = rp;
     if (aabb) {
       float* o = aabb + 6 * i;
-      o[0] = lo.x; o[1] = lo.y; o[2] = lo.z; o[3] = hi.x; o[4] = hi.y; o[5] = hi.z;
+      o[0] = lo[0]; o[1] = lo[1]; o[2] = lo[2]; o[3] = hi[0]; o[4] = hi[1]; o[5] = hi[2];
     }
   }
   if (i == 0 && scene_bounds) {
@@ -68,9 +94,10 @@ __global__ void export_kernel(const Node* __restrict__ nodes, const KeyT* __rest
   }
 }
 
-void launch_export(const Node* nodes, const void* scratch, const ScratchLayout& L, int n, void* sorted_codes,
+void launch_export(const void* nodes_, const void* scratch, const ScratchLayout& L, int n, void* sorted_codes,
                    uint32_t* perm, int32_t* left_child, int32_t* rope, float* aabb, float* scene_bounds,
                    cudaStream_t stream) {
+  const char* nodes = static_cast<const char*>(nodes_);
   const char* base = static_cast<const char*>(scratch);
   const Header* header = reinterpret_cast<const Header*>(base + L.header);
   const uint32_t* vals = reinterpret_cast<const uint32_t*>(base + L.vals[0]);
@@ -125,8 +152,7 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   mark(3);
   launch_sort(sort_buffers(scratch, L), L.key_bytes, L.passes, (int)n, stream, events ? events + 4 : nullptr);
   launch_hierarchy(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
-                   store, static_cast<Node*>(nodes), (int)n, reinterpret_cast<int2*>(base + L.queue),
-                   &header->queue_count, stream);
+                   store, nodes, (int)n, header, reinterpret_cast<int2*>(base + L.queue), &header->queue_count, stream);
   mark(12);
   return check_launch();
 }
@@ -151,7 +177,7 @@ static int query(const void* nodes, int64_t n, const float* queries, int64_t q, 
   }
   if (!nodes || !queries || misaligned(nodes) || misaligned(queries)) return BVH_ERR_INVALID_ARGUMENT;
   if (fill && !indices) return BVH_ERR_INVALID_ARGUMENT;  // nnz = 0 callers still pass a valid pointer
-  launch_traverse(static_cast<const Node*>(nodes), (int)n, queries, q, kind, fill, order, counts, offsets, indices, stream);
+  launch_traverse(nodes, (int)n, queries, q, kind, fill, order, counts, offsets, indices, stream);
   return check_launch();
 }
 
@@ -180,8 +206,8 @@ static int query_order(const void* nodes, int64_t n, const float* queries, int64
   char* base = static_cast<char*>(scratch);
   if (cudaMemsetAsync(base, 0, L.zero_bytes, stream) != cudaSuccess) return BVH_ERR_CUDA;
   SortBuffers B = sort_buffers(scratch, L);
-  launch_query_morton(queries, (int)q, kind, static_cast<const Node*>(nodes), static_cast<uint32_t*>(B.keys[0]), B.hist,
-                      stream);
+  launch_query_morton(queries, (int)q, kind, static_cast<const NodesHeader*>(nodes), static_cast<uint32_t*>(B.keys[0]),
+                      B.hist, stream);
   B.final_vals = order;
   launch_sort(B, 4, 4, (int)q, stream, nullptr);
   return check_launch();
@@ -197,7 +223,8 @@ int bvh_sizes(int64_t n, int morton_bits, size_t* node_bytes, size_t* scratch_by
   if (n < 0 || !node_bytes || !scratch_bytes) return BVH_ERR_INVALID_ARGUMENT;
   if (morton_bits != 30 && morton_bits != 63) return BVH_ERR_MORTON_BITS;
   if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
-  *node_bytes = (n > 0) ? sizeof(bvh::Node) * (size_t)(2 * n - 1) : sizeof(bvh::Node);
+  // header + internal records + leaf records at their larger (box) size: one size for both leaf formats
+  *node_bytes = bvh::leaf_offset_bytes(n) + sizeof(bvh::Node) * (size_t)(n > 0 ? n : 1);
   *scratch_bytes = bvh::scratch_layout(n, morton_bits).total;
   return BVH_OK;
 }
@@ -277,7 +304,7 @@ int bvh_export(const void* nodes, const void* scratch, int64_t n, int morton_bit
   if (n == 0) return BVH_OK;
   if (!nodes || !scratch) return BVH_ERR_INVALID_ARGUMENT;
   const bvh::ScratchLayout L = bvh::scratch_layout(n, morton_bits);
-  bvh::launch_export(static_cast<const bvh::Node*>(nodes), scratch, L, (int)n, sorted_codes, perm, left_child, rope,
+  bvh::launch_export(nodes, scratch, L, (int)n, sorted_codes, perm, left_child, rope,
                      aabb, scene_bounds, static_cast<cudaStream_t>(stream));
   return bvh::check_launch();
 }

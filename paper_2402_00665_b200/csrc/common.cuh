@@ -18,6 +18,34 @@ struct __align__(32) Node {
   float4 hi;
 };
 
+// ---- layout of the caller's `nodes` buffer ----------------------------------------------------------------
+//   [0, 64)                          NodesHeader (written by the build; queries read the leaf format there)
+//   [64, 64 + 32 (n-1))              internal records I_0 .. I_{n-2} (Karras index), one Node each
+//   [leaf_offset_bytes(n), ...)      leaf records L_0 .. L_{n-1} in Morton order:
+//        point leaves (bvh_build_points): float4 {x, y, z, bitcast(payload)}          16 bytes
+//        box leaves   (bvh_build_boxes) : Node {min.xyz, bitcast(payload)} {max.xyz, 0}  32 bytes
+//   payload = original primitive index | kLeafRopeInternal if the leaf's skip-connection is the INTERNAL node
+//   i+1 (else it is leaf i+1; the last leaf's is the sentinel): Algorithm 2 needs one bit.
+constexpr uint32_t kNodesMagic = 0x42564832u;   // "BVH2"
+constexpr int kNodesHeaderBytes = 64;
+constexpr int kLeafPoints = 0, kLeafBoxes = 1;
+constexpr uint32_t kLeafRopeInternal = 0x80000000u;
+constexpr uint32_t kLeafPrimMask = 0x7fffffffu;
+struct NodesHeader {
+  uint32_t magic;
+  int32_t n;
+  int32_t leaf_kind;
+  int32_t reserved;
+  float scene_lo[3];   // = box of the root, bit for bit (D1)
+  float scene_hi[3];
+  uint32_t pad[6];
+};
+static_assert(sizeof(NodesHeader) == kNodesHeaderBytes, "nodes header is 64 bytes");
+__host__ __device__ inline size_t leaf_offset_bytes(int64_t n) {
+  return (size_t)kNodesHeaderBytes + sizeof(Node) * (size_t)(n > 1 ? n - 1 : 0);
+}
+__host__ __device__ inline size_t leaf_record_bytes(int leaf_kind) { return leaf_kind == kLeafPoints ? 16 : 32; }
+
 // ---- scratch layout of one build (offsets in bytes from the caller's scratch pointer) ---------------
 struct ScratchLayout {
   size_t header;        // Header (below)
@@ -95,22 +123,23 @@ struct SortBuffers {
 SortBuffers sort_buffers(void* scratch, const ScratchLayout& L);
 void launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStream_t stream, void* const* pass_events);
 // Morton codes (30-bit) of query centres in the frame of the root box + digit histograms: orders queries.
-void launch_query_morton(const float* queries, int q, int kind, const Node* root, uint32_t* codes, uint32_t* hist,
+void launch_query_morton(const float* queries, int q, int kind, const NodesHeader* frame, uint32_t* codes, uint32_t* hist,
                          cudaStream_t stream);
 // K4+K5: leaf gather + modified Apetrei bottom-up pass (Algorithm 4 with boxes).
 void launch_hierarchy(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
-                      int* store, Node* nodes, int n, int2* queue, uint32_t* queue_count, cudaStream_t stream);
+                      int* store, void* nodes, int n, const Header* header, int2* queue, uint32_t* queue_count,
+                      cudaStream_t stream);
 int hierarchy_queue_capacity(int n);
 // K6/K8: stackless traversal.  kind 0 = spheres (xyzr), 1 = boxes (minmax).  fill: offsets/indices used.
 // order (optional): thread t serves query order[t] (results still land in row order[t]).
-void launch_traverse(const Node* nodes, int n, const float* queries, int64_t q, int kind, bool fill,
+void launch_traverse(const void* nodes, int n, const float* queries, int64_t q, int kind, bool fill,
                      const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* indices,
                      cudaStream_t stream);
 // K7: exclusive scan of int32 counts into int64 offsets[q+1].
 size_t scan_scratch_bytes(int64_t q);
 void launch_scan(const int32_t* counts, int64_t q, int64_t* offsets, void* scratch, cudaStream_t stream);
 // Parity export.
-void launch_export(const Node* nodes, const void* scratch, const ScratchLayout& L, int n, void* sorted_codes,
+void launch_export(const void* nodes, const void* scratch, const ScratchLayout& L, int n, void* sorted_codes,
                    uint32_t* perm, int32_t* left_child, int32_t* rope, float* aabb, float* scene_bounds,
                    cudaStream_t stream);
 

@@ -20,7 +20,14 @@
 
 namespace bvh {
 
-constexpr int kSortThreads = 256;
+#ifndef BVH_SORT_THREADS
+#define BVH_SORT_THREADS 256
+#endif
+#ifndef BVH_EARLY_PUBLISH
+#define BVH_EARLY_PUBLISH 1
+#endif
+constexpr int kSortThreads = BVH_SORT_THREADS;   // >= 256: thread d < 256 owns digit d
+constexpr bool kEarlyPublish = BVH_EARLY_PUBLISH != 0;
 constexpr int kSortWarps = kSortThreads / 32;
 constexpr uint32_t kFlagPartial = 1u << 30;
 constexpr uint32_t kFlagInclusive = 2u << 30;
@@ -34,21 +41,29 @@ struct SortCfg {
 
 int sort_tile_items(int key_bytes) { return key_bytes == 4 ? SortCfg<uint32_t>::TILE : SortCfg<uint64_t>::TILE; }
 
-__device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t* p) {
+// Tile status words are single 32-bit values (flag + count in one word), so relaxed GPU-scope accesses
+// are all the protocol needs: a reader either sees the whole word or the zero it was initialised with.
+__device__ __forceinline__ uint32_t ld_status(const uint32_t* p) {
   uint32_t v;
-  asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p));
+  asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
-__device__ __forceinline__ void st_volatile_u32(uint32_t* p, uint32_t v) {
-  asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+__device__ __forceinline__ void st_status(uint32_t* p, uint32_t v) {
+  asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
+
+#ifndef BVH_LOOKBACK_BATCH
+#define BVH_LOOKBACK_BATCH 8
+#endif
+constexpr int kLookbackBatch = BVH_LOOKBACK_BATCH;
 
 template <typename KeyT>
 struct SortSmem {
   uint32_t warp_hist[kSortWarps][256];
   uint32_t tile_excl[256];     // first tile-sorted position of each digit
   uint32_t digit_base[256];    // global position of tile-sorted position 0 of each digit (mod 2^32; n < 2^30)
-  uint32_t scan[2][kSortWarps];
+  uint32_t tile_hist[256];     // early publish: digit counts of the tile, by shared-memory atomics
+  uint32_t scan[2][8];
   uint32_t tile;
   KeyT keys[SortCfg<KeyT>::TILE];
   uint32_t vals[SortCfg<KeyT>::TILE];
@@ -85,6 +100,8 @@ __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restr
   constexpr int ITEMS = SortCfg<KeyT>::ITEMS;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int warp_off = warp * 32 * ITEMS + lane;
+  const bool owner = tid < 256;                       // thread d owns digit d
+  uint32_t* my_status = status + (size_t)tile * 256 + tid;
 
   // ---- load keys (coalesced; warp-contiguous runs) ------------------------------------------------------
   KeyT key[ITEMS];
@@ -92,6 +109,30 @@ __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restr
   for (int j = 0; j < ITEMS; ++j) {
     const int t = warp_off + j * 32;
     key[j] = (FULL || t < valid_in_tile) ? keys_in[tile_base + t] : (KeyT)0;
+  }
+
+  // ---- early publish: the tile's digit counts, long before the (expensive) ranking is done -----------------
+  // A later tile that looks back never has to spin on this tile's ranking; it only walks over published counts.
+  uint32_t tile_count = 0;
+  if (kEarlyPublish) {
+#pragma unroll
+    for (int j = 0; j < ITEMS; ++j) {
+      const uint32_t d = (uint32_t)(key[j] >> shift) & 0xFFu;
+      const bool valid = FULL || (warp_off + j * 32) < valid_in_tile;
+      // a warp whose 32 keys share the digit (constant high digits, coincident points) adds once
+      int all_same;
+      __match_all_sync(0xffffffffu, valid ? d : 0x100u, &all_same);
+      if (all_same) {
+        if (lane == 0 && valid) atomicAdd(&s.tile_hist[d], 32u);
+      } else if (valid) {
+        atomicAdd(&s.tile_hist[d], 1u);
+      }
+    }
+    __syncthreads();
+    if (owner) {
+      tile_count = s.tile_hist[tid];
+      st_status(my_status, (tile == 0 ? kFlagInclusive : kFlagPartial) | tile_count);
+    }
   }
 
   // ---- rank within the warp, in tile order ---------------------------------------------------------------
@@ -131,60 +172,86 @@ __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restr
   __syncthreads();
 
   // ---- per digit (thread d owns digit d): exclusive scan over warps, publish tile count, look back -------
-  uint32_t tile_count = 0;
+  uint32_t tile_excl = 0, glob_excl = 0, g = 0;
+  if (owner) {
+    uint32_t sum = 0;
 #pragma unroll
-  for (int w = 0; w < kSortWarps; ++w) {
-    const uint32_t c = s.warp_hist[w][tid];
-    s.warp_hist[w][tid] = tile_count;
-    tile_count += c;
-  }
-  uint32_t* my_status = status + (size_t)tile * 256 + tid;
-  st_volatile_u32(my_status, (tile == 0 ? kFlagInclusive : kFlagPartial) | tile_count);
-
-  // exclusive scan of tile_count over digits (tile-sorted layout) and of the global histogram over digits
-  const uint32_t g = hist[tid];
-  uint32_t incl_t = tile_count, incl_g = g;
-#pragma unroll
-  for (int off = 1; off < 32; off <<= 1) {
-    const uint32_t a = __shfl_up_sync(0xffffffffu, incl_t, off);
-    const uint32_t b = __shfl_up_sync(0xffffffffu, incl_g, off);
-    if (lane >= off) {
-      incl_t += a;
-      incl_g += b;
+    for (int w = 0; w < kSortWarps; ++w) {
+      const uint32_t c = s.warp_hist[w][tid];
+      s.warp_hist[w][tid] = sum;
+      sum += c;
     }
-  }
-  if (lane == 31) {
-    s.scan[0][warp] = incl_t;
-    s.scan[1][warp] = incl_g;
+    if (!kEarlyPublish) {
+      tile_count = sum;
+      st_status(my_status, (tile == 0 ? kFlagInclusive : kFlagPartial) | tile_count);
+    }
+    // exclusive scan of tile_count over digits (tile-sorted layout) and of the global histogram over digits
+    g = hist[tid];
+    uint32_t incl_t = tile_count, incl_g = g;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      const uint32_t a = __shfl_up_sync(0xffffffffu, incl_t, off);
+      const uint32_t b = __shfl_up_sync(0xffffffffu, incl_g, off);
+      if (lane >= off) {
+        incl_t += a;
+        incl_g += b;
+      }
+    }
+    if (lane == 31) {
+      s.scan[0][warp] = incl_t;
+      s.scan[1][warp] = incl_g;
+    }
+    tile_excl = incl_t - tile_count;
+    glob_excl = incl_g - g;
   }
   __syncthreads();
-  uint32_t base_t = 0, base_g = 0;
+  if (owner) {
 #pragma unroll
-  for (int w = 0; w < kSortWarps; ++w) {
-    if (w < warp) {
-      base_t += s.scan[0][w];
-      base_g += s.scan[1][w];
+    for (int w = 0; w < 8; ++w) {
+      if (w < warp) {
+        tile_excl += s.scan[0][w];
+        glob_excl += s.scan[1][w];
+      }
     }
-  }
-  const uint32_t tile_excl = base_t + incl_t - tile_count;
-  const uint32_t glob_excl = base_g + incl_g - g;
 
-  // decoupled look-back over the previous tiles' counts of this digit
-  uint32_t excl = 0;
-  if (tile > 0) {
-    int64_t t = (int64_t)tile - 1;
-    while (true) {
-      const uint32_t sw = ld_volatile_u32(status + (size_t)t * 256 + tid);
-      const uint32_t flag = sw & ~kValueMask;
-      if (flag == 0) continue;  // not published yet: that tile is running (ticket order), spin
-      excl += sw & kValueMask;
-      if (flag == kFlagInclusive) break;
-      --t;
+    // decoupled look-back over the previous tiles' counts of this digit.  Tiles start faster than one status
+    // word can be fetched (about 20 tiles per L2 round trip on C3) and not in perfect order, so the chain to the
+    // nearest tile that already knows its inclusive prefix is several tiles long: the words of kLookbackBatch
+    // predecessors are fetched at once and consumed in order.  A word that is not published yet (flag 0) is
+    // polled alone, with a pause, so that waiting tiles do not flood the L2 slice that holds it.
+    uint32_t excl = 0;
+    if (tile > 0) {
+      int64_t t = (int64_t)tile - 1;
+      bool done = false;
+      while (!done) {
+        uint32_t sw[kLookbackBatch];
+#pragma unroll
+        for (int u = 0; u < kLookbackBatch; ++u)
+          sw[u] = (t - u >= 0) ? ld_status(status + (size_t)(t - u) * 256 + tid) : kFlagInclusive;
+        int used = 0;
+#pragma unroll
+        for (int u = 0; u < kLookbackBatch; ++u) {
+          const uint32_t flag = sw[u] & ~kValueMask;
+          if (!done && used == u && flag != 0) {
+            excl += sw[u] & kValueMask;
+            done = (flag == kFlagInclusive);
+            used = u + 1;
+          }
+        }
+        t -= used;
+        if (!done && used < kLookbackBatch) {   // tile t is running but has not published: wait for that one word
+          uint32_t w;
+          while (((w = ld_status(status + (size_t)t * 256 + tid)) & ~kValueMask) == 0) __nanosleep(64);
+          excl += w & kValueMask;
+          done = ((w & ~kValueMask) == kFlagInclusive);
+          --t;
+        }
+      }
+      st_status(my_status, kFlagInclusive | (excl + tile_count));
     }
-    st_volatile_u32(my_status, kFlagInclusive | (excl + tile_count));
+    s.tile_excl[tid] = tile_excl;
+    s.digit_base[tid] = glob_excl + excl - tile_excl;
   }
-  s.tile_excl[tid] = tile_excl;
-  s.digit_base[tid] = glob_excl + excl - tile_excl;
   __syncthreads();
 
   // ---- permute through shared memory into tile-sorted order -----------------------------------------------
@@ -214,7 +281,7 @@ __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restr
 }
 
 template <typename KeyT, bool IOTA>
-__global__ void __launch_bounds__(kSortThreads, 4)
+__global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads)
 onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_out, const uint32_t* __restrict__ vals_in,
                      uint32_t* __restrict__ vals_out, const uint32_t* __restrict__ hist, uint32_t* status,
                      uint32_t* tile_counter, int n, int shift) {
@@ -225,6 +292,7 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_o
   const int tid = threadIdx.x;
   if (tid == 0) s.tile = atomicAdd(tile_counter, 1u);
   for (int i = tid; i < kSortWarps * 256; i += kSortThreads) (&s.warp_hist[0][0])[i] = 0;
+  if (tid < 256) s.tile_hist[tid] = 0;
   __syncthreads();
   const uint32_t tile = s.tile;
   const uint32_t tile_base = tile * (uint32_t)TILE;

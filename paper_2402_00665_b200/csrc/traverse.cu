@@ -1,23 +1,33 @@
 // traverse.cu -- K6 / K8: the paper's Algorithm 1 (reading G3), stackless traversal
-// with skip-connections for a predicate query, one thread per query.  The count pass (K6) counts the
-// leaves that satisfy the predicate; the fill pass (K8) repeats the walk and stores the original
-// primitive index of each such leaf at offsets[query] + k ("Store the result", Alg. 1 L5).
+// with skip-connections for a predicate query.  The count pass (K6) counts the leaves that satisfy
+// the predicate; the fill pass (K8) repeats the walk and stores the original primitive index of each
+// such leaf at offsets[query] + k ("Store the result", Alg. 1 L5).
 //
-// B200 specifics
-//  * A node is one 32-byte record = one sector, fetched with ONE 256-bit load (LDG.E.ENL2.256, new on
-//    sm_100): one L1 wavefront per lane and visit instead of two 128-bit halves of the same sector.
-//  * Scheduling.  The grid is persistent: 148 SMs x kTravCtasPerSm CTAs, and CTA b works on query chunk
-//    ((k*148 + b%148) * R + b/148) at its step k.  Blocks b, b+148, b+296, ... are co-resident on one SM,
-//    so at any time an SM's 2048 threads serve 2048 consecutive positions of the (Morton-ordered) query
-//    list: their node reads overlap and stay in that SM's L1 (data divergence).  The
-//    mapping of blocks to SMs is only a locality assumption; any mapping gives the same results.
-//  * Fill output.  Hits of a row are staged in a per-thread 8-slot shared-memory ring indexed by the
-//    global output position, and an aligned group of 8 leaves as one 256-bit store = one full sector
-//    (no partial-sector writes, 8x fewer store requests than 4-byte stores to 32 different rows per warp).
+// Work split inside a warp (32 queries, neighbours on the Morton curve when `order` is given):
+//  * WALK, one lane per query.  Each lane follows Algorithm 1 over the internal nodes: one 32-byte record =
+//    one sector = ONE 256-bit load (LDG.E.ENL2.256, new on sm_100) per visit; hit -> left child, miss ->
+//    skip-connection.  No stack, no per-thread memory.
+//  * SCAN, the whole warp per leaf range.  In Karras ordering the leaves below a node are the consecutive
+//    leaf records [first, last], and the walk knows both bounds for free: the node a skip-connection leads to
+//    starts right after the subtree it skips (Algorithm 2: N_skip is node range_right + 1),
+//    and `first` is inherited on the way down (a left child starts where its parent starts).  When a node that
+//    satisfies the predicate covers at most kScanLeaves leaves, the lane does not walk that small subtree
+//    node by node: it posts the range, and the warp tests those leaves together, lane l taking leaf
+//    first + l -- one coalesced load of consecutive leaf records instead of 32 scattered ones, no
+//    divergence, and in the fill pass the hits of the row leave as one contiguous run of stores
+//    (warp-cooperative CSR output; ballot + popc give each hit its slot).  Every leaf of the subtree is
+//    still tested, in ascending order, so the result and its order are those of Algorithm 1.
+//  * Scheduling.  The grid is persistent: 148 SMs x CTAs per SM, and CTA b works on query chunk
+//    ((k*148 + b%148) * R + b/148) at its step k, so that at any time the threads of an SM serve consecutive
+//    positions of the (Morton-ordered) query list: their node reads overlap and stay in that SM's L1
+//    (data divergence).  The block-to-SM mapping is only a locality assumption.
 //
 // Predicates (D8): sphere {c, r} -- squared distance from c to the box, fp32 round-to-nearest with
 // explicit intrinsics (no FMA contraction): d = max(max(lo - c, c - hi), 0) per axis,
 // d2 = (dx*dx + dy*dy) + dz*dz, hit iff d2 <= r*r.  Box -- closed-interval overlap on each axis.
+// A point leaf stores the point once; with lo = hi = p the sphere formula reduces exactly to
+// d = |p - c| (lo - c and c - hi are exact negatives of each other under round-to-nearest) and the box
+// test to min <= p <= max, which is what the point-leaf tests below compute.
 #include "common.cuh"
 
 namespace bvh {
@@ -26,10 +36,11 @@ namespace bvh {
 #define BVH_TRAV_CTAS 8
 #endif
 #ifndef BVH_SCAN_LEAVES
-#define BVH_SCAN_LEAVES 32
+#define BVH_SCAN_LEAVES 128
 #endif
 constexpr int kTravThreads = 128;
-constexpr int kTravCtasPerSm = BVH_TRAV_CTAS;  // 8 x 128 threads: 64 registers per thread for the leaf-scan batch
+constexpr int kTravCtasPerSm = BVH_TRAV_CTAS;
+constexpr int kScanLeaves = BVH_SCAN_LEAVES;
 
 struct NodeRec {
   float lox, loy, loz;
@@ -38,182 +49,238 @@ struct NodeRec {
   int rope;
 };
 
-__device__ __forceinline__ NodeRec load_node(const Node* __restrict__ nodes, int idx) {
+__device__ __forceinline__ NodeRec load_rec(const Node* __restrict__ p) {
   NodeRec r;
-  float l, p;
+  float l, q;
   asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-               : "=f"(r.lox), "=f"(r.loy), "=f"(r.loz), "=f"(l), "=f"(r.hix), "=f"(r.hiy), "=f"(r.hiz), "=f"(p)
-               : "l"(nodes + idx));
+               : "=f"(r.lox), "=f"(r.loy), "=f"(r.loz), "=f"(l), "=f"(r.hix), "=f"(r.hiy), "=f"(r.hiz), "=f"(q)
+               : "l"(p));
   r.left = __float_as_int(l);
-  r.rope = __float_as_int(p);
+  r.rope = __float_as_int(q);
   return r;
 }
 
 struct SphereQuery {
+  static constexpr int kWords = 4;
   float cx, cy, cz, r2;
   __device__ __forceinline__ void load(const float* __restrict__ q, int64_t j) {
     const float4 v = __ldg(reinterpret_cast<const float4*>(q) + j);
     cx = v.x; cy = v.y; cz = v.z;
     r2 = __fmul_rn(v.w, v.w);
   }
-  __device__ __forceinline__ bool hit(const NodeRec& n) const {
-    const float dx = fmaxf(fmaxf(__fsub_rn(n.lox, cx), __fsub_rn(cx, n.hix)), 0.0f);
-    const float dy = fmaxf(fmaxf(__fsub_rn(n.loy, cy), __fsub_rn(cy, n.hiy)), 0.0f);
-    const float dz = fmaxf(fmaxf(__fsub_rn(n.loz, cz), __fsub_rn(cz, n.hiz)), 0.0f);
+  __device__ __forceinline__ SphereQuery from_lane(int src) const {
+    SphereQuery o;
+    o.cx = __shfl_sync(0xffffffffu, cx, src);
+    o.cy = __shfl_sync(0xffffffffu, cy, src);
+    o.cz = __shfl_sync(0xffffffffu, cz, src);
+    o.r2 = __shfl_sync(0xffffffffu, r2, src);
+    return o;
+  }
+  __device__ __forceinline__ bool hit_box(float lox, float loy, float loz, float hix, float hiy, float hiz) const {
+    const float dx = fmaxf(fmaxf(__fsub_rn(lox, cx), __fsub_rn(cx, hix)), 0.0f);
+    const float dy = fmaxf(fmaxf(__fsub_rn(loy, cy), __fsub_rn(cy, hiy)), 0.0f);
+    const float dz = fmaxf(fmaxf(__fsub_rn(loz, cz), __fsub_rn(cz, hiz)), 0.0f);
+    const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+    return d2 <= r2;
+  }
+  __device__ __forceinline__ bool hit_point(float x, float y, float z) const {
+    const float dx = fabsf(__fsub_rn(x, cx)), dy = fabsf(__fsub_rn(y, cy)), dz = fabsf(__fsub_rn(z, cz));
     const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
     return d2 <= r2;
   }
 };
 
 struct BoxQuery {
+  static constexpr int kWords = 6;
   float lo[3], hi[3];
   __device__ __forceinline__ void load(const float* __restrict__ q, int64_t j) {
     const float2* p = reinterpret_cast<const float2*>(q + 6 * j);
     const float2 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
     lo[0] = a.x; lo[1] = a.y; lo[2] = b.x; hi[0] = b.y; hi[1] = c.x; hi[2] = c.y;
   }
-  __device__ __forceinline__ bool hit(const NodeRec& n) const {
-    return lo[0] <= n.hix && n.lox <= hi[0] && lo[1] <= n.hiy && n.loy <= hi[1] && lo[2] <= n.hiz && n.loz <= hi[2];
+  __device__ __forceinline__ BoxQuery from_lane(int src) const {
+    BoxQuery o;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      o.lo[a] = __shfl_sync(0xffffffffu, lo[a], src);
+      o.hi[a] = __shfl_sync(0xffffffffu, hi[a], src);
+    }
+    return o;
+  }
+  __device__ __forceinline__ bool hit_box(float lox, float loy, float loz, float hix, float hiy, float hiz) const {
+    return lo[0] <= hix && lox <= hi[0] && lo[1] <= hiy && loy <= hi[1] && lo[2] <= hiz && loz <= hi[2];
+  }
+  __device__ __forceinline__ bool hit_point(float x, float y, float z) const {
+    return lo[0] <= x && x <= hi[0] && lo[1] <= y && y <= hi[1] && lo[2] <= z && z <= hi[2];
   }
 };
 
-// Output side of the fill pass for one thread: ring of 8 slots per thread in shared memory.
-template <bool FILL>
-struct Emitter {
-  int (*ring)[kTravThreads];
-  int32_t* indices;
-  int64_t base;
-  int count;
-  bool vec_store;
-  __device__ __forceinline__ void emit(int value) {
-    if (FILL) {
-      const int64_t gi = base + count;                       // global output position of this hit
-      ring[gi & 7][threadIdx.x] = value;
-      if (((gi + 1) & 7) == 0) {                             // an aligned group of 8 positions is complete
-        const int64_t g0 = gi - 7;
-        if (g0 >= base && vec_store) {
-          asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(indices + g0),
-                       "r"(ring[0][threadIdx.x]), "r"(ring[1][threadIdx.x]), "r"(ring[2][threadIdx.x]),
-                       "r"(ring[3][threadIdx.x]), "r"(ring[4][threadIdx.x]), "r"(ring[5][threadIdx.x]),
-                       "r"(ring[6][threadIdx.x]), "r"(ring[7][threadIdx.x])
-                       : "memory");
-        } else {                                             // head of a row that starts inside the group
-          for (int64_t g = (g0 > base ? g0 : base); g <= gi; ++g) indices[g] = ring[g & 7][threadIdx.x];
-        }
-      }
-    }
-    ++count;
+// One leaf record: loaded first (so that several loads can be in flight), tested later.
+template <bool POINT_LEAF>
+struct LeafRec;
+template <>
+struct LeafRec<true> {
+  float4 v;
+  __device__ __forceinline__ void load(const char* __restrict__ leaves, int i) {
+    v = __ldg(reinterpret_cast<const float4*>(leaves) + i);
   }
-  __device__ __forceinline__ void finish() {                 // tail of the row: the incomplete last group
-    if (FILL) {
-      const int64_t end = base + count;
-      int64_t g = end & ~(int64_t)7;
-      if (g < base) g = base;
-      for (; g < end; ++g) indices[g] = ring[g & 7][threadIdx.x];
-    }
+  __device__ __forceinline__ uint32_t payload() const { return __float_as_uint(v.w); }
+  template <typename Query>
+  __device__ __forceinline__ bool hit(const Query& q) const { return q.hit_point(v.x, v.y, v.z); }
+};
+template <>
+struct LeafRec<false> {
+  NodeRec r;
+  __device__ __forceinline__ void load(const char* __restrict__ leaves, int i) {
+    r = load_rec(reinterpret_cast<const Node*>(leaves) + i);
   }
+  __device__ __forceinline__ uint32_t payload() const { return (uint32_t)r.left; }
+  template <typename Query>
+  __device__ __forceinline__ bool hit(const Query& q) const { return q.hit_box(r.lox, r.loy, r.loz, r.hix, r.hiy, r.hiz); }
 };
 
-// Leaf-range shortcut.  In Karras ordering the leaves below a node are the consecutive leaf records
-// [first, last], and the walk knows both bounds for free: the node a skip-connection leads to starts right
-// after the subtree it skips (Algorithm 2: N_skip is node range_right + 1), so
-// last + 1 = index of N_skip, and `first` is inherited on the way down (a left child starts where its
-// parent starts).  When a node that satisfies the predicate covers at most kScanLeaves leaves, its leaves are
-// tested directly from their consecutive records (independent, contiguous 256-bit loads: 4 leaves per 128-byte
-// line) instead of walking the small subtree node by node.  Every leaf of the subtree is still tested, in the
-// same ascending order, so the result and its order are those of Algorithm 1.
-constexpr int kScanLeaves = BVH_SCAN_LEAVES;
-#ifndef BVH_SCAN_BATCH
-#define BVH_SCAN_BATCH 2
+#ifndef BVH_SCAN_UNROLL
+#define BVH_SCAN_UNROLL 4
 #endif
-constexpr int kScanBatch = BVH_SCAN_BATCH;
 
-template <typename Query, bool FILL>
-__global__ void __launch_bounds__(kTravThreads, kTravCtasPerSm)
-traverse_kernel(const Node* __restrict__ nodes, int n, const float* __restrict__ queries, int64_t q,
-                const uint32_t* __restrict__ order, int32_t* __restrict__ counts, const int64_t* __restrict__ offsets,
-                int32_t* __restrict__ indices, int64_t num_chunks, int ctas_per_sm, bool vec_store) {
-  __shared__ int s_ring[FILL ? 8 : 1][kTravThreads];
+template <typename Query, bool FILL, bool POINT_LEAF>
+__device__ __forceinline__ void traverse_body(const char* __restrict__ nodes, int n, const float* __restrict__ queries,
+                                              int64_t q, const uint32_t* __restrict__ order, int32_t* __restrict__ counts,
+                                              const int64_t* __restrict__ offsets, int32_t* __restrict__ indices,
+                                              int64_t num_chunks, int ctas_per_sm) {
+  constexpr int U = POINT_LEAF ? BVH_SCAN_UNROLL : (BVH_SCAN_UNROLL > 2 ? 2 : BVH_SCAN_UNROLL);   // leaf loads in flight per lane
+  const Node* __restrict__ internal = reinterpret_cast<const Node*>(nodes + kNodesHeaderBytes);
+  const char* __restrict__ leaves = nodes + leaf_offset_bytes(n);
   const int leaf_base = n - 1;
+  const int lane = threadIdx.x & 31;
+  const uint32_t lt_mask = (1u << lane) - 1u;
   const int64_t sm_slot = blockIdx.x % kNumSMs;
   const int64_t r = blockIdx.x / kNumSMs;
   for (int64_t k = 0;; ++k) {
     const int64_t chunk = (k * kNumSMs + sm_slot) * ctas_per_sm + r;
     if (chunk >= num_chunks) break;
     const int64_t t = chunk * kTravThreads + threadIdx.x;
-    if (t >= q) continue;
-    const int64_t j = order ? (int64_t)order[t] : t;
+    const bool have = t < q;
+    const int64_t j = have ? (order ? (int64_t)order[t] : t) : 0;
     Query query;
     query.load(queries, j);
-    Emitter<FILL> out{s_ring, indices, FILL ? offsets[j] : 0, 0, vec_store};
-    int node = 0;                                            // L1: start from the root
+    int32_t* row = FILL ? indices + (have ? offsets[j] : 0) : nullptr;   // this query's CSR row
+    int count = 0;
+    int node = have ? 0 : kSentinel;                         // L1: start from the root
     int first = 0;                                           // first leaf below `node`
-    int scan_i = 0, scan_end = 0;                            // pending leaf-range scan [scan_i, scan_end)
-    // One loop for both activities, so that the lanes of a warp stay converged: every trip loads kScanBatch
-    // records (tree step: the node and nothing else; scan step: the next kScanBatch consecutive leaves).
-    do {                                                     // L2
-      const bool scanning = scan_i < scan_end;
-      NodeRec rec[kScanBatch];
-      rec[0] = load_node(nodes, scanning ? leaf_base + scan_i : node);
+    int scan_i = 0, scan_end = 0;                            // posted leaf range [scan_i, scan_end)
+    while (true) {                                           // L2 ... L11 for the 32 queries of the warp
+      const bool walking = node != kSentinel;
+      uint32_t posted = __ballot_sync(0xffffffffu, scan_i < scan_end);
+      if (!__any_sync(0xffffffffu, walking) && posted == 0) break;
+      // ---- WALK, first half: fetch this lane's node; the record is consumed after the SCAN below, which runs while
+      // the load is in flight ----
+      const bool at_internal = walking && node < leaf_base;
+      NodeRec rec;
+      if (at_internal) rec = load_rec(internal + node);
+      // ---- SCAN: the warp tests every range posted in the previous round, 32 consecutive leaves per step ----------
+      while (posted) {
+        const int o = __ffs(posted) - 1;
+        posted &= posted - 1;
+        const Query oq = query.from_lane(o);
+        const int begin = __shfl_sync(0xffffffffu, scan_i, o);
+        const int end = __shfl_sync(0xffffffffu, scan_end, o);
+        int ocount = __shfl_sync(0xffffffffu, count, o);
+        int32_t* orow = nullptr;
+        if (FILL) orow = reinterpret_cast<int32_t*>(__shfl_sync(0xffffffffu, reinterpret_cast<unsigned long long>(row), o));
+        for (int c = begin + lane; c < end + lane; c += 32 * U) {   // c - lane is warp-uniform
+          LeafRec<POINT_LEAF> leaf[U];
 #pragma unroll
-      for (int u = 1; u < kScanBatch; ++u)
-        if (scanning && scan_i + u < scan_end) rec[u] = load_node(nodes, leaf_base + scan_i + u);
-      const bool hit0 = query.hit(rec[0]);                   // L3
-      if (scanning) {
-        if (hit0) out.emit(rec[0].left);                     // L4-5 on the leaves of the range, in order
+          for (int u = 0; u < U; ++u)
+            if (c + 32 * u < end) leaf[u].load(leaves, c + 32 * u);
 #pragma unroll
-        for (int u = 1; u < kScanBatch; ++u)
-          if (scan_i + u < scan_end && query.hit(rec[u])) out.emit(rec[u].left);
-        scan_i += kScanBatch;
-      } else {
-        const int rope = rec[0].rope;
-        // first leaf after this subtree = index of the skip target (leaf or internal alike); n after the last one
-        const int next_first = rope < 0 ? n : (rope >= leaf_base ? rope - leaf_base : rope);
-        int next = rope;                                     // L6 / L10: N_skip
-        if (hit0) {
-          if (node >= leaf_base) {                           // L4-5
-            out.emit(rec[0].left);
-          } else if (next_first - first <= kScanLeaves) {    // small subtree: test its leaves directly
-            scan_i = first;
-            scan_end = next_first;
-          } else {
-            next = rec[0].left;                              // L8: N_left (same first leaf)
+          for (int u = 0; u < U; ++u) {
+            const bool hit = (c + 32 * u < end) && leaf[u].hit(oq);                   // L3-5 on leaf c + 32u
+            const uint32_t m = __ballot_sync(0xffffffffu, hit);
+            if (FILL && hit) orow[ocount + __popc(m & lt_mask)] = (int)(leaf[u].payload() & kLeafPrimMask);
+            ocount += __popc(m);
           }
         }
-        if (next == rope) first = next_first;
-        node = next;
+        if (lane == o) {
+          count = ocount;
+          scan_i = scan_end;
+        }
       }
-    } while (node != kSentinel || scan_i < scan_end);        // L11
-    out.finish();
-    if (!FILL) counts[j] = out.count;
+      // ---- WALK, second half: one step of Algorithm 1 per lane ---------------------------------------------------
+      if (walking) {
+        if (!at_internal) {                                  // a single leaf (reached as a child or through a rope)
+          const int i = node - leaf_base;
+          LeafRec<POINT_LEAF> leaf;
+          leaf.load(leaves, i);
+          const uint32_t payload = leaf.payload();
+          if (leaf.hit(query)) {                             // L3-5
+            if (FILL) row[count] = (int)(payload & kLeafPrimMask);
+            ++count;
+          }
+          // L6: N_skip of leaf i (Algorithm 2): leaf i+1 or internal node i+1, one bit in the record
+          node = (i == n - 1) ? kSentinel : ((payload & kLeafRopeInternal) ? i + 1 : leaf_base + i + 1);
+          first = i + 1;
+        } else {
+          const int rope = rec.rope;
+          // first leaf after this subtree = index of the skip target (leaf or internal alike); n after the last one
+          const int next_first = rope < 0 ? n : (rope >= leaf_base ? rope - leaf_base : rope);
+          int next = rope;                                   // L10: N_skip
+          if (query.hit_box(rec.lox, rec.loy, rec.loz, rec.hix, rec.hiy, rec.hiz)) {   // L3
+            if (next_first - first <= kScanLeaves) {         // small subtree: post its leaves, continue after it
+              scan_i = first;
+              scan_end = next_first;
+            } else {
+              next = rec.left;                               // L8: N_left (same first leaf)
+            }
+          }
+          if (next == rope) first = next_first;
+          node = next;
+        }
+      }
+    }
+    if (!FILL && have) counts[j] = count;
   }
 }
 
-void launch_traverse(const Node* nodes, int n, const float* queries, int64_t q, int kind, bool fill,
-                     const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* indices,
-                     cudaStream_t stream) {
+// The leaf format (point or box records) is a property of the hierarchy, recorded in its header by the build;
+// the kernel reads it there (one uniform branch), so the query entry points need no extra argument.
+template <typename Query, bool FILL>
+__global__ void __launch_bounds__(kTravThreads, kTravCtasPerSm)
+traverse_kernel(const char* __restrict__ nodes, int n, const float* __restrict__ queries, int64_t q,
+                const uint32_t* __restrict__ order, int32_t* __restrict__ counts, const int64_t* __restrict__ offsets,
+                int32_t* __restrict__ indices, int64_t num_chunks, int ctas_per_sm) {
+  if (reinterpret_cast<const NodesHeader*>(nodes)->leaf_kind == kLeafPoints)
+    traverse_body<Query, FILL, true>(nodes, n, queries, q, order, counts, offsets, indices, num_chunks, ctas_per_sm);
+  else
+    traverse_body<Query, FILL, false>(nodes, n, queries, q, order, counts, offsets, indices, num_chunks, ctas_per_sm);
+}
+
+template <typename Query>
+static void launch_traverse_kind(const char* nodes, int n, const float* queries, int64_t q, bool fill,
+                                 const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* indices,
+                                 cudaStream_t stream) {
   const int64_t num_chunks = (q + kTravThreads - 1) / kTravThreads;
-  // persistent grid: up to 148 x 16 CTAs; fewer CTAs per SM when there is not enough work to fill them
+  // persistent grid: up to 148 x kTravCtasPerSm CTAs; fewer CTAs per SM when there is not enough work to fill them
   int ctas_per_sm = (int)((num_chunks + kNumSMs - 1) / kNumSMs);
   if (ctas_per_sm > kTravCtasPerSm) ctas_per_sm = kTravCtasPerSm;
   if (ctas_per_sm < 1) ctas_per_sm = 1;
   const unsigned g = (unsigned)(kNumSMs * ctas_per_sm);
-  const bool vec = (reinterpret_cast<uintptr_t>(indices) & 31u) == 0;
-  if (kind == 0) {
-    if (fill)
-      traverse_kernel<SphereQuery, true><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, order, counts, offsets,
-                                                                        indices, num_chunks, ctas_per_sm, vec);
-    else
-      traverse_kernel<SphereQuery, false><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, order, counts, offsets,
-                                                                         indices, num_chunks, ctas_per_sm, vec);
-  } else {
-    if (fill)
-      traverse_kernel<BoxQuery, true><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, order, counts, offsets,
-                                                                     indices, num_chunks, ctas_per_sm, vec);
-    else
-      traverse_kernel<BoxQuery, false><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, order, counts, offsets,
-                                                                      indices, num_chunks, ctas_per_sm, vec);
-  }
+  if (fill)
+    traverse_kernel<Query, true><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, order, counts, offsets, indices,
+                                                                num_chunks, ctas_per_sm);
+  else
+    traverse_kernel<Query, false><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, order, counts, offsets, indices,
+                                                                 num_chunks, ctas_per_sm);
+}
+
+void launch_traverse(const void* nodes, int n, const float* queries, int64_t q, int kind, bool fill,
+                     const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* indices,
+                     cudaStream_t stream) {
+  const char* base = static_cast<const char*>(nodes);
+  if (kind == 0)
+    launch_traverse_kind<SphereQuery>(base, n, queries, q, fill, order, counts, offsets, indices, stream);
+  else
+    launch_traverse_kind<BoxQuery>(base, n, queries, q, fill, order, counts, offsets, indices, stream);
 }
 
 }  // namespace bvh
