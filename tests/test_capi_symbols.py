@@ -44,11 +44,11 @@ def test_sizes_and_errors_host_only(lib):
 
     assert binding.bvh_version() >= 1
     nb, sb = binding.bvh_sizes(1000, 30)
-    assert nb == 32 * 1999
+    assert nb == 64 + 32 * 1999      # 64-byte header + (n-1) internal + n leaf records at their larger size
     assert sb >= 1000 * (4 + 2 * 4 + 2 * 4)
     nb63, sb63 = binding.bvh_sizes(1000, 63)
     assert nb63 == nb and sb63 > sb
-    assert binding.bvh_sizes(0, 30)[0] == 32
+    assert binding.bvh_sizes(0, 30)[0] == 64 + 32
     with pytest.raises(binding.BvhError, match="MORTON_BITS"):
         binding.bvh_sizes(10, 32)
     with pytest.raises(binding.BvhError, match="TOO_LARGE"):
