@@ -23,8 +23,6 @@ ScratchLayout scratch_layout(int64_t n, int morton_bits) {
   off += align_up((size_t)L.passes * L.tiles * 256 * sizeof(uint32_t), 256);
   L.zero_bytes = off;
   const size_t nn = (size_t)(n > 0 ? n : 1);
-  L.store = off;
-  off += align_up(nn * sizeof(int32_t), 256);
   for (int b = 0; b < 2; ++b) {
     L.keys[b] = off;
     off += align_up(nn * L.key_bytes, 256);
@@ -33,9 +31,11 @@ ScratchLayout scratch_layout(int64_t n, int morton_bits) {
     L.vals[b] = off;
     off += align_up(nn * sizeof(uint32_t), 256);
   }
-  L.queue = off;
-  L.queue_capacity = hierarchy_queue_capacity((int)nn);
-  off += align_up((size_t)L.queue_capacity * sizeof(int2), 256);
+  L.segments = hierarchy_total_segments((int)nn);
+  L.seg_items = off;
+  off += align_up((size_t)L.segments * hierarchy_seg_capacity() * sizeof(int2), 256);
+  L.seg_count = off;
+  off += align_up((size_t)L.segments * sizeof(int32_t), 256);
   L.total = off;
   return L;
 }
@@ -137,14 +137,12 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   char* base = static_cast<char*>(scratch);
   Header* header = reinterpret_cast<Header*>(base + L.header);
   uint32_t* hist = reinterpret_cast<uint32_t*>(base + L.hist);
-  int* store = reinterpret_cast<int*>(base + L.store);
 
   auto mark = [&](int k) {
     if (events && events[k]) cudaEventRecord(static_cast<cudaEvent_t>(events[k]), stream);
   };
   mark(0);
   if (cudaMemsetAsync(base, 0, L.zero_bytes, stream) != cudaSuccess) return BVH_ERR_CUDA;
-  if (cudaMemsetAsync(store, 0xFF, (size_t)n * sizeof(int), stream) != cudaSuccess) return BVH_ERR_CUDA;
   mark(1);
   launch_scene_bounds(prim, (int)n, is_box, header, stream);
   mark(2);
@@ -152,7 +150,8 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   mark(3);
   launch_sort(sort_buffers(scratch, L), L.key_bytes, L.passes, (int)n, stream, events ? events + 4 : nullptr);
   launch_hierarchy(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
-                   store, nodes, (int)n, header, reinterpret_cast<int2*>(base + L.queue), &header->queue_count, stream);
+                   nodes, (int)n, header, reinterpret_cast<int2*>(base + L.seg_items), reinterpret_cast<int*>(base + L.seg_count),
+                   stream);
   mark(12);
   return check_launch();
 }

@@ -52,12 +52,12 @@ struct ScratchLayout {
   size_t hist;          // uint32 [passes][256]   global digit histograms
   size_t status;        // uint32 [passes][tiles][256]  onesweep tile status words
   size_t zero_bytes;    // header + hist + status are contiguous from 0 and zero-initialised per build
-  size_t store;         // int32 [n]  Algorithm 4's `store` (n-1 used), initialised to -1
   size_t keys[2];       // KeyT [n]   ping-pong; sorted codes end in keys[0]
   size_t vals[2];       // uint32 [n] ping-pong; permutation ends in vals[0]
-  size_t queue;         // int2 [queue_capacity]  nodes handed from the block-local to the global bottom-up phase
+  size_t seg_items;     // int2 [segments][192]  subtrees handed from one level of the bottom-up pass to the next
+  size_t seg_count;     // int32 [segments]      how many each window handed over
   size_t total;
-  int queue_capacity;
+  int segments;         // windows of all levels of the bottom-up pass (hierarchy.cu)
   int passes;
   int tiles;
   int key_bytes;
@@ -66,8 +66,7 @@ struct ScratchLayout {
 struct Header {
   uint32_t bounds_enc[8];    // [0..2] = ~ord(min.xyz), [3..5] = ord(max.xyz), maximised with atomicMax
   uint32_t tile_counter[8];  // one dynamic tile counter per sort pass
-  uint32_t queue_count;      // entries in the bottom-up pass's hand-over queue
-  uint32_t pad[47];
+  uint32_t pad[48];
 };
 static_assert(sizeof(Header) == 256, "header is one 256-byte block");
 
@@ -126,10 +125,12 @@ void launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStr
 void launch_query_morton(const float* queries, int q, int kind, const NodesHeader* frame, uint32_t* codes, uint32_t* hist,
                          cudaStream_t stream);
 // K4+K5: leaf gather + modified Apetrei bottom-up pass (Algorithm 4 with boxes).
+constexpr int kMaxHierLevels = 8;
 void launch_hierarchy(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
-                      int* store, void* nodes, int n, const Header* header, int2* queue, uint32_t* queue_count,
-                      cudaStream_t stream);
-int hierarchy_queue_capacity(int n);
+                      void* nodes, int n, const Header* header, int2* seg_items, int* seg_count, cudaStream_t stream);
+int hierarchy_levels(int n, int segs[kMaxHierLevels]);   // windows per level, level 1 first; returns the level count
+int hierarchy_total_segments(int n);
+int hierarchy_seg_capacity();
 // K6/K8: stackless traversal.  kind 0 = spheres (xyzr), 1 = boxes (minmax).  fill: offsets/indices used.
 // order (optional): thread t serves query order[t] (results still land in row order[t]).
 void launch_traverse(const void* nodes, int n, const float* queries, int64_t q, int kind, bool fill,
