@@ -21,8 +21,11 @@ ScratchLayout scratch_layout(int64_t n, int morton_bits) {
   off += align_up((size_t)L.passes * 256 * sizeof(uint32_t), 256);
   L.status = off;
   off += align_up((size_t)L.passes * L.tiles * 256 * sizeof(uint32_t), 256);
-  L.zero_bytes = off;
   const size_t nn = (size_t)(n > 0 ? n : 1);
+  L.segments = hierarchy_total_segments((int)nn);
+  L.arrivals = off;
+  off += align_up((size_t)L.segments * sizeof(uint32_t), 256);
+  L.zero_bytes = off;
   for (int b = 0; b < 2; ++b) {
     L.keys[b] = off;
     off += align_up(nn * L.key_bytes, 256);
@@ -31,7 +34,6 @@ ScratchLayout scratch_layout(int64_t n, int morton_bits) {
     L.vals[b] = off;
     off += align_up(nn * sizeof(uint32_t), 256);
   }
-  L.segments = hierarchy_total_segments((int)nn);
   L.seg_items = off;
   off += align_up((size_t)L.segments * hierarchy_seg_capacity() * sizeof(int2), 256);
   L.seg_count = off;
@@ -151,7 +153,7 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   launch_sort(sort_buffers(scratch, L), L.key_bytes, L.passes, (int)n, stream, events ? events + 4 : nullptr);
   launch_hierarchy(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
                    nodes, (int)n, header, reinterpret_cast<int2*>(base + L.seg_items), reinterpret_cast<int*>(base + L.seg_count),
-                   stream);
+                   reinterpret_cast<uint32_t*>(base + L.arrivals), stream);
   mark(12);
   return check_launch();
 }

@@ -51,10 +51,11 @@ struct ScratchLayout {
   size_t header;        // Header (below)
   size_t hist;          // uint32 [passes][256]   global digit histograms
   size_t status;        // uint32 [passes][tiles][256]  onesweep tile status words
-  size_t zero_bytes;    // header + hist + status are contiguous from 0 and zero-initialised per build
+  size_t arrivals;      // uint32 [segments]  children arrived at each window of the bottom-up pass (hierarchy.cu)
+  size_t zero_bytes;    // header + hist + status + arrivals are contiguous from 0 and zero-initialised per build
   size_t keys[2];       // KeyT [n]   ping-pong; sorted codes end in keys[0]
   size_t vals[2];       // uint32 [n] ping-pong; permutation ends in vals[0]
-  size_t seg_items;     // int2 [segments][192]  subtrees handed from one level of the bottom-up pass to the next
+  size_t seg_items;     // int2 [segments][192]  subtrees handed from one window of the bottom-up pass to its parent
   size_t seg_count;     // int32 [segments]      how many each window handed over
   size_t total;
   int segments;         // windows of all levels of the bottom-up pass (hierarchy.cu)
@@ -127,7 +128,8 @@ void launch_query_morton(const float* queries, int q, int kind, const NodesHeade
 // K4+K5: leaf gather + modified Apetrei bottom-up pass (Algorithm 4 with boxes).
 constexpr int kMaxHierLevels = 8;
 void launch_hierarchy(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
-                      void* nodes, int n, const Header* header, int2* seg_items, int* seg_count, cudaStream_t stream);
+                      void* nodes, int n, const Header* header, int2* seg_items, int* seg_count, uint32_t* arrivals,
+                      cudaStream_t stream);
 int hierarchy_levels(int n, int segs[kMaxHierLevels]);   // windows per level, level 1 first; returns the level count
 int hierarchy_total_segments(int n);
 int hierarchy_seg_capacity();

@@ -248,3 +248,40 @@ def test_empty_inputs(B):
     off, idx = B.query(bvh, _dev(np.array([[5, 5, 5, 0.1], [-5, 0, 0, 0.1]], np.float32)))
     torch.cuda.synchronize()
     assert off.cpu().tolist() == [0, 0, 0]
+
+
+def test_deep_skewed_hierarchy(B, oracle_lib):
+    """Heavy-tailed coordinates (u^12): a deep, lopsided radix tree with long runs of equal codes near the origin, so
+    windows of the bottom-up pass hand over many subtrees and the upper windows see long chains."""
+    u = W.uniform_cube(300_000, seed=77).astype(np.float64)
+    pts = (u ** 12).astype(np.float32) + np.float32(0.0)
+    for bits in (30, 63):
+        o = oracle_lib.build_bvh(pts, bits)
+        bvh = gpu_build(B, pts, bits)
+        assert_build_equal(export_np(bvh), o, f"skewed {bits}")
+    assert_query_equal(B, bvh, o, oracle_lib, W.spheres_at(pts[:3000], 1e-3), "skewed")
+
+
+def test_merge_windows_multipass_reduced_capacity(B, oracle_lib, tmp_path):
+    """The upper windows of the bottom-up pass shorten an item list that does not fit their shared memory by passes
+    compacted in place.  With the product's capacity (2048 items per window) only degenerate inputs get there, so
+    this test compiles the same sources with the smallest legal capacity (384 items, 128 threads) and checks the
+    result of that build bit for bit: 64 hand-overs of ~8 subtrees each overflow 384 on ordinary data."""
+    import shutil
+
+    from paper_2402_00665_b200 import build as cuda_build
+
+    if shutil.which("nvcc") is None and not __import__("os").path.exists("/usr/local/cuda/bin/nvcc"):
+        pytest.skip("no nvcc on this box")
+    lib = cuda_build.build(out=str(tmp_path / "libbvh_small_windows.so"),
+                           extra=["-DBVH_MERGE_MAX_ITEMS=384", "-DBVH_MERGE_THREADS=128"])
+    saved = (B._lib, B.LIB_PATH)
+    try:
+        B._lib, B.LIB_PATH = None, lib
+        B.load_library()
+        for name, n in (("C3", 1_200_000), ("C5", 700_001)):
+            w = W.make(name, n=n, q=0)
+            o = oracle_lib.build_bvh(w.prims, w.morton_bits)
+            assert_build_equal(export_np(gpu_build(B, w.prims, w.morton_bits)), o, name)
+    finally:
+        B._lib, B.LIB_PATH = saved
