@@ -53,7 +53,7 @@ __device__ __forceinline__ void st_status(uint32_t* p, uint32_t v) {
 }
 
 #ifndef BVH_LOOKBACK_BATCH
-#define BVH_LOOKBACK_BATCH 8
+#define BVH_LOOKBACK_BATCH 4
 #endif
 constexpr int kLookbackBatch = BVH_LOOKBACK_BATCH;
 
@@ -70,29 +70,37 @@ struct SortSmem {
 };
 
 // Lanes of the warp whose digit equals this lane's: AND over the 8 digit bits of (ballot of the bit) or its
-// complement.  `peers` enters as the mask of participating lanes.
+// complement.  `peers` enters as the mask of participating lanes.  MATCH_ANY: one MATCH.ANY instruction instead;
+// its cost grows with the number of distinct digits in the warp, so it only pays for the most significant
+// digit (few distinct values among 32 keys that are neighbours in the input; measured on C3: 59 vs 68 us for
+// that pass, but 105 vs 75 us for the least significant one).
+template <bool MATCH_ANY>
 __device__ __forceinline__ uint32_t match_digit(uint32_t d, uint32_t peers) {
+  if (MATCH_ANY) {
+    peers &= __match_any_sync(0xffffffffu, d);
+  } else {
 #pragma unroll
-  for (int b = 0; b < 8; ++b) {
-    // four SASS instructions per bit: bit test -> predicate, VOTE, and one predicated LOP3 per polarity
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        ".reg .b32 t, bal;\n\t"
-        "and.b32 t, %1, %2;\n\t"
-        "setp.ne.u32 p, t, 0;\n\t"
-        "vote.sync.ballot.b32 bal, p, 0xffffffff;\n\t"
-        "@p and.b32 %0, %0, bal;\n\t"
-        "@!p not.b32 bal, bal;\n\t"
-        "@!p and.b32 %0, %0, bal;\n\t"
-        "}"
-        : "+r"(peers)
-        : "r"(d), "r"(1u << b));
+    for (int b = 0; b < 8; ++b) {
+      // four SASS instructions per bit: bit test -> predicate, VOTE, and one predicated LOP3 per polarity
+      asm volatile(
+          "{\n\t"
+          ".reg .pred p;\n\t"
+          ".reg .b32 t, bal;\n\t"
+          "and.b32 t, %1, %2;\n\t"
+          "setp.ne.u32 p, t, 0;\n\t"
+          "vote.sync.ballot.b32 bal, p, 0xffffffff;\n\t"
+          "@p and.b32 %0, %0, bal;\n\t"
+          "@!p not.b32 bal, bal;\n\t"
+          "@!p and.b32 %0, %0, bal;\n\t"
+          "}"
+          : "+r"(peers)
+          : "r"(d), "r"(1u << b));
+    }
   }
   return peers;
 }
 
-template <typename KeyT, bool IOTA, bool FULL>
+template <typename KeyT, bool IOTA, bool FULL, bool TOP>
 __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_out,
                                           const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ vals_out,
                                           const uint32_t* __restrict__ hist, uint32_t* status, uint32_t tile,
@@ -136,7 +144,8 @@ __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restr
   }
 
   // ---- rank within the warp, in tile order ---------------------------------------------------------------
-  uint32_t rank[ITEMS];
+  uint32_t rank2[ITEMS / 2];                          // two 16-bit ranks per register (a rank is < TILE <= 65536)
+  static_assert(ITEMS % 2 == 0 && SortCfg<KeyT>::TILE <= 65536, "packed ranks");
   const uint32_t lt_mask = (1u << lane) - 1u;
   uint32_t* my_hist = s.warp_hist[warp];
 #pragma unroll
@@ -144,10 +153,10 @@ __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restr
     const uint32_t d = (uint32_t)(key[j] >> shift) & 0xFFu;
     uint32_t peers;
     if (FULL) {
-      peers = match_digit(d, 0xffffffffu);
+      peers = match_digit<TOP>(d, 0xffffffffu);
     } else {
       const bool valid = (warp_off + j * 32) < valid_in_tile;
-      peers = match_digit(d, __ballot_sync(0xffffffffu, valid));
+      peers = match_digit<TOP>(d, __ballot_sync(0xffffffffu, valid));
       if (!valid) peers = 0;
     }
     // every peer reads the warp's running count of its digit (a broadcast), the lowest peer then bumps it
@@ -156,7 +165,10 @@ __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restr
     __syncwarp();
     if (below == 0 && (FULL || peers)) my_hist[d] = pre + __popc(peers);
     __syncwarp();
-    rank[j] = pre + below;
+    if (j & 1)
+      rank2[j / 2] |= (pre + below) << 16;
+    else
+      rank2[j / 2] = pre + below;
   }
 
   // values are only needed for the scatter: issue their loads now, they land during the look-back
@@ -259,7 +271,7 @@ __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restr
   for (int j = 0; j < ITEMS; ++j) {
     if (FULL || (warp_off + j * 32) < valid_in_tile) {
       const uint32_t d = (uint32_t)(key[j] >> shift) & 0xFFu;
-      const uint32_t pos = s.tile_excl[d] + my_hist[d] + rank[j];
+      const uint32_t pos = s.tile_excl[d] + my_hist[d] + ((j & 1) ? (rank2[j / 2] >> 16) : (rank2[j / 2] & 0xFFFFu));
       s.keys[pos] = key[j];
       s.vals[pos] = val[j];
     }
@@ -280,8 +292,11 @@ __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restr
   }
 }
 
-template <typename KeyT, bool IOTA>
-__global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads)
+#ifndef BVH_SORT_MINBLOCKS
+#define BVH_SORT_MINBLOCKS 4
+#endif
+template <typename KeyT, bool IOTA, bool TOP>
+__global__ void __launch_bounds__(kSortThreads, BVH_SORT_MINBLOCKS)
 onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_out, const uint32_t* __restrict__ vals_in,
                      uint32_t* __restrict__ vals_out, const uint32_t* __restrict__ hist, uint32_t* status,
                      uint32_t* tile_counter, int n, int shift) {
@@ -298,9 +313,9 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_o
   const uint32_t tile_base = tile * (uint32_t)TILE;
   const int valid_in_tile = min(TILE, n - (int)tile_base);
   if (valid_in_tile == TILE)
-    sort_tile<KeyT, IOTA, true>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, TILE, shift);
+    sort_tile<KeyT, IOTA, true, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, TILE, shift);
   else
-    sort_tile<KeyT, IOTA, false>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, valid_in_tile,
+    sort_tile<KeyT, IOTA, false, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, valid_in_tile,
                                  shift);
 }
 
@@ -309,17 +324,21 @@ static void sort_all(const SortBuffers& B, int n, int passes, cudaStream_t strea
   const int tiles = (n + SortCfg<KeyT>::TILE - 1) / SortCfg<KeyT>::TILE;
   KeyT* keys[2] = {static_cast<KeyT*>(B.keys[0]), static_cast<KeyT*>(B.keys[1])};
   const size_t smem = sizeof(SortSmem<KeyT>);
-  cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   for (int p = 0; p < passes; ++p) {
     const int in = p & 1, out = in ^ 1;
     uint32_t* st = B.status + (size_t)p * tiles * 256;
     uint32_t* vout = (p == passes - 1 && B.final_vals) ? B.final_vals : B.vals[out];
     if (p == 0)
-      onesweep_pass_kernel<KeyT, true><<<tiles, kSortThreads, smem, stream>>>(
+      onesweep_pass_kernel<KeyT, true, false><<<tiles, kSortThreads, smem, stream>>>(
           keys[in], keys[out], nullptr, vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
+    else if (p == passes - 1)
+      onesweep_pass_kernel<KeyT, false, true><<<tiles, kSortThreads, smem, stream>>>(
+          keys[in], keys[out], B.vals[in], vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
     else
-      onesweep_pass_kernel<KeyT, false><<<tiles, kSortThreads, smem, stream>>>(
+      onesweep_pass_kernel<KeyT, false, false><<<tiles, kSortThreads, smem, stream>>>(
           keys[in], keys[out], B.vals[in], vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
     if (pass_events && pass_events[p]) cudaEventRecord(static_cast<cudaEvent_t>(pass_events[p]), stream);
   }

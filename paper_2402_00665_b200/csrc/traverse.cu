@@ -68,13 +68,14 @@ struct SphereQuery {
     cx = v.x; cy = v.y; cz = v.z;
     r2 = __fmul_rn(v.w, v.w);
   }
-  __device__ __forceinline__ SphereQuery from_lane(int src) const {
-    SphereQuery o;
-    o.cx = __shfl_sync(0xffffffffu, cx, src);
-    o.cy = __shfl_sync(0xffffffffu, cy, src);
-    o.cz = __shfl_sync(0xffffffffu, cz, src);
-    o.r2 = __shfl_sync(0xffffffffu, r2, src);
-    return o;
+  // one slot of kSlotWords floats per thread in shared memory: how the warp reads the query of the lane it scans for
+  static constexpr int kSlotWords = 4;
+  __device__ __forceinline__ void to_shared(float* slot) const {
+    *reinterpret_cast<float4*>(slot) = make_float4(cx, cy, cz, r2);
+  }
+  __device__ __forceinline__ void from_shared(const float* slot) {
+    const float4 v = *reinterpret_cast<const float4*>(slot);     // one broadcast LDS.128
+    cx = v.x; cy = v.y; cz = v.z; r2 = v.w;
   }
   __device__ __forceinline__ bool hit_box(float lox, float loy, float loz, float hix, float hiy, float hiz) const {
     const float dx = fmaxf(fmaxf(__fsub_rn(lox, cx), __fsub_rn(cx, hix)), 0.0f);
@@ -98,14 +99,15 @@ struct BoxQuery {
     const float2 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
     lo[0] = a.x; lo[1] = a.y; lo[2] = b.x; hi[0] = b.y; hi[1] = c.x; hi[2] = c.y;
   }
-  __device__ __forceinline__ BoxQuery from_lane(int src) const {
-    BoxQuery o;
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-      o.lo[a] = __shfl_sync(0xffffffffu, lo[a], src);
-      o.hi[a] = __shfl_sync(0xffffffffu, hi[a], src);
-    }
-    return o;
+  static constexpr int kSlotWords = 8;
+  __device__ __forceinline__ void to_shared(float* slot) const {
+    reinterpret_cast<float4*>(slot)[0] = make_float4(lo[0], lo[1], lo[2], hi[0]);
+    reinterpret_cast<float2*>(slot)[2] = make_float2(hi[1], hi[2]);
+  }
+  __device__ __forceinline__ void from_shared(const float* slot) {
+    const float4 a = reinterpret_cast<const float4*>(slot)[0];
+    const float2 b = reinterpret_cast<const float2*>(slot)[2];
+    lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; hi[0] = a.w; hi[1] = b.x; hi[2] = b.y;
   }
   __device__ __forceinline__ bool hit_box(float lox, float loy, float loz, float hix, float hiy, float hiz) const {
     return lo[0] <= hix && lox <= hi[0] && lo[1] <= hiy && loy <= hi[1] && lo[2] <= hiz && loz <= hi[2];
@@ -149,10 +151,15 @@ __device__ __forceinline__ void traverse_body(const char* __restrict__ nodes, in
                                               const int64_t* __restrict__ offsets, int32_t* __restrict__ indices,
                                               int64_t num_chunks, int ctas_per_sm) {
   constexpr int U = POINT_LEAF ? BVH_SCAN_UNROLL : (BVH_SCAN_UNROLL > 2 ? 2 : BVH_SCAN_UNROLL);   // leaf loads in flight per lane
+  // what a lane posts for the warp to read: its query, the leaf range to scan, (fill) where its row starts
+  __shared__ __align__(16) float s_query[kTravThreads * Query::kSlotWords];
+  __shared__ int2 s_range[kTravThreads];
+  __shared__ int64_t s_row[FILL ? kTravThreads : 1];
   const Node* __restrict__ internal = reinterpret_cast<const Node*>(nodes + kNodesHeaderBytes);
   const char* __restrict__ leaves = nodes + leaf_offset_bytes(n);
   const int leaf_base = n - 1;
   const int lane = threadIdx.x & 31;
+  const int warp_first = threadIdx.x - lane;               // slot of lane 0 of this warp
   const uint32_t lt_mask = (1u << lane) - 1u;
   const int64_t sm_slot = blockIdx.x % kNumSMs;
   const int64_t r = blockIdx.x / kNumSMs;
@@ -164,15 +171,20 @@ __device__ __forceinline__ void traverse_body(const char* __restrict__ nodes, in
     const int64_t j = have ? (order ? (int64_t)order[t] : t) : 0;
     Query query;
     query.load(queries, j);
-    int32_t* row = FILL ? indices + (have ? offsets[j] : 0) : nullptr;   // this query's CSR row
+    __syncwarp();                                            // the previous chunk's scans are over
+    query.to_shared(s_query + threadIdx.x * Query::kSlotWords);
+    if (FILL) s_row[threadIdx.x] = have ? offsets[j] : 0;    // this query's CSR row
+    __syncwarp();
+    int32_t* const row = FILL ? indices + s_row[FILL ? threadIdx.x : 0] : nullptr;
     int count = 0;
     int node = have ? 0 : kSentinel;                         // L1: start from the root
     int first = 0;                                           // first leaf below `node`
-    int scan_i = 0, scan_end = 0;                            // posted leaf range [scan_i, scan_end)
+    bool post = false;                                       // this lane posted a leaf range in the last round
     while (true) {                                           // L2 ... L11 for the 32 queries of the warp
       const bool walking = node != kSentinel;
-      uint32_t posted = __ballot_sync(0xffffffffu, scan_i < scan_end);
+      uint32_t posted = __ballot_sync(0xffffffffu, post);
       if (!__any_sync(0xffffffffu, walking) && posted == 0) break;
+      post = false;
       // ---- WALK, first half: fetch this lane's node; the record is consumed after the SCAN below, which runs while
       // the load is in flight ----
       const bool at_internal = walking && node < leaf_base;
@@ -182,28 +194,40 @@ __device__ __forceinline__ void traverse_body(const char* __restrict__ nodes, in
       while (posted) {
         const int o = __ffs(posted) - 1;
         posted &= posted - 1;
-        const Query oq = query.from_lane(o);
-        const int begin = __shfl_sync(0xffffffffu, scan_i, o);
-        const int end = __shfl_sync(0xffffffffu, scan_end, o);
-        int ocount = __shfl_sync(0xffffffffu, count, o);
+        Query oq;
+        oq.from_shared(s_query + (warp_first + o) * Query::kSlotWords);
+        const int2 range = s_range[warp_first + o];
+        const int end = range.y;
+        int ocount = 0;                                    // count: this lane's hits; fill: the row's running length
         int32_t* orow = nullptr;
-        if (FILL) orow = reinterpret_cast<int32_t*>(__shfl_sync(0xffffffffu, reinterpret_cast<unsigned long long>(row), o));
-        for (int c = begin + lane; c < end + lane; c += 32 * U) {   // c - lane is warp-uniform
+        if (FILL) {
+          ocount = __shfl_sync(0xffffffffu, count, o);
+          orow = indices + s_row[warp_first + o];
+        }
+        for (int c = range.x + lane; c < end + lane; c += 32 * U) {   // c - lane is warp-uniform
           LeafRec<POINT_LEAF> leaf[U];
 #pragma unroll
           for (int u = 0; u < U; ++u)
             if (c + 32 * u < end) leaf[u].load(leaves, c + 32 * u);
 #pragma unroll
           for (int u = 0; u < U; ++u) {
-            const bool hit = (c + 32 * u < end) && leaf[u].hit(oq);                   // L3-5 on leaf c + 32u
-            const uint32_t m = __ballot_sync(0xffffffffu, hit);
-            if (FILL && hit) orow[ocount + __popc(m & lt_mask)] = (int)(leaf[u].payload() & kLeafPrimMask);
-            ocount += __popc(m);
+            const bool inside = c + 32 * u < end;
+            const bool sat = leaf[u].hit(oq);              // evaluated on every lane (no branch); masked below
+            const bool hit = inside & sat;                 // L3-5 on leaf c + 32u
+            if (FILL) {
+              const uint32_t m = __ballot_sync(0xffffffffu, hit);
+              if (hit) orow[ocount + __popc(m & lt_mask)] = (int)(leaf[u].payload() & kLeafPrimMask);
+              ocount += __popc(m);
+            } else {
+              ocount += hit ? 1 : 0;
+            }
           }
         }
-        if (lane == o) {
-          count = ocount;
-          scan_i = scan_end;
+        if (FILL) {
+          if (lane == o) count = ocount;
+        } else {
+          const int total = __reduce_add_sync(0xffffffffu, ocount);   // one REDUX per range instead of a ballot per step
+          if (lane == o) count += total;
         }
       }
       // ---- WALK, second half: one step of Algorithm 1 per lane ---------------------------------------------------
@@ -227,8 +251,8 @@ __device__ __forceinline__ void traverse_body(const char* __restrict__ nodes, in
           int next = rope;                                   // L10: N_skip
           if (query.hit_box(rec.lox, rec.loy, rec.loz, rec.hix, rec.hiy, rec.hiz)) {   // L3
             if (next_first - first <= kScanLeaves) {         // small subtree: post its leaves, continue after it
-              scan_i = first;
-              scan_end = next_first;
+              s_range[threadIdx.x] = make_int2(first, next_first);
+              post = true;
             } else {
               next = rec.left;                               // L8: N_left (same first leaf)
             }
@@ -237,6 +261,7 @@ __device__ __forceinline__ void traverse_body(const char* __restrict__ nodes, in
           node = next;
         }
       }
+      __syncwarp();                                          // posted ranges are visible to the warp
     }
     if (!FILL && have) counts[j] = count;
   }
