@@ -33,6 +33,8 @@ __device__ __forceinline__ void fold_role(int role, bool is_box, float mn, float
 
 __global__ void __launch_bounds__(kBoundsThreads) scene_bounds_kernel(const float* __restrict__ prim, int64_t nfloats,
                                                                       bool is_box, Header* __restrict__ header) {
+  pdl_wait();
+  pdl_trigger();
   const float inf = __int_as_float(0x7f800000);
   float mn[3][4], mx[3][4];
 #pragma unroll
@@ -109,7 +111,7 @@ void launch_scene_bounds(const float* prim, int n, bool is_box, Header* header, 
   const int64_t cap = (int64_t)kNumSMs * 8;
   if (blocks > cap) blocks = cap;
   if (blocks < 1) blocks = 1;
-  scene_bounds_kernel<<<(unsigned)blocks, kBoundsThreads, 0, stream>>>(prim, nfloats, is_box, header);
+  launch_pdl(scene_bounds_kernel, dim3((unsigned)blocks), dim3(kBoundsThreads), 0, stream, prim, nfloats, is_box, header);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -157,6 +159,8 @@ __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __r
                                                                 KeyT* __restrict__ codes, uint32_t* __restrict__ hist) {
   __shared__ uint32_t s_hist[PASSES * 256];
   for (int i = threadIdx.x; i < PASSES * 256; i += kMortonThreads) s_hist[i] = 0;
+  pdl_wait();
+  pdl_trigger();
   float scene[6];
   if (FROM_ROOT) {
 #pragma unroll
@@ -223,14 +227,14 @@ void launch_morton(const float* prim, int n, bool is_box, int morton_bits, const
   const unsigned g = morton_grid(n);
   if (morton_bits == 30) {
     if (is_box)
-      morton_kernel<uint32_t, 4, 6, false><<<g, kMortonThreads, 0, stream>>>(prim, n, header, nullptr, (uint32_t*)codes, hist);
+      launch_pdl(morton_kernel<uint32_t, 4, 6, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint32_t*)codes, hist);
     else
-      morton_kernel<uint32_t, 4, 3, false><<<g, kMortonThreads, 0, stream>>>(prim, n, header, nullptr, (uint32_t*)codes, hist);
+      launch_pdl(morton_kernel<uint32_t, 4, 3, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint32_t*)codes, hist);
   } else {
     if (is_box)
-      morton_kernel<uint64_t, 8, 6, false><<<g, kMortonThreads, 0, stream>>>(prim, n, header, nullptr, (uint64_t*)codes, hist);
+      launch_pdl(morton_kernel<uint64_t, 8, 6, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint64_t*)codes, hist);
     else
-      morton_kernel<uint64_t, 8, 3, false><<<g, kMortonThreads, 0, stream>>>(prim, n, header, nullptr, (uint64_t*)codes, hist);
+      launch_pdl(morton_kernel<uint64_t, 8, 3, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint64_t*)codes, hist);
   }
 }
 
@@ -238,9 +242,9 @@ void launch_query_morton(const float* queries, int q, int kind, const NodesHeade
                          cudaStream_t stream) {
   const unsigned g = morton_grid(q);
   if (kind == 0)
-    morton_kernel<uint32_t, 4, 4, true><<<g, kMortonThreads, 0, stream>>>(queries, q, nullptr, root, codes, hist);
+    launch_pdl(morton_kernel<uint32_t, 4, 4, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist);
   else
-    morton_kernel<uint32_t, 4, 6, true><<<g, kMortonThreads, 0, stream>>>(queries, q, nullptr, root, codes, hist);
+    launch_pdl(morton_kernel<uint32_t, 4, 6, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist);
 }
 
 }  // namespace bvh

@@ -466,6 +466,8 @@ hierarchy_local_kernel(const float* __restrict__ prim, const KeyT* __restrict__ 
   Node* nodes = reinterpret_cast<Node*>(nodes_base + kNodesHeaderBytes);   // internal records, by Karras index
   char* leaves = nodes_base + leaf_offset_bytes(n);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  pdl_wait();
+  pdl_trigger();
   if (blockIdx.x == 0 && tid == 0) {                          // the hierarchy's header: leaf format and root box
     NodesHeader* h = reinterpret_cast<NodesHeader*>(nodes_base);
     float sb[6];
@@ -665,6 +667,8 @@ hierarchy_merge_kernel(const KeyT* __restrict__ codes, char* nodes_base, int n, 
   __shared__ uint32_t s_wsum[kMergeThreads / 32 + 1];
   __shared__ int s_last;
   const int tid = threadIdx.x;
+  pdl_wait();
+  pdl_trigger();
   int window = blockIdx.x;
   for (int level = 1; level < lv.levels; ++level) {     // array index of the level this block is a window of
     merge_window<KeyT>(S, s_wsum, codes, nodes_base, n, leaf_kind, window,
@@ -720,16 +724,16 @@ static void launch_hierarchy_keys(const float* prim, bool is_box, const KeyT* co
     off += lv.segs[l];
   }
   if (is_box)
-    hierarchy_local_kernel<KeyT, true><<<lv.segs[0], kHierThreads, 0, stream>>>(prim, codes, perm, nodes, n, header, seg_items,
+    launch_pdl(hierarchy_local_kernel<KeyT, true>, dim3(lv.segs[0]), dim3(kHierThreads), 0, stream, prim, codes, perm, nodes, n, header, seg_items,
                                                                                seg_count);
   else
-    hierarchy_local_kernel<KeyT, false><<<lv.segs[0], kHierThreads, 0, stream>>>(prim, codes, perm, nodes, n, header, seg_items,
+    launch_pdl(hierarchy_local_kernel<KeyT, false>, dim3(lv.segs[0]), dim3(kHierThreads), 0, stream, prim, codes, perm, nodes, n, header, seg_items,
                                                                                 seg_count);
   if (lv.levels > 1) {
     using D = typename Delta<KeyT>::T;
     const size_t smem = sizeof(MergeSmem<D>);
     cudaFuncSetAttribute(hierarchy_merge_kernel<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    hierarchy_merge_kernel<KeyT><<<lv.segs[1], kMergeThreads, smem, stream>>>(codes, nodes, n, is_box ? kLeafBoxes : kLeafPoints,
+    launch_pdl(hierarchy_merge_kernel<KeyT>, dim3(lv.segs[1]), dim3(kMergeThreads), smem, stream, codes, nodes, n, is_box ? kLeafBoxes : kLeafPoints,
                                                                              seg_items, seg_count, arrivals, lv);
   }
 }

@@ -305,9 +305,11 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_o
   SortSmem<KeyT>& s = *reinterpret_cast<SortSmem<KeyT>*>(smem_raw);
 
   const int tid = threadIdx.x;
-  if (tid == 0) s.tile = atomicAdd(tile_counter, 1u);
   for (int i = tid; i < kSortWarps * 256; i += kSortThreads) (&s.warp_hist[0][0])[i] = 0;
   if (tid < 256) s.tile_hist[tid] = 0;
+  pdl_wait();
+  pdl_trigger();
+  if (tid == 0) s.tile = atomicAdd(tile_counter, 1u);
   __syncthreads();
   const uint32_t tile = s.tile;
   const uint32_t tile_base = tile * (uint32_t)TILE;
@@ -332,14 +334,14 @@ static void sort_all(const SortBuffers& B, int n, int passes, cudaStream_t strea
     uint32_t* st = B.status + (size_t)p * tiles * 256;
     uint32_t* vout = (p == passes - 1 && B.final_vals) ? B.final_vals : B.vals[out];
     if (p == 0)
-      onesweep_pass_kernel<KeyT, true, false><<<tiles, kSortThreads, smem, stream>>>(
-          keys[in], keys[out], nullptr, vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
+      launch_pdl(onesweep_pass_kernel<KeyT, true, false>, dim3(tiles), dim3(kSortThreads), smem, stream,
+                 keys[in], keys[out], nullptr, vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
     else if (p == passes - 1)
-      onesweep_pass_kernel<KeyT, false, true><<<tiles, kSortThreads, smem, stream>>>(
-          keys[in], keys[out], B.vals[in], vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
+      launch_pdl(onesweep_pass_kernel<KeyT, false, true>, dim3(tiles), dim3(kSortThreads), smem, stream,
+                 keys[in], keys[out], B.vals[in], vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
     else
-      onesweep_pass_kernel<KeyT, false, false><<<tiles, kSortThreads, smem, stream>>>(
-          keys[in], keys[out], B.vals[in], vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
+      launch_pdl(onesweep_pass_kernel<KeyT, false, false>, dim3(tiles), dim3(kSortThreads), smem, stream,
+                 keys[in], keys[out], B.vals[in], vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
     if (pass_events && pass_events[p]) cudaEventRecord(static_cast<cudaEvent_t>(pass_events[p]), stream);
   }
 }
