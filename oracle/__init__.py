@@ -50,11 +50,11 @@ def _L():
         lib.oracle_ropes_alg2.argtypes = [u64p, i32p, i32p, i64, i32p]
         lib.oracle_boxes.argtypes = [fp, c_int, u32p, i32p, i32p, i64, fp]
         lib.oracle_build.argtypes = [fp, i64, c_int, c_int, u64p, u32p, i32p, i32p, fp, fp, i32p]
-        for name in ("oracle_query_spheres_tree", "oracle_query_boxes_tree"):
+        for name in ("oracle_query_spheres_tree", "oracle_query_boxes_tree", "oracle_query_rays_tree"):
             f = getattr(lib, name)
             f.argtypes = [fp, i32p, i32p, i64, fp, i64]
             f.restype = c_void_p
-        for name in ("oracle_query_spheres_brute", "oracle_query_boxes_brute"):
+        for name in ("oracle_query_spheres_brute", "oracle_query_boxes_brute", "oracle_query_rays_brute"):
             f = getattr(lib, name)
             f.argtypes = [fp, i64, c_int, fp, i64]
             f.restype = c_void_p
@@ -220,6 +220,23 @@ def query_boxes_brute(prim, minmax):
     a, n, is_box = _prims(prim)
     qa = np.ascontiguousarray(minmax, np.float32)
     h = _L().oracle_query_boxes_brute(_p(a, c_float), n, is_box, _p(qa, c_float), qa.shape[0])
+    return _finish(h, qa.shape[0])
+
+
+def query_rays_tree(bvh: Bvh, rays):
+    """D9 (NEXT-1): rays [q,8] = {origin.xyz, direction.xyz, tmin, tmax}; stack traversal of the oracle tree."""
+    qa = np.ascontiguousarray(rays, np.float32)
+    assert qa.ndim == 2 and qa.shape[1] == 8
+    h = _L().oracle_query_rays_tree(_p(bvh.aabb, c_float), _p(bvh.left_child, c_int32),
+                                    _p(bvh.right_child, c_int32), bvh.n, _p(qa, c_float), qa.shape[0])
+    return _finish(h, qa.shape[0])
+
+
+def query_rays_brute(prim, rays):
+    a, n, is_box = _prims(prim)
+    qa = np.ascontiguousarray(rays, np.float32)
+    assert qa.ndim == 2 and qa.shape[1] == 8
+    h = _L().oracle_query_rays_brute(_p(a, c_float), n, is_box, _p(qa, c_float), qa.shape[0])
     return _finish(h, qa.shape[0])
 
 

@@ -103,6 +103,38 @@ inline bool box_hits_box(const float qlo[3], const float qhi[3], const float lo[
   return true;
 }
 
+// D9 ray-vs-box (NEXT-1; "all triangles ... that a ray intersects").  Ray {o.xyz, d.xyz, tmin, tmax}:
+// the points o + t d, tmin <= t <= tmax.  Slab test, fp32 round-to-nearest, one operation per step:
+// per axis with d != 0: inv = 1 / d, t1 = (lo - o) * inv, t2 = (hi - o) * inv, the ray's interval is clipped to
+// [min(t1,t2), max(t1,t2)]; per axis with d == 0 the ray never leaves the slab or never enters it: lo <= o <= hi
+// (closed, G12).  Hit iff the clipped interval is not empty (tn <= tf: touching counts).
+inline bool ray_hits_box(const float ray[8], const float lo[3], const float hi[3]) {
+  float tn = ray[6], tf = ray[7];
+  for (int a = 0; a < 3; ++a) {
+    const float o = ray[a], d = ray[3 + a];
+    if (d == 0.0f) {
+      if (!(lo[a] <= o && o <= hi[a])) return false;
+    } else {
+      const float inv = 1.0f / d;
+      float t1 = lo[a] - o;
+      t1 = t1 * inv;
+      float t2 = hi[a] - o;
+      t2 = t2 * inv;
+      const float tmin_a = t1 < t2 ? t1 : t2;
+      const float tmax_a = t1 < t2 ? t2 : t1;
+      tn = fmax2(tn, tmin_a);
+      tf = tf < tmax_a ? tf : tmax_a;
+    }
+  }
+  return tn <= tf;
+}
+
+inline bool query_hits_box(int kind, const float* queries, int64_t j, const float lo[3], const float hi[3]) {
+  if (kind == 0) return sphere_hits_box(queries + 4 * j, queries[4 * j + 3], lo, hi);
+  if (kind == 1) return box_hits_box(queries + 6 * j, queries + 6 * j + 3, lo, hi);
+  return ray_hits_box(queries + 8 * j, lo, hi);
+}
+
 struct CsrResult {
   std::vector<int64_t> offsets;
   std::vector<int32_t> indices;
@@ -337,11 +369,7 @@ static void* query_tree(int kind, const float* aabb, const int32_t* left_child,
         int32_t node = stack.back();
         stack.pop_back();
         const float* b = aabb + 6 * (int64_t)node;
-        bool hit;
-        if (kind == 0)
-          hit = sphere_hits_box(queries + 4 * j, queries[4 * j + 3], b, b + 3);
-        else
-          hit = box_hits_box(queries + 6 * j, queries + 6 * j + 3, b, b + 3);
+        const bool hit = query_hits_box(kind, queries, j, b, b + 3);
         if (!hit) continue;
         if (node >= leaf_base) {
           res->indices.push_back(left_child[node]);
@@ -366,6 +394,11 @@ void* oracle_query_boxes_tree(const float* aabb, const int32_t* left_child,
   return query_tree(1, aabb, left_child, right_child, n, minmax, q);
 }
 
+void* oracle_query_rays_tree(const float* aabb, const int32_t* left_child, const int32_t* right_child,
+                             int64_t n, const float* rays, int64_t q) {
+  return query_tree(2, aabb, left_child, right_child, n, rays, q);
+}
+
 // Brute force: the plain definition of range search: every primitive is tested.
 // Reports original primitive indices in ascending order.
 static void* query_brute(int kind, const float* prim, int64_t n, int is_box, const float* queries,
@@ -375,12 +408,7 @@ static void* query_brute(int kind, const float* prim, int64_t n, int is_box, con
   for (int64_t j = 0; j < q; ++j) {
     for (int64_t i = 0; i < n; ++i) {
       Box b = prim_box(prim, i, is_box);
-      bool hit;
-      if (kind == 0)
-        hit = sphere_hits_box(queries + 4 * j, queries[4 * j + 3], b.lo, b.hi);
-      else
-        hit = box_hits_box(queries + 6 * j, queries + 6 * j + 3, b.lo, b.hi);
-      if (hit) res->indices.push_back((int32_t)i);
+      if (query_hits_box(kind, queries, j, b.lo, b.hi)) res->indices.push_back((int32_t)i);
     }
     res->offsets[(size_t)j + 1] = (int64_t)res->indices.size();
   }
@@ -395,6 +423,10 @@ void* oracle_query_spheres_brute(const float* prim, int64_t n, int is_box, const
 void* oracle_query_boxes_brute(const float* prim, int64_t n, int is_box, const float* minmax,
                                int64_t q) {
   return query_brute(1, prim, n, is_box, minmax, q);
+}
+
+void* oracle_query_rays_brute(const float* prim, int64_t n, int is_box, const float* rays, int64_t q) {
+  return query_brute(2, prim, n, is_box, rays, q);
 }
 
 int64_t oracle_result_nnz(void* h) { return (int64_t) static_cast<CsrResult*>(h)->indices.size(); }

@@ -137,6 +137,17 @@ def spheres_at(centres: np.ndarray, radius: float) -> np.ndarray:
     return _f32(out)
 
 
+def rays_at(origins: np.ndarray, directions: np.ndarray, tmin: float, tmax: float) -> np.ndarray:
+    """[q,8] fp32 {origin.xyz, direction.xyz, tmin, tmax} (NEXT-1 ray queries: the segment o + t d, tmin <= t <= tmax)."""
+    q = origins.shape[0]
+    out = np.empty((q, 8), np.float32)
+    out[:, :3] = origins
+    out[:, 3:6] = directions
+    out[:, 6] = np.float32(tmin)
+    out[:, 7] = np.float32(tmax)
+    return _f32(out)
+
+
 # ---- the five configs ------------------------------------------------------------------------------
 
 @dataclass

@@ -390,3 +390,87 @@ def test_p5_touching_counts(oracle_lib):
     assert list(i) == [0]
     o, i = oracle_lib.query_boxes_brute(prim, np.array([[0, 0, 0, 0.99999994, 1, 1]], np.float32))
     assert list(i) == []
+
+
+# ---- D9 (NEXT-1): ray predicate -----------------------------------------------------------------------------
+
+def test_d9_ray_closed_forms(oracle_lib):
+    """Axis-aligned and diagonal rays against boxes on a lattice: hits known by inspection; touching counts (G12);
+    a ray parallel to a slab is inside it or never enters it; [tmin, tmax] clips the ray."""
+    boxes = np.array([[0, 0, 0, 1, 1, 1], [2, 0, 0, 3, 1, 1], [0, 2, 0, 1, 3, 1], [2, 2, 2, 3, 3, 3]], np.float32)
+    rays = np.array([
+        [-1, .5, .5, 1, 0, 0, 0, 10],      # +x through boxes 0 and 1
+        [-1, .5, .5, 1, 0, 0, 0, 2.5],     # stops at x = 1.5: box 0 only
+        [-1, .5, .5, 1, 0, 0, 2.5, 10],    # starts at x = 1.5: box 1 only
+        [-1, .5, .5, -1, 0, 0, 0, 10],     # points away
+        [.5, -1, .5, 0, 1, 0, 0, 10],      # +y through boxes 0 and 2
+        [-1, 1, .5, 1, 0, 0, 0, 10],       # grazes the face y = 1: touching counts
+        [-1, 1.5, .5, 1, 0, 0, 0, 10],     # between the rows: nothing
+        [-1, -1, -1, 1, 1, 1, 0, 10],      # the diagonal: boxes 0 and 3
+        [-1, -1, -1, 1, 1, 1, 0, 3],       # ... clipped at (2,2,2): reaches the corner of box 3 (touching)
+        [-1, -1, -1, 1, 1, 1, 0, 2.5],     # ... clipped before box 3
+        [-1, .5, .5, 2, 0, 0, 0, 1],       # faster ray: t in [0,1] covers x in [-1,1]: box 0
+    ], np.float32)
+    off, idx = oracle_lib.query_rays_brute(boxes, rays)
+    rows = [sorted(idx[off[j]:off[j + 1]].tolist()) for j in range(len(rays))]
+    assert rows == [[0, 1], [0], [1], [], [0, 2], [0, 1], [], [0, 3], [0, 3], [0], [0]]
+
+
+def test_d9_ray_matches_exact_rational(oracle_lib):
+    """Inputs on which every fp32 operation of D9 is exact (coordinates and t in multiples of 1/8, direction
+    components 0, +-1/2, +-1, +-2): the oracle must equal the slab test evaluated in exact rational arithmetic."""
+    from fractions import Fraction as F
+
+    rng = np.random.default_rng(9)
+    nb, nr = 60, 400
+    lo = rng.integers(-40, 40, size=(nb, 3))
+    ext = rng.integers(0, 24, size=(nb, 3))
+    boxes = (np.concatenate([lo, lo + ext], axis=1) / 8.0).astype(np.float32)
+    o = rng.integers(-48, 48, size=(nr, 3)) / 8.0
+    d = rng.choice([0.0, 0.5, -0.5, 1.0, -1.0, 2.0, -2.0], size=(nr, 3))
+    tmin = rng.integers(0, 16, size=nr) / 8.0
+    tmax = tmin + rng.integers(0, 80, size=nr) / 8.0
+    rays = np.concatenate([o, d, tmin[:, None], tmax[:, None]], axis=1).astype(np.float32)
+    off, idx = oracle_lib.query_rays_brute(boxes, rays)
+    for j in range(nr):
+        expect = []
+        for i in range(nb):
+            tn, tf, ok = F(float(tmin[j])), F(float(tmax[j])), True
+            for a in range(3):
+                oa, da = F(float(o[j, a])), F(float(d[j, a]))
+                l, h = F(float(boxes[i, a])), F(float(boxes[i, 3 + a]))
+                if da == 0:
+                    ok = ok and (l <= oa <= h)
+                else:
+                    t1, t2 = (l - oa) / da, (h - oa) / da
+                    tn, tf = max(tn, min(t1, t2)), min(tf, max(t1, t2))
+            if ok and tn <= tf:
+                expect.append(i)
+        assert idx[off[j]:off[j + 1]].tolist() == expect, j
+
+
+def _ray_case(name, n, q):
+    """Boxes a ray has a chance to hit, and rays through them: (prims [n,6], rays [q,8])."""
+    if name == "C2":
+        prims = W.boxes_around(W.make("C2", n=n, q=0).prims, 0.01)
+        origins = W.uniform_cube(q, seed=77)
+    else:
+        prims = W.make("C4", n=n, q=0, radius=0.02).prims
+        origins = W.uniform_cube(q, seed=78) * np.float32(3.0) - np.float32(1.5)
+    rays = W.rays_at(origins, W.sphere_surface(q, seed=55), 0.0, 0.4 if name == "C2" else 3.0)
+    rays[: q // 4, 3] = 0.0                       # some rays parallel to the x slabs
+    rays[q // 4: q // 3, 4:6] = 0.0               # some along the x axis
+    rays[q // 4: q // 3, 3] = 1.0
+    return prims, rays
+
+
+@pytest.mark.parametrize("name,n,q", [("C2", 30000, 300), ("C4", 30000, 300)])
+def test_d9_ray_tree_equals_brute(oracle_lib, name, n, q):
+    """The hit set does not depend on the tree (every step of D9 is monotone in the box, so a hit leaf implies hit
+    ancestors): stack traversal of the oracle tree = brute force over all primitives."""
+    prims, rays = _ray_case(name, n, q)
+    o = oracle_lib.build_bvh(prims, 63)
+    toff, tidx = oracle_lib.query_rays_tree(o, rays)
+    boff, bidx = oracle_lib.query_rays_brute(prims, rays)
+    assert np.array_equal(toff, boff) and toff[-1] > q
+    assert np.array_equal(csr_rows_sorted(toff, tidx), bidx)
