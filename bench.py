@@ -334,6 +334,31 @@ def run_ours(args) -> dict | None:
         e2e_q += qq
     dist_barrier(world, device)
 
+    # ---- NEXT-1: ray queries through the same traversal kernel (only where a ray can hit something: box primitives)
+    rays_info = None
+    if is_box and rank == 0:
+        qr = int(min(max(q, 1), 1 << 20))
+        lo, hi = w.prims[:, :3].min(axis=0), w.prims[:, 3:].max(axis=0)
+        origins = workloads.uniform_cube(qr, seed=2001) * (hi - lo) * np.float32(1.2) + lo - (hi - lo) * np.float32(0.1)
+        h_rays = workloads.rays_at(origins.astype(np.float32), workloads.sphere_surface(qr, seed=2002), 0.0,
+                                   float(np.linalg.norm(hi - lo)))
+        d_rays = torch.from_numpy(h_rays).to(device)
+        wr = binding.QueryWorkspace(qr, device)
+        off_r, idx_r = binding.query(bvh, d_rays, wr)          # sizes the result
+        ridx = torch.empty(max(int(idx_r.numel()), 1), dtype=torch.int32, device=device)
+        rt = []
+        for _ in range(4):
+            flush.fill_(1)
+            r0 = ev()
+            binding.query(bvh, d_rays, wr, indices=ridx)
+            r1 = ev()
+            torch.cuda.synchronize()
+            rt.append(r0.elapsed_time(r1))
+        rms = float(np.median(rt[1:]))
+        rays_info = {"q": qr, "ms": round(rms, 4), "mrays_per_s": round(qr / (rms * 1e-3) / 1e6, 3),
+                     "hits_per_ray": round(int(off_r[qr].item()) / qr, 3),
+                     "what": "order + count + scan + fill of segments through the scene box, random directions"}
+
     # ---- reduce over ranks: time = max, units = sum -----------------------------------------------------------------
     keys = sorted(acc)
     mx, sm = reduce_max_sum([acc[k] for k in keys] + [e2e_b, e2e_q], [float(n), float(q), float(nnz)], world, device)
@@ -386,6 +411,8 @@ def run_ours(args) -> dict | None:
                         "nnz read-back, alloc, fill -> CSR offsets+indices D2H; wall clock, through binding.Bvh/query"},
         "clocks": clocks,
     }
+    if rays_info:
+        line["next1_rays"] = rays_info
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(w)
     return line

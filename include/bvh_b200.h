@@ -22,10 +22,12 @@
  * in ONE index space of 2n-1 nodes: internal node I_k -> k (k in [0, n-2], Karras
  * numbering: siblings at consecutive indices, root = 0), leaf L_i -> (n-1)+i where
  * i is the position in Morton order.  The sentinel is -1.  For n = 1 the single
- * leaf is node 0.  `nodes` is an opaque array of (2n-1) 32-byte records
- *     { float min[3]; int32 left_child;  float max[3]; int32 rope; }
- * For an internal node `left_child` is its left child (PAPER.md:46 N_left); for a leaf it is the
- * ORIGINAL index of the primitive stored there.  `rope` is the skip-connection N_skip.
+ * leaf is node 0.  `nodes` is an opaque buffer of bvh_sizes' node_bytes: a 64-byte header, the n-1 internal
+ * records { float min[3]; int32 left_child;  float max[3]; int32 rope; } by Karras index, then the n leaf records
+ * in Morton order (16 bytes {x, y, z, payload} after bvh_build_points, 32 bytes after bvh_build_boxes; the
+ * payload is the ORIGINAL index of the primitive plus one bit that tells whether the leaf's skip-connection is
+ * the leaf or the internal node i+1, Algorithm 2).  bvh_export turns it into the canonical arrays of the
+ * unified index space: left_child (PAPER.md:46 N_left; for a leaf: the primitive), rope (N_skip), boxes.
  */
 #ifndef BVH_B200_H
 #define BVH_B200_H
@@ -47,9 +49,10 @@ extern "C" {
 /* Library version, for the binding's sanity check. */
 int bvh_version(void);
 
-/* Bytes the caller must provide for a hierarchy over n primitives: node_bytes = 32*(2n-1) (32 when
- * n = 0), scratch_bytes = codes + permutation ping-pong buffers, radix-sort histograms and tile
- * status words, the `store` array of Algorithm 4 and the scene bounds.  Host call. */
+/* Bytes the caller must provide for a hierarchy over n primitives: node_bytes = 64 + 32*(n-1) + 32*n (one
+ * size for both leaf formats), scratch_bytes = codes + permutation ping-pong buffers, radix-sort histograms
+ * and tile status words, the hand-over segments and arrival counters of the bottom-up pass (the `store`
+ * array of Algorithm 4, lives in shared memory) and the scene bounds.  Host call. */
 int bvh_sizes(int64_t n, int morton_bits, size_t* node_bytes, size_t* scratch_bytes);
 
 /* Build (PAPER.md:83-93 with steps 3-4 replaced by Algorithm 4).
@@ -112,6 +115,21 @@ int bvh_query_spheres_fill(const void* nodes, int64_t n, const float* xyzr, int6
                            const int64_t* offsets, int32_t* indices, void* stream);
 int bvh_query_boxes_fill(const void* nodes, int64_t n, const float* minmax, int64_t q, const uint32_t* order,
                          const int64_t* offsets, int32_t* indices, void* stream);
+
+/* NEXT-1: ray queries, "all [primitives] that a ray intersects", through the same
+ * Algorithm 1 kernel with a third predicate.  A ray is 8 floats {origin.xyz, direction.xyz, tmin, tmax}: the points
+ * o + t d with tmin <= t <= tmax (a segment; tmax may be large).  Predicate D9: slab test in fp32
+ * round-to-nearest; per axis with d != 0, inv = 1/d, t1 = (min - o) * inv, t2 = (max - o) * inv clip the interval;
+ * per axis with d == 0 the test is min <= o <= max; hit iff the clipped interval is not empty (touching counts).
+ * Direction components must be 0 or normal numbers whose reciprocal is finite; not checked.  rays: q*8 floats,
+ * 16-byte aligned.  Same count -> bvh_scan_counts -> fill protocol, same CSR, same `order` semantics (rays are
+ * ordered by the Morton code of their origin clamped into the root box). */
+int bvh_query_order_rays(const void* nodes, int64_t n, const float* rays, int64_t q, uint32_t* order, void* scratch,
+                         size_t scratch_bytes, void* stream);
+int bvh_query_rays_count(const void* nodes, int64_t n, const float* rays, int64_t q, const uint32_t* order,
+                         int32_t* counts, void* stream);
+int bvh_query_rays_fill(const void* nodes, int64_t n, const float* rays, int64_t q, const uint32_t* order,
+                        const int64_t* offsets, int32_t* indices, void* stream);
 
 /* Parity export: the canonical arrays of a finished build, for bit-exact comparison.
  * sorted_codes: uint32[n] when morton_bits = 30, uint64[n] when 63.  perm: uint32[n], original

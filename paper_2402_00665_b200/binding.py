@@ -46,6 +46,9 @@ SYMBOLS = {
     "bvh_scan_counts": [_P, c_int64, _P, _P, c_size_t, _P],
     "bvh_query_spheres_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
     "bvh_query_boxes_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
+    "bvh_query_order_rays": [_P, c_int64, _P, c_int64, _P, _P, c_size_t, _P],
+    "bvh_query_rays_count": [_P, c_int64, _P, c_int64, _P, _P, _P],
+    "bvh_query_rays_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
     "bvh_export": [_P, _P, c_int64, c_int, _P, _P, _P, _P, _P, _P, _P],
 }
 
@@ -156,6 +159,22 @@ def bvh_query_boxes_count(nodes, n: int, minmax, q: int, order, counts) -> None:
            "bvh_query_boxes_count")
 
 
+def bvh_query_order_rays(nodes, n: int, rays, q: int, order, scratch) -> None:
+    _check(load_library().bvh_query_order_rays(_ptr(nodes), n, _ptr(rays), q, _ptr(order), _ptr(scratch),
+                                               scratch.numel() * scratch.element_size(), _stream()),
+           "bvh_query_order_rays")
+
+
+def bvh_query_rays_count(nodes, n: int, rays, q: int, order, counts) -> None:
+    _check(load_library().bvh_query_rays_count(_ptr(nodes), n, _ptr(rays), q, _ptr(order), _ptr(counts), _stream()),
+           "bvh_query_rays_count")
+
+
+def bvh_query_rays_fill(nodes, n: int, rays, q: int, order, offsets, indices) -> None:
+    _check(load_library().bvh_query_rays_fill(_ptr(nodes), n, _ptr(rays), q, _ptr(order), _ptr(offsets),
+                                              _ptr(indices), _stream()), "bvh_query_rays_fill")
+
+
 def bvh_scan_sizes(q: int) -> int:
     sb = c_size_t()
     _check(load_library().bvh_scan_sizes(q, ctypes.byref(sb)), "bvh_scan_sizes")
@@ -237,22 +256,24 @@ class QueryWorkspace:
 
 def query(bvh: Bvh, queries: torch.Tensor, ws: QueryWorkspace | None = None, indices: torch.Tensor | None = None,
           ordered: bool = True):
-    """Range search.  queries: float32 CUDA [q,4] spheres {x,y,z,r} or [q,6] boxes {min,max}.
+    """Range search.  queries: float32 CUDA [q,4] spheres {x,y,z,r}, [q,6] boxes {min,max} or [q,8] rays
+    {origin, direction, tmin, tmax}.
 
     order (Morton schedule of the queries) -> count -> scan -> fill.  Returns (offsets int64[q+1], indices
     int32[nnz]) on the device.  Reads nnz back once (the path's only device->host sync) unless ``indices`` is
     passed in with enough room."""
-    if queries.dtype != torch.float32 or queries.dim() != 2 or queries.shape[1] not in (4, 6):
-        raise BvhError(f"expected float32 [q,4] or [q,6], got {queries.dtype} {tuple(queries.shape)}")
+    if queries.dtype != torch.float32 or queries.dim() != 2 or queries.shape[1] not in (4, 6, 8):
+        raise BvhError(f"expected float32 [q,4], [q,6] or [q,8], got {queries.dtype} {tuple(queries.shape)}")
     q = int(queries.shape[0])
     ws = ws or QueryWorkspace(q, queries.device)
-    spheres = queries.shape[1] == 4
-    count = bvh_query_spheres_count if spheres else bvh_query_boxes_count
-    fill = bvh_query_spheres_fill if spheres else bvh_query_boxes_fill
+    order_fn, count, fill = {
+        4: (bvh_query_order_spheres, bvh_query_spheres_count, bvh_query_spheres_fill),
+        6: (bvh_query_order_boxes, bvh_query_boxes_count, bvh_query_boxes_fill),
+        8: (bvh_query_order_rays, bvh_query_rays_count, bvh_query_rays_fill),
+    }[int(queries.shape[1])]
     order = None
     if ordered and q > 0:
-        (bvh_query_order_spheres if spheres else bvh_query_order_boxes)(bvh.nodes, bvh.n, queries, q, ws.order,
-                                                                        ws.order_scratch)
+        order_fn(bvh.nodes, bvh.n, queries, q, ws.order, ws.order_scratch)
         order = ws.order
     count(bvh.nodes, bvh.n, queries, q, order, ws.counts)
     bvh_scan_counts(ws.counts, q, ws.offsets, ws.scan_scratch)

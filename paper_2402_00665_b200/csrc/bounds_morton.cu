@@ -150,7 +150,8 @@ __device__ __forceinline__ uint32_t quantise(float lo, float hi, float slo, floa
   return min(q, cell_max);
 }
 
-// PRIM_FLOATS: 3 = points, 6 = boxes {min,max}, 4 = sphere queries {x,y,z,r} (centre only; used to order queries).
+// PRIM_FLOATS: 3 = points, 6 = boxes {min,max}, 4 = sphere queries {x,y,z,r} (centre only; used to order queries),
+// 8 = ray queries {o.xyz, d.xyz, tmin, tmax} (origin only; used to order queries).
 // FROM_ROOT: the frame is the root box of a finished hierarchy (kept in its NodesHeader) instead of the build header.
 template <typename KeyT, int PASSES, int PRIM_FLOATS, bool FROM_ROOT>
 __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __restrict__ prim, int n,
@@ -181,8 +182,8 @@ __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __r
       const float2* p = reinterpret_cast<const float2*>(prim + 6 * i);
       const float2 a = __ldcs(p), b = __ldcs(p + 1), c = __ldcs(p + 2);
       lo[0] = a.x; lo[1] = a.y; lo[2] = b.x; hi[0] = b.y; hi[1] = c.x; hi[2] = c.y;
-    } else if (PRIM_FLOATS == 4) {
-      const float4 v = __ldg(reinterpret_cast<const float4*>(prim) + i);
+    } else if (PRIM_FLOATS == 4 || PRIM_FLOATS == 8) {
+      const float4 v = __ldg(reinterpret_cast<const float4*>(prim) + (PRIM_FLOATS / 4) * i);
       lo[0] = hi[0] = v.x; lo[1] = hi[1] = v.y; lo[2] = hi[2] = v.z;
     } else {
       const float* p = prim + 3 * i;
@@ -243,6 +244,8 @@ void launch_query_morton(const float* queries, int q, int kind, const NodesHeade
   const unsigned g = morton_grid(q);
   if (kind == 0)
     launch_pdl(morton_kernel<uint32_t, 4, 4, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist);
+  else if (kind == 2)
+    launch_pdl(morton_kernel<uint32_t, 4, 8, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist);
   else
     launch_pdl(morton_kernel<uint32_t, 4, 6, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist);
 }

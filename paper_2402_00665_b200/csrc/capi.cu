@@ -262,6 +262,21 @@ int bvh_query_order_boxes(const void* nodes, int64_t n, const float* minmax, int
   return bvh::query_order(nodes, n, minmax, q, 1, order, scratch, scratch_bytes, stream);
 }
 
+int bvh_query_order_rays(const void* nodes, int64_t n, const float* rays, int64_t q, uint32_t* order, void* scratch,
+                         size_t scratch_bytes, void* stream) {
+  return bvh::query_order(nodes, n, rays, q, 2, order, scratch, scratch_bytes, stream);
+}
+
+int bvh_query_rays_count(const void* nodes, int64_t n, const float* rays, int64_t q, const uint32_t* order,
+                         int32_t* counts, void* stream) {
+  return bvh::query(nodes, n, rays, q, 2, false, order, counts, nullptr, nullptr, stream);
+}
+
+int bvh_query_rays_fill(const void* nodes, int64_t n, const float* rays, int64_t q, const uint32_t* order,
+                        const int64_t* offsets, int32_t* indices, void* stream) {
+  return bvh::query(nodes, n, rays, q, 2, true, order, nullptr, offsets, indices, stream);
+}
+
 int bvh_query_spheres_count(const void* nodes, int64_t n, const float* xyzr, int64_t q, const uint32_t* order,
                             int32_t* counts, void* stream) {
   return bvh::query(nodes, n, xyzr, q, 0, false, order, counts, nullptr, nullptr, stream);

@@ -163,7 +163,8 @@ void launch_hierarchy(const float* prim, bool is_box, const void* sorted_codes, 
 int hierarchy_levels(int n, int segs[kMaxHierLevels]);   // windows per level, level 1 first; returns the level count
 int hierarchy_total_segments(int n);
 int hierarchy_seg_capacity();
-// K6/K8: stackless traversal.  kind 0 = spheres (xyzr), 1 = boxes (minmax).  fill: offsets/indices used.
+// K6/K8: stackless traversal.  kind 0 = spheres (xyzr), 1 = boxes (minmax), 2 = rays (o.xyz, d.xyz, tmin, tmax).
+// fill: offsets/indices used.
 // order (optional): thread t serves query order[t] (results still land in row order[t]).
 void launch_traverse(const void* nodes, int n, const float* queries, int64_t q, int kind, bool fill,
                      const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* indices,

@@ -117,6 +117,64 @@ struct BoxQuery {
   }
 };
 
+// Ray {o.xyz, d.xyz, tmin, tmax} (NEXT-1; "a ray intersects"): D9 of DESIGN.md, the slab test.  Per axis
+// with d != 0: inv = 1 / d, t1 = (lo - o) * inv, t2 = (hi - o) * inv clip [tmin, tmax] to [min(t1,t2), max(t1,t2)];
+// per axis with d == 0: lo <= o <= hi.  Hit iff the clipped interval is not empty.  1 / d is computed once per ray
+// (the same IEEE division the oracle does per test); an axis with d == 0 keeps inv = 0 and is tested by bounds.
+struct RayQuery {
+  static constexpr int kWords = 8;
+  float o[3], inv[3], tmin, tmax;
+  uint32_t par;        // bit a: d[a] == 0
+  __device__ __forceinline__ void load(const float* __restrict__ q, int64_t j) {
+    const float4 a = __ldg(reinterpret_cast<const float4*>(q) + 2 * j);
+    const float4 b = __ldg(reinterpret_cast<const float4*>(q) + 2 * j + 1);
+    o[0] = a.x; o[1] = a.y; o[2] = a.z;
+    const float d[3] = {a.w, b.x, b.y};
+    tmin = b.z; tmax = b.w;
+    par = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      if (d[k] == 0.0f) {
+        par |= 1u << k;
+        inv[k] = 0.0f;
+      } else {
+        inv[k] = __fdiv_rn(1.0f, d[k]);
+      }
+    }
+  }
+  static constexpr int kSlotWords = 12;
+  __device__ __forceinline__ void to_shared(float* slot) const {
+    reinterpret_cast<float4*>(slot)[0] = make_float4(o[0], o[1], o[2], tmin);
+    reinterpret_cast<float4*>(slot)[1] = make_float4(inv[0], inv[1], inv[2], tmax);
+    reinterpret_cast<uint32_t*>(slot)[8] = par;
+  }
+  __device__ __forceinline__ void from_shared(const float* slot) {
+    const float4 a = reinterpret_cast<const float4*>(slot)[0];
+    const float4 b = reinterpret_cast<const float4*>(slot)[1];
+    o[0] = a.x; o[1] = a.y; o[2] = a.z; tmin = a.w;
+    inv[0] = b.x; inv[1] = b.y; inv[2] = b.z; tmax = b.w;
+    par = reinterpret_cast<const uint32_t*>(slot)[8];
+  }
+  __device__ __forceinline__ bool hit_box(float lox, float loy, float loz, float hix, float hiy, float hiz) const {
+    const float lo[3] = {lox, loy, loz}, hi[3] = {hix, hiy, hiz};
+    float tn = tmin, tf = tmax;
+    bool ok = true;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const float t1 = __fmul_rn(__fsub_rn(lo[k], o[k]), inv[k]);
+      const float t2 = __fmul_rn(__fsub_rn(hi[k], o[k]), inv[k]);
+      if ((par >> k) & 1u) {
+        ok = ok && (lo[k] <= o[k]) && (o[k] <= hi[k]);
+      } else {
+        tn = fmaxf(tn, fminf(t1, t2));
+        tf = fminf(tf, fmaxf(t1, t2));
+      }
+    }
+    return ok && (tn <= tf);
+  }
+  __device__ __forceinline__ bool hit_point(float x, float y, float z) const { return hit_box(x, y, z, x, y, z); }
+};
+
 // One leaf record: loaded first (so that several loads can be in flight), tested later.
 template <bool POINT_LEAF>
 struct LeafRec;
@@ -304,8 +362,10 @@ void launch_traverse(const void* nodes, int n, const float* queries, int64_t q, 
   const char* base = static_cast<const char*>(nodes);
   if (kind == 0)
     launch_traverse_kind<SphereQuery>(base, n, queries, q, fill, order, counts, offsets, indices, stream);
-  else
+  else if (kind == 1)
     launch_traverse_kind<BoxQuery>(base, n, queries, q, fill, order, counts, offsets, indices, stream);
+  else
+    launch_traverse_kind<RayQuery>(base, n, queries, q, fill, order, counts, offsets, indices, stream);
 }
 
 }  // namespace bvh

@@ -285,3 +285,55 @@ def test_merge_windows_multipass_reduced_capacity(B, oracle_lib, tmp_path):
             assert_build_equal(export_np(gpu_build(B, w.prims, w.morton_bits)), o, name)
     finally:
         B._lib, B.LIB_PATH = saved
+
+
+# ---- NEXT-1: ray queries (D9) ---------------------------------------------------------------------------------
+
+def _rays_through(prims, q, seed, tmax):
+    lo, hi = prims[:, :3].min(axis=0), prims[:, -3:].max(axis=0)
+    origins = W.uniform_cube(q, seed=seed) * (hi - lo) * np.float32(1.2) + lo - (hi - lo) * np.float32(0.1)
+    rays = W.rays_at(origins.astype(np.float32), W.sphere_surface(q, seed=seed + 1), 0.0, tmax)
+    rays[: q // 5, 3] = 0.0                        # parallel to the x slabs
+    rays[q // 5: q // 4, 4:6] = 0.0                # along the x axis
+    rays[q // 5: q // 4, 3] = -1.0
+    rays[q // 4: q // 3, 6] = np.float32(0.05)     # tmin > 0
+    return rays
+
+
+@pytest.mark.parametrize("name,n,q,half,tmax", [("C2", 60_001, 20_000, 0.004, 0.5), ("C4", 80_000, 20_000, 0.01, 3.0),
+                                               ("C3", 100_000, 8_000, 0.0005, 0.3)])
+def test_ray_queries_parity(B, oracle_lib, name, n, q, half, tmax):
+    """Ray predicate through the same Algorithm 1 kernel: CSR bit-equal to the oracle's stack traversal, raw order
+    included; box leaves (32-byte records)."""
+    w = W.make(name, n=n, q=0, radius=half if name == "C4" else None)
+    prims = w.prims if name == "C4" else W.boxes_around(w.prims, half)
+    rays = _rays_through(prims, q, seed=31, tmax=tmax)
+    if name == "C3":                               # clustered: start the rays inside the clusters
+        rays[:, :3] = w.prims[:q] + np.float32(0.0003)
+    o = oracle_lib.build_bvh(prims, w.morton_bits)
+    bvh = gpu_build(B, prims, w.morton_bits)
+    goff, gidx = gpu_query(B, bvh, rays)
+    ooff, oidx = oracle_lib.query_rays_tree(o, rays)
+    assert np.array_equal(goff, ooff) and ooff[-1] > q // 2
+    assert np.array_equal(gidx[: goff[-1]], oidx)
+
+
+def test_ray_queries_point_leaves_and_brute_force(B, oracle_lib):
+    """Point leaves (16-byte records): a ray hits a point only if it passes exactly through it, so the rays start AT
+    primitives and run along an axis or towards another primitive's coordinates; checked against brute force."""
+    pts = (W.uniform_cube(20_000, seed=12) * np.float32(64.0)).round().astype(np.float32) / np.float32(64.0)  # a lattice: many exact hits
+    q = 3000
+    d = np.zeros((q, 3), np.float32)
+    d[np.arange(q), np.arange(q) % 3] = np.float32(1.0)
+    d[::7] = np.float32([1.0, 1.0, 0.0])
+    d[::11] = np.float32([-2.0, 1.0, 0.5])
+    rays = W.rays_at(pts[:q], d, 0.0, 0.75)
+    bvh = gpu_build(B, pts, 63)
+    goff, gidx = gpu_query(B, bvh, rays)
+    boff, bidx = oracle_lib.query_rays_brute(pts, rays)
+    assert np.array_equal(goff, boff) and np.all(np.diff(goff) >= 1) and goff[-1] > 3 * q
+    assert np.array_equal(csr_rows_sorted(goff, gidx[: goff[-1]]), bidx)
+    # unordered = ordered
+    o2, i2 = B.query(bvh, _dev(rays), ordered=False)
+    torch.cuda.synchronize()
+    assert np.array_equal(o2.cpu().numpy(), goff) and np.array_equal(i2.cpu().numpy(), gidx[: goff[-1]])
