@@ -118,10 +118,10 @@ __device__ __forceinline__ void load_box_cg(const char* nodes, int n, int leaf_k
 #define BVH_MERGE_FAN 64
 #endif
 #ifndef BVH_MERGE_MAX_ITEMS
-#define BVH_MERGE_MAX_ITEMS 2048
+#define BVH_MERGE_MAX_ITEMS 1024
 #endif
 #ifndef BVH_MERGE_THREADS
-#define BVH_MERGE_THREADS 512
+#define BVH_MERGE_THREADS 1024
 #endif
 constexpr int kSegCap = 192;                       // >= 186 = 2 x 93 bits of augmented key
 constexpr int kMergeFan = BVH_MERGE_FAN;           // windows of the level below per merge window

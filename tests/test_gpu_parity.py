@@ -264,7 +264,7 @@ def test_deep_skewed_hierarchy(B, oracle_lib):
 
 def test_merge_windows_multipass_reduced_capacity(B, oracle_lib, tmp_path):
     """The upper windows of the bottom-up pass shorten an item list that does not fit their shared memory by passes
-    compacted in place.  With the product's capacity (2048 items per window) only degenerate inputs get there, so
+    compacted in place.  With the product's capacity (1024 items per window) few inputs get there, so
     this test compiles the same sources with the smallest legal capacity (384 items, 128 threads) and checks the
     result of that build bit for bit: 64 hand-overs of ~8 subtrees each overflow 384 on ordinary data."""
     import shutil
