@@ -35,7 +35,13 @@ constexpr uint32_t kValueMask = (1u << 30) - 1u;
 
 template <typename KeyT>
 struct SortCfg {
-  static constexpr int ITEMS = (sizeof(KeyT) == 4) ? 16 : 12;
+#ifndef BVH_SORT_ITEMS32
+#define BVH_SORT_ITEMS32 16
+#endif
+#ifndef BVH_SORT_ITEMS64
+#define BVH_SORT_ITEMS64 12
+#endif
+  static constexpr int ITEMS = (sizeof(KeyT) == 4) ? BVH_SORT_ITEMS32 : BVH_SORT_ITEMS64;
   static constexpr int TILE = kSortThreads * ITEMS;
 };
 
