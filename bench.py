@@ -41,7 +41,7 @@ NOMINAL_HBM_GBS = 8000.0   # the denominator BASELINE.json north_star names
 
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture for that kernel/workload exists).
-NCU_TRAFFIC_BYTES = {"fill": 4_345_000_000, "count": 363_380_000}   # profiles/r01c_ncu.md rows 17, 13 (DRAM rd + wr)
+NCU_TRAFFIC_BYTES = {"fill": 4_259_000_000, "count": 327_110_000}   # profiles/r01c_ncu.md rows 17, 13 (DRAM rd + wr)
 
 
 # ---- byte model (restated in DESIGN.md "Roofline") ---------------------------------------
