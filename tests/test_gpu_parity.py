@@ -337,3 +337,47 @@ def test_ray_queries_point_leaves_and_brute_force(B, oracle_lib):
     o2, i2 = B.query(bvh, _dev(rays), ordered=False)
     torch.cuda.synchronize()
     assert np.array_equal(o2.cpu().numpy(), goff) and np.array_equal(i2.cpu().numpy(), gidx[: goff[-1]])
+
+
+def test_cuda_graph_capture_and_replay(B):
+    """The C ABI only enqueues work (no allocation, no synchronisation, no host read): a whole build + ordered
+    count / scan / fill can be captured in a CUDA graph and replayed; the replay reproduces the eager result on the
+    captured inputs and follows the inputs when their contents change."""
+    w = W.make("C5", n=65_536 + 77, q=4096, radius=0.02)
+    d, dq = _dev(w.prims), _dev(w.queries)
+    bvh, ws = B.Bvh(w.n, w.morton_bits), B.QueryWorkspace(w.q)
+    bvh.nodes.zero_()
+    bvh.build(d)
+    off, idx = B.query(bvh, dq, ws)
+    torch.cuda.synchronize()
+    ref_nodes, ref_off, ref_idx = bvh.nodes.clone(), off.clone(), idx.clone()
+    indices = torch.empty(2 * idx.numel() + 16, dtype=torch.int32, device="cuda")
+    g, s = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        bvh.build(d)                                   # warm-up on the capture stream
+        B.query(bvh, dq, ws, indices=indices)
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g, stream=s):
+            bvh.build(d)
+            B.query(bvh, dq, ws, indices=indices)      # indices passed in: no nnz read-back inside the capture
+    for _ in range(3):
+        bvh.nodes.zero_(); indices.zero_(); ws.offsets.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(bvh.nodes, ref_nodes)
+        assert torch.equal(ws.offsets[: w.q + 1], ref_off) and torch.equal(indices[: ref_idx.numel()], ref_idx)
+    # new contents in the captured buffers: the replay builds and queries the new scene
+    w2 = W.make("C2", n=w.n, q=w.q, radius=0.02)
+    d.copy_(_dev(w2.prims)); dq.copy_(_dev(w2.queries))
+    g.replay()
+    torch.cuda.synchronize()
+    got_off, got_nodes = ws.offsets[: w.q + 1].clone(), bvh.nodes.clone()
+    nnz = int(got_off[-1])
+    got_idx = indices[:nnz].clone()
+    bvh2 = B.Bvh(w.n, w.morton_bits)
+    bvh2.nodes.zero_()
+    bvh2.build(d)
+    off2, idx2 = B.query(bvh2, dq)
+    torch.cuda.synchronize()
+    assert nnz <= indices.numel() and torch.equal(got_off, off2) and torch.equal(got_idx, idx2)
+    assert torch.equal(got_nodes, bvh2.nodes)
