@@ -359,6 +359,30 @@ def run_ours(args) -> dict | None:
                      "hits_per_ray": round(int(off_r[qr].item()) / qr, 3),
                      "what": "order + count + scan + fill of segments through the scene box, random directions"}
 
+    # ---- NEXT-2: the construction the paper compares itself with (Karras top-down + Algorithm 2 + separate box pass),
+    # same bounds / Morton / sort, same output bytes: how much the single bottom-up pass saves on this GPU
+    variant_info = None
+    if rank == 0 and not args.no_variant:
+        vscratch = torch.empty(binding.bvh_variant_sizes(n, bits, 1), dtype=torch.uint8, device=device)
+        vnodes = torch.empty_like(bvh.nodes)
+        vt = []
+        for _ in range(6):
+            flush.fill_(1)
+            v0 = ev()
+            binding.bvh_build_variant(d_prims, is_box, n, bits, vnodes, vscratch, 1)
+            v1 = ev()
+            torch.cuda.synchronize()
+            vt.append(v0.elapsed_time(v1))
+        vms = float(np.median(vt[1:]))
+        common = sum(acc[k] for k in build_names if k != "hierarchy") / args.steps     # staged: everything but the last step
+        variant_info = {"variant": "karras_topdown + algorithm2 ropes + separate box pass", "build_ms": round(vms, 4),
+                        "alg4_build_ms": round(acc["_build"] / args.steps, 4),
+                        "last_step_ms_estimate": {"variant": round(vms - common, 4),
+                                                  "alg4": round(acc["_build"] / args.steps - common, 4)},
+                        "what": "whole build as one call, median of 5; the last step = build minus the staged times of "
+                                "memset, bounds, Morton and sort (rank 0)"}
+        del vscratch, vnodes
+
     # ---- reduce over ranks: time = max, units = sum -----------------------------------------------------------------
     keys = sorted(acc)
     mx, sm = reduce_max_sum([acc[k] for k in keys] + [e2e_b, e2e_q], [float(n), float(q), float(nnz)], world, device)
@@ -413,6 +437,8 @@ def run_ours(args) -> dict | None:
     }
     if rays_info:
         line["next1_rays"] = rays_info
+    if variant_info:
+        line["next2_variant"] = variant_info
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(w)
     return line
@@ -493,6 +519,7 @@ def main(argv=None):
     ap.add_argument("--n", type=int, default=0, help="override the primitive count (non-default: for quick checks)")
     ap.add_argument("--q", type=int, default=0, help="override the query count")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-variant", action="store_true", help="skip the NEXT-2 comparison build (Karras top-down)")
     args = ap.parse_args(argv)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     line = run_reference(args) if args.impl == "reference" else run_ours(args)

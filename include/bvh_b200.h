@@ -131,6 +131,18 @@ int bvh_query_rays_count(const void* nodes, int64_t n, const float* rays, int64_
 int bvh_query_rays_fill(const void* nodes, int64_t n, const float* rays, int64_t q, const uint32_t* order,
                         const int64_t* offsets, int32_t* indices, void* stream);
 
+/* NEXT-2: a MEASUREMENT variant of the build, not a product path.  variant = 1 replaces the last step
+ * (the single bottom-up pass of Algorithm 4) by what the paper compares itself with: Karras' top-down construction,
+ * one thread per internal node searching its range and split on the common-prefix length of the augmented keys
+ * (PAPER.md:99-101), skip-connections by Algorithm 2, and a separate bottom-up pass for the boxes
+ * with atomic arrival counters in global memory.  Bounds, Morton codes, sort and the layout of `nodes`
+ * are unchanged, and `nodes` comes out byte-identical to bvh_build_points / bvh_build_boxes.  scratch must hold
+ * bvh_variant_sizes bytes (the product's scratch plus parent / child / counter arrays).  stage_events as in
+ * bvh_build_staged (may be NULL); event [12] closes the replaced step.  bvh_variant_sizes is a host call. */
+int bvh_variant_sizes(int64_t n, int morton_bits, int variant, size_t* scratch_bytes);
+int bvh_build_variant(const float* prim, int prim_is_box, int64_t n, int morton_bits, void* nodes, void* scratch,
+                      size_t scratch_bytes, int variant, void* stream, void* const* stage_events);
+
 /* Parity export: the canonical arrays of a finished build, for bit-exact comparison.
  * sorted_codes: uint32[n] when morton_bits = 30, uint64[n] when 63.  perm: uint32[n], original
  * index at each Morton position.  left_child, rope: int32[2n-1].  aabb: float[2n-1][6]

@@ -49,6 +49,8 @@ SYMBOLS = {
     "bvh_query_order_rays": [_P, c_int64, _P, c_int64, _P, _P, c_size_t, _P],
     "bvh_query_rays_count": [_P, c_int64, _P, c_int64, _P, _P, _P],
     "bvh_query_rays_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
+    "bvh_variant_sizes": [c_int64, c_int, c_int, ctypes.POINTER(c_size_t)],
+    "bvh_build_variant": [_P, c_int, c_int64, c_int, _P, _P, c_size_t, c_int, _P, ctypes.POINTER(c_void_p)],
     "bvh_export": [_P, _P, c_int64, c_int, _P, _P, _P, _P, _P, _P, _P],
 }
 
@@ -173,6 +175,19 @@ def bvh_query_rays_count(nodes, n: int, rays, q: int, order, counts) -> None:
 def bvh_query_rays_fill(nodes, n: int, rays, q: int, order, offsets, indices) -> None:
     _check(load_library().bvh_query_rays_fill(_ptr(nodes), n, _ptr(rays), q, _ptr(order), _ptr(offsets),
                                               _ptr(indices), _stream()), "bvh_query_rays_fill")
+
+
+def bvh_variant_sizes(n: int, morton_bits: int, variant: int) -> int:
+    sb = c_size_t()
+    _check(load_library().bvh_variant_sizes(n, morton_bits, variant, ctypes.byref(sb)), "bvh_variant_sizes")
+    return sb.value
+
+
+def bvh_build_variant(prim, prim_is_box: int, n: int, morton_bits: int, nodes, scratch, variant: int) -> None:
+    """NEXT-2 measurement variant (1 = Karras top-down + Algorithm 2 + separate box pass); same `nodes` bytes."""
+    _check(load_library().bvh_build_variant(_ptr(prim), prim_is_box, n, morton_bits, _ptr(nodes), _ptr(scratch),
+                                            scratch.numel() * scratch.element_size(), variant, _stream(), None),
+           "bvh_build_variant")
 
 
 def bvh_scan_sizes(q: int) -> int:

@@ -125,7 +125,7 @@ static inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_
 static int check_launch() { return cudaGetLastError() == cudaSuccess ? BVH_OK : BVH_ERR_CUDA; }
 
 static int build(const float* prim, bool is_box, int64_t n, int morton_bits, void* nodes, void* scratch,
-                 size_t scratch_bytes, void* stream_, void* const* events = nullptr) {
+                 size_t scratch_bytes, void* stream_, void* const* events = nullptr, int variant = 0) {
   if (n < 0) return BVH_ERR_INVALID_ARGUMENT;
   if (morton_bits != 30 && morton_bits != 63) return BVH_ERR_MORTON_BITS;
   if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
@@ -134,7 +134,8 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   if (misaligned(prim) || misaligned(nodes) || misaligned(scratch)) return BVH_ERR_INVALID_ARGUMENT;
   if ((reinterpret_cast<uintptr_t>(nodes) & 31u) != 0) return BVH_ERR_INVALID_ARGUMENT;
   const ScratchLayout L = scratch_layout(n, morton_bits);
-  if (scratch_bytes < L.total) return BVH_ERR_SCRATCH;
+  if (variant != 0 && variant != 1) return BVH_ERR_INVALID_ARGUMENT;
+  if (scratch_bytes < L.total + (variant == 1 ? variant_extra_bytes(n) : 0)) return BVH_ERR_SCRATCH;
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   char* base = static_cast<char*>(scratch);
   Header* header = reinterpret_cast<Header*>(base + L.header);
@@ -151,6 +152,13 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   launch_morton(prim, (int)n, is_box, morton_bits, header, base + L.keys[0], hist, stream);
   mark(3);
   launch_sort(sort_buffers(scratch, L), L.key_bytes, L.passes, (int)n, stream, events ? events + 4 : nullptr);
+  if (variant == 1) {
+    if (launch_variant_karras(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
+                              nodes, (int)n, header, base + L.total, stream) != 0)
+      return BVH_ERR_CUDA;
+    mark(12);
+    return check_launch();
+  }
   launch_hierarchy(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
                    nodes, (int)n, header, reinterpret_cast<int2*>(base + L.seg_items), reinterpret_cast<int*>(base + L.seg_count),
                    reinterpret_cast<uint32_t*>(base + L.arrivals), stream);
@@ -243,6 +251,19 @@ int bvh_build_boxes(const float* minmax, int64_t n, int morton_bits, void* nodes
 int bvh_build_staged(const float* prim, int prim_is_box, int64_t n, int morton_bits, void* nodes, void* scratch,
                      size_t scratch_bytes, void* stream, void* const* stage_events) {
   return bvh::build(prim, prim_is_box != 0, n, morton_bits, nodes, scratch, scratch_bytes, stream, stage_events);
+}
+
+int bvh_variant_sizes(int64_t n, int morton_bits, int variant, size_t* scratch_bytes) {
+  if (n < 0 || !scratch_bytes || variant != 1) return BVH_ERR_INVALID_ARGUMENT;
+  if (morton_bits != 30 && morton_bits != 63) return BVH_ERR_MORTON_BITS;
+  if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
+  *scratch_bytes = bvh::scratch_layout(n, morton_bits).total + bvh::variant_extra_bytes(n);
+  return BVH_OK;
+}
+
+int bvh_build_variant(const float* prim, int prim_is_box, int64_t n, int morton_bits, void* nodes, void* scratch,
+                      size_t scratch_bytes, int variant, void* stream, void* const* stage_events) {
+  return bvh::build(prim, prim_is_box != 0, n, morton_bits, nodes, scratch, scratch_bytes, stream, stage_events, variant);
 }
 
 int bvh_query_order_sizes(int64_t q, size_t* scratch_bytes) {

@@ -163,6 +163,10 @@ void launch_hierarchy(const float* prim, bool is_box, const void* sorted_codes, 
 int hierarchy_levels(int n, int segs[kMaxHierLevels]);   // windows per level, level 1 first; returns the level count
 int hierarchy_total_segments(int n);
 int hierarchy_seg_capacity();
+// NEXT-2 measurement variant (variants.cu): Karras' top-down hierarchy + Algorithm 2 + a separate box pass.
+size_t variant_extra_bytes(int64_t n);
+int launch_variant_karras(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
+                          void* nodes, int n, const Header* header, void* extra, cudaStream_t stream);
 // K6/K8: stackless traversal.  kind 0 = spheres (xyzr), 1 = boxes (minmax), 2 = rays (o.xyz, d.xyz, tmin, tmax).
 // fill: offsets/indices used.
 // order (optional): thread t serves query order[t] (results still land in row order[t]).

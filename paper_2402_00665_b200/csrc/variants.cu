@@ -1,0 +1,215 @@
+// variants.cu -- NEXT-2: the construction the paper compares itself with, built to MEASURE the
+// paper's claim on B200, not as a product path.  The paper says the bottom-up merge is "a faster algorithm" than
+// Karras' per-node search and that Karras needs "a separate bottom-up pass for boxes"
+// (PAPER.md:93); it gives no number.  bvh_build_variant(variant = 1) replaces the last step of the build (K4+K5,
+// hierarchy.cu) by exactly that:
+//   1. karras_leaf_kernel      leaf records (permuted gather) and leaf skip-connections (Alg. 4 L5-8, same as K4);
+//   2. karras_topdown_kernel   one thread per internal node i: range by the direction / doubling / binary search on
+//                              the common-prefix length delta(i, j) of the augmented keys, split by binary search
+//                              (Karras 2012 as the paper restates it), children at the split
+//                              (gamma, gamma + 1), skip-connection by Algorithm 2 from the
+//                              node's own range, parent pointers of both children;
+//   3. karras_box_kernel       boxes bottom-up: every leaf walks up; at a parent the first child to arrive stops
+//                              (atomic counter in global memory), the second reads both children's boxes through
+//                              L2, writes the parent's record and carries on.
+// Bounds, Morton codes, sort, node layout and leaf format are the product's, so the resulting `nodes` buffer must be
+// byte-identical to the one Algorithm 4 produces (tests/test_gpu_parity.py::test_variant_karras_topdown).
+#include "../../include/bvh_b200.h"
+#include "common.cuh"
+
+namespace bvh {
+
+// Common-prefix length of the augmented keys (code, sorted position) i and j; -1 outside [0, n-1].
+template <typename KeyT>
+__device__ __forceinline__ int prefix_len(const KeyT* __restrict__ codes, int n, KeyT ci, int i, int j) {
+  if (j < 0 || j >= n) return -1;
+  const KeyT cj = codes[j];
+  if (sizeof(KeyT) == 4) {
+    const uint64_t x = ((uint64_t)(uint32_t)(ci ^ cj) << 32) | (uint32_t)(i ^ j);
+    return __clzll((long long)x);
+  } else {
+    const uint64_t x = (uint64_t)(ci ^ cj);
+    return x ? __clzll((long long)x) : 64 + __clz(i ^ j);
+  }
+}
+
+struct VariantScratch {
+  int32_t* parent;   // [2n-1] parent of every node of the unified index space
+  uint32_t* flags;   // [n-1]   children arrived at each internal node (zeroed)
+  int32_t* left;     // [n-1]   left child, by Karras index
+  int32_t* right;    // [n-1]   right child
+  int32_t* rope;     // [n-1]   skip-connection, by Karras index
+};
+static inline size_t align256(size_t x) { return (x + 255) / 256 * 256; }
+size_t variant_extra_bytes(int64_t n) {
+  const size_t nn = (size_t)(n > 0 ? n : 1);
+  return align256(4 * (2 * nn)) + 4 * align256(4 * nn);
+}
+static VariantScratch variant_scratch(char* base, int64_t n) {
+  const size_t nn = (size_t)(n > 0 ? n : 1);
+  VariantScratch v;
+  v.parent = reinterpret_cast<int32_t*>(base);
+  base += align256(4 * (2 * nn));
+  v.flags = reinterpret_cast<uint32_t*>(base);
+  base += align256(4 * nn);
+  v.left = reinterpret_cast<int32_t*>(base);
+  base += align256(4 * nn);
+  v.right = reinterpret_cast<int32_t*>(base);
+  base += align256(4 * nn);
+  v.rope = reinterpret_cast<int32_t*>(base);
+  return v;
+}
+
+template <typename KeyT, bool IS_BOX>
+__global__ void __launch_bounds__(256)
+karras_leaf_kernel(const float* __restrict__ prim, const KeyT* __restrict__ codes, const uint32_t* __restrict__ perm,
+                   char* nodes_base, int n, const Header* __restrict__ header) {
+  pdl_wait();
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) {
+    NodesHeader* h = reinterpret_cast<NodesHeader*>(nodes_base);
+    float sb[6];
+    load_scene_bounds(header, sb);
+    h->magic = kNodesMagic;
+    h->n = n;
+    h->leaf_kind = IS_BOX ? kLeafBoxes : kLeafPoints;
+    h->reserved = 0;
+    for (int a = 0; a < 3; ++a) {
+      h->scene_lo[a] = sb[a];
+      h->scene_hi[a] = sb[3 + a];
+    }
+  }
+  if (i >= n) return;
+  const uint32_t o = perm[i];
+  const KeyT ci = codes[i];
+  // leaf skip-connection (Algorithm 2 for a leaf): leaf i+1 if keys i, i+1 share a longer prefix than i+1, i+2
+  const bool rope_internal = (i != n - 1) && !(prefix_len(codes, n, ci, i, i + 1) > prefix_len(codes, n, codes[i + 1], i + 1, i + 2));
+  const uint32_t payload = o | (rope_internal ? kLeafRopeInternal : 0u);
+  char* leaves = nodes_base + leaf_offset_bytes(n);
+  if (IS_BOX) {
+    const float2* p = reinterpret_cast<const float2*>(prim + 6 * (size_t)o);
+    const float2 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
+    float4* rec = reinterpret_cast<float4*>(leaves + 32 * (size_t)i);
+    rec[0] = make_float4(a.x, a.y, b.x, __uint_as_float(payload));
+    rec[1] = make_float4(b.y, c.x, c.y, 0.0f);
+  } else {
+    const float* p = prim + 3 * (size_t)o;
+    reinterpret_cast<float4*>(leaves)[i] = make_float4(__ldg(p), __ldg(p + 1), __ldg(p + 2), __uint_as_float(payload));
+  }
+}
+
+template <typename KeyT>
+__global__ void __launch_bounds__(256)
+karras_topdown_kernel(const KeyT* __restrict__ codes, int n, VariantScratch v) {
+  pdl_wait();
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n - 1) return;
+  const int leaf_base = n - 1;
+  const KeyT ci = codes[i];
+  auto delta = [&](int j) { return prefix_len(codes, n, ci, i, j); };
+  // direction of the range and the prefix every key of the range shares beyond its neighbour on the other side
+  const int d = (delta(i + 1) - delta(i - 1)) < 0 ? -1 : 1;
+  const int dmin = delta(i - d);
+  int lmax = 2;
+  while (delta(i + lmax * d) > dmin) lmax <<= 1;            // upper bound of the range length
+  int l = 0;
+  for (int t = lmax >> 1; t >= 1; t >>= 1)
+    if (delta(i + (l + t) * d) > dmin) l += t;               // the other end, by binary search
+  const int j = i + l * d;
+  const int dnode = delta(j);
+  int s = 0;                                                 // split: the last key that shares more than dnode with key i
+  for (int t = (l + 1) >> 1;; t = (t + 1) >> 1) {
+    if (delta(i + (s + t) * d) > dnode) s += t;
+    if (t == 1) break;
+  }
+  const int gamma = i + s * d + min(d, 0);
+  const int first = min(i, j), last = max(i, j);
+  const int left = (first == gamma) ? leaf_base + gamma : gamma;          // children at gamma, gamma + 1
+  const int right = (last == gamma + 1) ? leaf_base + gamma + 1 : gamma + 1;
+  // Algorithm 2: the skip-connection is the node whose range starts at last + 1
+  int rope = kSentinel;
+  if (last != n - 1) {
+    const int r = last + 1;
+    const KeyT cr = codes[r];
+    rope = (prefix_len(codes, n, cr, r, r - 1) > prefix_len(codes, n, cr, r, r + 1)) ? leaf_base + r : r;
+  }
+  v.left[i] = left;
+  v.right[i] = right;
+  v.rope[i] = rope;
+  v.parent[left] = i;
+  v.parent[right] = i;
+  if (i == 0) v.parent[0] = kSentinel;
+}
+
+__device__ __forceinline__ void load_box_any(const char* nodes, int n, int leaf_kind, int idx, float lo[3], float hi[3]) {
+  const int leaf_base = n - 1;
+  if (idx >= leaf_base && leaf_kind == kLeafPoints) {
+    const float4 p = __ldcg(reinterpret_cast<const float4*>(nodes + leaf_offset_bytes(n)) + (idx - leaf_base));
+    lo[0] = hi[0] = p.x; lo[1] = hi[1] = p.y; lo[2] = hi[2] = p.z;
+  } else {
+    const Node* rec = (idx >= leaf_base) ? reinterpret_cast<const Node*>(nodes + leaf_offset_bytes(n)) + (idx - leaf_base)
+                                         : reinterpret_cast<const Node*>(nodes + kNodesHeaderBytes) + idx;
+    const float4 a = __ldcg(reinterpret_cast<const float4*>(rec));
+    const float4 b = __ldcg(reinterpret_cast<const float4*>(rec) + 1);
+    lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; hi[0] = b.x; hi[1] = b.y; hi[2] = b.z;
+  }
+}
+
+// Boxes, bottom-up (the "separate bottom-up pass" of PAPER.md:93).
+__global__ void __launch_bounds__(256) karras_box_kernel(char* nodes_base, int n, int leaf_kind, VariantScratch v) {
+  pdl_wait();
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n || n < 2) return;
+  const int leaf_base = n - 1;
+  Node* internal = reinterpret_cast<Node*>(nodes_base + kNodesHeaderBytes);
+  int node = leaf_base + i;
+  while (true) {
+    const int p = v.parent[node];
+    if (p < 0) return;                                       // the root is done
+    __threadfence();                                         // this child's record before its arrival
+    if (atomicAdd(&v.flags[p], 1u) == 0u) return;            // first child to arrive stops
+    __threadfence();
+    const int left = v.left[p], rc = v.right[p];
+    float lo[3], hi[3], lo2[3], hi2[3];
+    load_box_any(nodes_base, n, leaf_kind, left, lo, hi);
+    load_box_any(nodes_base, n, leaf_kind, rc, lo2, hi2);
+    for (int a = 0; a < 3; ++a) {
+      lo[a] = fminf(lo[a], lo2[a]);
+      hi[a] = fmaxf(hi[a], hi2[a]);
+    }
+    Node rec;
+    rec.lo = make_float4(lo[0], lo[1], lo[2], __int_as_float(left));
+    rec.hi = make_float4(hi[0], hi[1], hi[2], __int_as_float(v.rope[p]));
+    internal[p] = rec;
+    node = p;
+  }
+}
+
+template <typename KeyT>
+static void launch_variant_keys(const float* prim, bool is_box, const KeyT* codes, const uint32_t* perm, char* nodes, int n,
+                                const Header* header, VariantScratch v, cudaStream_t stream) {
+  const unsigned gl = (unsigned)((n + 255) / 256);
+  if (is_box)
+    launch_pdl(karras_leaf_kernel<KeyT, true>, dim3(gl), dim3(256), 0, stream, prim, codes, perm, nodes, n, header);
+  else
+    launch_pdl(karras_leaf_kernel<KeyT, false>, dim3(gl), dim3(256), 0, stream, prim, codes, perm, nodes, n, header);
+  if (n < 2) return;
+  launch_pdl(karras_topdown_kernel<KeyT>, dim3((unsigned)((n - 1 + 255) / 256)), dim3(256), 0, stream, codes, n, v);
+  launch_pdl(karras_box_kernel, dim3(gl), dim3(256), 0, stream, nodes, n, is_box ? kLeafBoxes : kLeafPoints, v);
+}
+
+// The last step of the build, Karras-style.  extra: variant_extra_bytes(n) of scratch after the product's layout.
+int launch_variant_karras(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
+                          void* nodes, int n, const Header* header, void* extra, cudaStream_t stream) {
+  VariantScratch v = variant_scratch(static_cast<char*>(extra), n);
+  if (n >= 2 && cudaMemsetAsync(v.flags, 0, sizeof(uint32_t) * (size_t)(n - 1), stream) != cudaSuccess) return -1;
+  if (key_bytes == 4)
+    launch_variant_keys<uint32_t>(prim, is_box, static_cast<const uint32_t*>(sorted_codes), perm, static_cast<char*>(nodes), n,
+                                  header, v, stream);
+  else
+    launch_variant_keys<uint64_t>(prim, is_box, static_cast<const uint64_t*>(sorted_codes), perm, static_cast<char*>(nodes), n,
+                                  header, v, stream);
+  return 0;
+}
+
+}  // namespace bvh

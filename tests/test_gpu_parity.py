@@ -381,3 +381,28 @@ def test_cuda_graph_capture_and_replay(B):
     torch.cuda.synchronize()
     assert nnz <= indices.numel() and torch.equal(got_off, off2) and torch.equal(got_idx, idx2)
     assert torch.equal(got_nodes, bvh2.nodes)
+
+
+@pytest.mark.parametrize("name,n", [("C1", 4096), ("C2", 100_001), ("C3", 300_000), ("C4", 120_000), ("C5", 70_000)])
+def test_variant_karras_topdown(B, oracle_lib, name, n):
+    """NEXT-2: Karras' top-down construction + Algorithm 2 + a separate box pass gives the same bytes as the single
+    bottom-up pass ("identical hierarchy structure"), and both equal the oracle."""
+    w = W.make(name, n=n, q=0)
+    is_box = int(w.prims.shape[1] == 6)
+    a = B.Bvh(w.n, w.morton_bits)
+    a.nodes.zero_()
+    a.build(_dev(w.prims))
+    v = B.Bvh(w.n, w.morton_bits)
+    v.scratch = torch.empty(B.bvh_variant_sizes(w.n, w.morton_bits, 1), dtype=torch.uint8, device="cuda")
+    v.nodes.zero_()
+    B.bvh_build_variant(_dev(w.prims), is_box, w.n, w.morton_bits, v.nodes, v.scratch, 1)
+    torch.cuda.synchronize()
+    assert torch.equal(a.nodes, v.nodes)
+    assert_build_equal(export_np(v), oracle_lib.build_bvh(w.prims, w.morton_bits), name)
+    for tiny in (1, 2, 3, 5):
+        pts = W.uniform_cube(tiny, seed=tiny)
+        t = B.Bvh(tiny, 63)
+        t.scratch = torch.empty(B.bvh_variant_sizes(tiny, 63, 1), dtype=torch.uint8, device="cuda")
+        B.bvh_build_variant(_dev(pts), 0, tiny, 63, t.nodes, t.scratch, 1)
+        torch.cuda.synchronize()
+        assert_build_equal(export_np(t), oracle_lib.build_bvh(pts, 63), f"tiny {tiny}")
