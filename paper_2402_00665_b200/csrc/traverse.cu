@@ -62,6 +62,7 @@ __device__ __forceinline__ NodeRec load_rec(const Node* __restrict__ p) {
 
 struct SphereQuery {
   static constexpr int kWords = 4;
+  static constexpr int kCtasPerSm = kTravCtasPerSm;
   float cx, cy, cz, r2;
   __device__ __forceinline__ void load(const float* __restrict__ q, int64_t j) {
     const float4 v = __ldg(reinterpret_cast<const float4*>(q) + j);
@@ -93,6 +94,7 @@ struct SphereQuery {
 
 struct BoxQuery {
   static constexpr int kWords = 6;
+  static constexpr int kCtasPerSm = kTravCtasPerSm;
   float lo[3], hi[3];
   __device__ __forceinline__ void load(const float* __restrict__ q, int64_t j) {
     const float2* p = reinterpret_cast<const float2*>(q + 6 * j);
@@ -121,8 +123,12 @@ struct BoxQuery {
 // with d != 0: inv = 1 / d, t1 = (lo - o) * inv, t2 = (hi - o) * inv clip [tmin, tmax] to [min(t1,t2), max(t1,t2)];
 // per axis with d == 0: lo <= o <= hi.  Hit iff the clipped interval is not empty.  1 / d is computed once per ray
 // (the same IEEE division the oracle does per test); an axis with d == 0 keeps inv = 0 and is tested by bounds.
+#ifndef BVH_TRAV_CTAS_RAYS
+#define BVH_TRAV_CTAS_RAYS 6
+#endif
 struct RayQuery {
   static constexpr int kWords = 8;
+  static constexpr int kCtasPerSm = BVH_TRAV_CTAS_RAYS;   // the ray state does not fit the 64 registers of 8 CTAs per SM
   float o[3], inv[3], tmin, tmax;
   uint32_t par;        // bit a: d[a] == 0
   __device__ __forceinline__ void load(const float* __restrict__ q, int64_t j) {
@@ -328,7 +334,7 @@ __device__ __forceinline__ void traverse_body(const char* __restrict__ nodes, in
 // The leaf format (point or box records) is a property of the hierarchy, recorded in its header by the build;
 // the kernel reads it there (one uniform branch), so the query entry points need no extra argument.
 template <typename Query, bool FILL>
-__global__ void __launch_bounds__(kTravThreads, kTravCtasPerSm)
+__global__ void __launch_bounds__(kTravThreads, Query::kCtasPerSm)
 traverse_kernel(const char* __restrict__ nodes, int n, const float* __restrict__ queries, int64_t q,
                 const uint32_t* __restrict__ order, int32_t* __restrict__ counts, const int64_t* __restrict__ offsets,
                 int32_t* __restrict__ indices, int64_t num_chunks, int ctas_per_sm) {
@@ -343,9 +349,9 @@ static void launch_traverse_kind(const char* nodes, int n, const float* queries,
                                  const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* indices,
                                  cudaStream_t stream) {
   const int64_t num_chunks = (q + kTravThreads - 1) / kTravThreads;
-  // persistent grid: up to 148 x kTravCtasPerSm CTAs; fewer CTAs per SM when there is not enough work to fill them
+  // persistent grid: up to 148 x Query::kCtasPerSm CTAs; fewer CTAs per SM when there is not enough work to fill them
   int ctas_per_sm = (int)((num_chunks + kNumSMs - 1) / kNumSMs);
-  if (ctas_per_sm > kTravCtasPerSm) ctas_per_sm = kTravCtasPerSm;
+  if (ctas_per_sm > Query::kCtasPerSm) ctas_per_sm = Query::kCtasPerSm;
   if (ctas_per_sm < 1) ctas_per_sm = 1;
   const unsigned g = (unsigned)(kNumSMs * ctas_per_sm);
   if (fill)
