@@ -500,7 +500,8 @@ def run_reference(args) -> dict | None:
     return {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": round((tb + tq) / args.steps * 1e3, 3), "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "u64 Morton codes / f32 boxes", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None,
+        "dtype": "u32 Morton codes / f32 boxes" if w.morton_bits == 30 else "u64 Morton codes / f32 boxes", "data": "synthetic",
         "config": config_dict(args, w, world, {"sample": sample}),
         "query": {"mqueries_per_s": round(qs / (tq / args.steps) / 1e6, 4)},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
