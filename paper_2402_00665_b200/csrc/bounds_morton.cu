@@ -104,14 +104,14 @@ __global__ void __launch_bounds__(kBoundsThreads) scene_bounds_kernel(const floa
   }
 }
 
-void launch_scene_bounds(const float* prim, int n, bool is_box, Header* header, cudaStream_t stream) {
+cudaError_t launch_scene_bounds(const float* prim, int n, bool is_box, Header* header, cudaStream_t stream) {
   const int64_t nfloats = (int64_t)n * (is_box ? 6 : 3);
   const int64_t chunks = nfloats / (96 * 4);
   int64_t blocks = (chunks + (kBoundsThreads / 32) - 1) / (kBoundsThreads / 32);
   const int64_t cap = (int64_t)kNumSMs * 8;
   if (blocks > cap) blocks = cap;
   if (blocks < 1) blocks = 1;
-  launch_pdl(scene_bounds_kernel, dim3((unsigned)blocks), dim3(kBoundsThreads), 0, stream, prim, nfloats, is_box, header);
+  return launch_pdl(scene_bounds_kernel, dim3((unsigned)blocks), dim3(kBoundsThreads), 0, stream, prim, nfloats, is_box, header);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -223,31 +223,31 @@ static unsigned morton_grid(int n) {
   return (unsigned)blocks;
 }
 
-void launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
+cudaError_t launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
                    uint32_t* hist, cudaStream_t stream) {
   const unsigned g = morton_grid(n);
   if (morton_bits == 30) {
     if (is_box)
-      launch_pdl(morton_kernel<uint32_t, 4, 6, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint32_t*)codes, hist);
+      return launch_pdl(morton_kernel<uint32_t, 4, 6, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint32_t*)codes, hist);
     else
-      launch_pdl(morton_kernel<uint32_t, 4, 3, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint32_t*)codes, hist);
+      return launch_pdl(morton_kernel<uint32_t, 4, 3, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint32_t*)codes, hist);
   } else {
     if (is_box)
-      launch_pdl(morton_kernel<uint64_t, 8, 6, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint64_t*)codes, hist);
+      return launch_pdl(morton_kernel<uint64_t, 8, 6, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint64_t*)codes, hist);
     else
-      launch_pdl(morton_kernel<uint64_t, 8, 3, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint64_t*)codes, hist);
+      return launch_pdl(morton_kernel<uint64_t, 8, 3, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint64_t*)codes, hist);
   }
 }
 
-void launch_query_morton(const float* queries, int q, int kind, const NodesHeader* root, uint32_t* codes, uint32_t* hist,
+cudaError_t launch_query_morton(const float* queries, int q, int kind, const NodesHeader* root, uint32_t* codes, uint32_t* hist,
                          cudaStream_t stream) {
   const unsigned g = morton_grid(q);
   if (kind == 0)
-    launch_pdl(morton_kernel<uint32_t, 4, 4, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist);
+    return launch_pdl(morton_kernel<uint32_t, 4, 4, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist);
   else if (kind == 2)
-    launch_pdl(morton_kernel<uint32_t, 4, 8, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist);
+    return launch_pdl(morton_kernel<uint32_t, 4, 8, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist);
   else
-    launch_pdl(morton_kernel<uint32_t, 4, 6, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist);
+    return launch_pdl(morton_kernel<uint32_t, 4, 6, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist);
 }
 
 }  // namespace bvh

@@ -147,11 +147,12 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   mark(0);
   if (cudaMemsetAsync(base, 0, L.zero_bytes, stream) != cudaSuccess) return BVH_ERR_CUDA;
   mark(1);
-  launch_scene_bounds(prim, (int)n, is_box, header, stream);
+  if (launch_scene_bounds(prim, (int)n, is_box, header, stream) != cudaSuccess) return BVH_ERR_CUDA;
   mark(2);
-  launch_morton(prim, (int)n, is_box, morton_bits, header, base + L.keys[0], hist, stream);
+  if (launch_morton(prim, (int)n, is_box, morton_bits, header, base + L.keys[0], hist, stream) != cudaSuccess) return BVH_ERR_CUDA;
   mark(3);
-  launch_sort(sort_buffers(scratch, L), L.key_bytes, L.passes, (int)n, stream, events ? events + 4 : nullptr);
+  if (launch_sort(sort_buffers(scratch, L), L.key_bytes, L.passes, (int)n, stream, events ? events + 4 : nullptr) != cudaSuccess)
+    return BVH_ERR_CUDA;
   if (variant == 1) {
     if (launch_variant_karras(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
                               nodes, (int)n, header, base + L.total, stream) != 0)
@@ -159,9 +160,10 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
     mark(12);
     return check_launch();
   }
-  launch_hierarchy(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
-                   nodes, (int)n, header, reinterpret_cast<int2*>(base + L.seg_items), reinterpret_cast<int*>(base + L.seg_count),
-                   reinterpret_cast<uint32_t*>(base + L.arrivals), stream);
+  if (launch_hierarchy(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
+                       nodes, (int)n, header, reinterpret_cast<int2*>(base + L.seg_items), reinterpret_cast<int*>(base + L.seg_count),
+                       reinterpret_cast<uint32_t*>(base + L.arrivals), stream) != cudaSuccess)
+    return BVH_ERR_CUDA;
   mark(12);
   return check_launch();
 }
@@ -215,10 +217,11 @@ static int query_order(const void* nodes, int64_t n, const float* queries, int64
   char* base = static_cast<char*>(scratch);
   if (cudaMemsetAsync(base, 0, L.zero_bytes, stream) != cudaSuccess) return BVH_ERR_CUDA;
   SortBuffers B = sort_buffers(scratch, L);
-  launch_query_morton(queries, (int)q, kind, static_cast<const NodesHeader*>(nodes), static_cast<uint32_t*>(B.keys[0]),
-                      B.hist, stream);
+  if (launch_query_morton(queries, (int)q, kind, static_cast<const NodesHeader*>(nodes), static_cast<uint32_t*>(B.keys[0]),
+                          B.hist, stream) != cudaSuccess)
+    return BVH_ERR_CUDA;
   B.final_vals = order;
-  launch_sort(B, 4, 4, (int)q, stream, nullptr);
+  if (launch_sort(B, 4, 4, (int)q, stream, nullptr) != cudaSuccess) return BVH_ERR_CUDA;
   return check_launch();
 }
 

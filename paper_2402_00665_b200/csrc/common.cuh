@@ -117,7 +117,7 @@ __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.lau
 __device__ __forceinline__ void pdl_trigger() {}
 #endif
 template <typename... KArgs, typename... Args>
-inline void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args&&... args) {
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args&&... args) {
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = grid;
   cfg.blockDim = block;
@@ -128,14 +128,15 @@ inline void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
-// ---- kernel launchers (each only enqueues on `stream`) -----------------------------------------------
+// ---- kernel launchers (each only enqueues on `stream` and returns the first launch error; a caller stops
+// enqueueing at the first failure) ---------------------------------------------------------------------------
 // K1: scene bounds.  is_box: prim is n*6 floats, else n*3.
-void launch_scene_bounds(const float* prim, int n, bool is_box, Header* header, cudaStream_t stream);
+cudaError_t launch_scene_bounds(const float* prim, int n, bool is_box, Header* header, cudaStream_t stream);
 // K2: Morton codes + the digit histograms of every sort pass.
-void launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
+cudaError_t launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
                    uint32_t* hist, cudaStream_t stream);
 // K3: one-sweep LSD radix sort of (key, index) pairs, `passes` 8-bit digits from the least significant.
 // Pass p reads keys[p&1]/vals[p&1] and writes the other buffer; with an even pass count the result is in
@@ -151,13 +152,13 @@ struct SortBuffers {
   uint32_t* final_vals;
 };
 SortBuffers sort_buffers(void* scratch, const ScratchLayout& L);
-void launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStream_t stream, void* const* pass_events);
+cudaError_t launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStream_t stream, void* const* pass_events);
 // Morton codes (30-bit) of query centres in the frame of the root box + digit histograms: orders queries.
-void launch_query_morton(const float* queries, int q, int kind, const NodesHeader* frame, uint32_t* codes, uint32_t* hist,
+cudaError_t launch_query_morton(const float* queries, int q, int kind, const NodesHeader* frame, uint32_t* codes, uint32_t* hist,
                          cudaStream_t stream);
 // K4+K5: leaf gather + modified Apetrei bottom-up pass (Algorithm 4 with boxes).
 constexpr int kMaxHierLevels = 8;
-void launch_hierarchy(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
+cudaError_t launch_hierarchy(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
                       void* nodes, int n, const Header* header, int2* seg_items, int* seg_count, uint32_t* arrivals,
                       cudaStream_t stream);
 int hierarchy_levels(int n, int segs[kMaxHierLevels]);   // windows per level, level 1 first; returns the level count

@@ -32,16 +32,22 @@ struct Delta<uint32_t> {
   static constexpr T kInf = 0xFFFFFFFFu;
   __device__ static __forceinline__ T make(uint32_t a, uint32_t b, int i) {
     const uint32_t x = a ^ b;                              // < 2^30
-    return x ? (x + 0x40000000u) : (uint32_t)(i ^ (i + 1));  // positions < 2^30
+    return x ? (x + 0x40000000u) : (uint32_t)(i ^ (i + 1));  // codes and positions < 2^30 (capi.cu rejects n >= 2^30)
   }
 };
+// 64-bit codes: the value kept is the INDEX of the highest differing bit, not the XOR itself.  Every comparison
+// Algorithm 4 makes is between delta*(l-1) and delta*(r) of a node's range [l, r], or between delta*(r) and
+// delta*(r+1) (L8, L26); in both cases the two XORs cannot share their highest set bit (sorted keys: a key cannot
+// have that bit both set, as the upper key of one pair, and clear, as the lower key of the other, under the
+// same prefix), so the order of the XORs is the order of their highest bits -- Karras' common-prefix length
+// (PAPER.md:97).  One 32-bit word instead of two: half the shuffles and shared memory of the 63-bit build.
 template <>
 struct Delta<uint64_t> {
-  using T = uint64_t;
-  static constexpr T kInf = 0xFFFFFFFFFFFFFFFFull;
+  using T = uint32_t;
+  static constexpr T kInf = 0xFFFFFFFFu;
   __device__ static __forceinline__ T make(uint64_t a, uint64_t b, int i) {
     const uint64_t x = a ^ b;                              // <= 2^63 - 1
-    return x ? (x + 0x7FFFFFFFFFFFFFFFull) : (uint64_t)(uint32_t)(i ^ (i + 1));
+    return x ? (0x40000000u + (uint32_t)(63 - __clzll((long long)x))) : (uint32_t)(i ^ (i + 1));
   }
 };
 
@@ -125,6 +131,8 @@ __device__ __forceinline__ void load_box_cg(const char* nodes, int n, int leaf_k
 #endif
 constexpr int kSegCap = 192;                       // >= 186 = 2 x 93 bits of augmented key
 constexpr int kMergeFan = BVH_MERGE_FAN;           // windows of the level below per merge window
+constexpr int kMergeFanMax = 128;                  // what the prefix / search code of merge_window is written for
+static_assert(kMergeFan >= 2 && kMergeFan <= kMergeFanMax, "merge_window handles up to kMergeFanMax child windows");
 constexpr int kMergeMaxItems = BVH_MERGE_MAX_ITEMS;  // items a merge window holds in shared memory at once
 static_assert(kMergeMaxItems >= 2 * kSegCap, "a pass over windows of kMergeMaxItems items must shrink the list");
 constexpr int kMergeThreads = BVH_MERGE_THREADS;
@@ -153,9 +161,11 @@ struct DeltaByItem {
 // Shared-memory state of M items in leaf order.  Item e lives in slot map.slot(e) of the arrays (level 1 leaves the
 // items where its warps staged them; the higher levels store them densely).  A subtree made of items [a, b] is
 // carried by one thread and keeps its box in the slot of item a.
+template <typename RT>
 struct ItemArrays {
-  int* l;        // first leaf of the item in this slot
-  int* r;        // last leaf
+  RT* l;         // first leaf of the item in this slot, minus `base` (level 1: offsets into the window, 16 bits)
+  RT* r;         // last leaf, minus `base`
+  int base;
   float* box;    // box[c * stride + slot], c = 0..5 (min.xyz, max.xyz)
   int stride;
   int* store;    // Algorithm 4's `store`, one entry per boundary (e | e+1), by item index: -1 empty, >= 0 first arrival, -2 both
@@ -178,14 +188,14 @@ struct ClimbEnd {
 };
 
 // Algorithm 4, L9-28, for the subtree that starts as item e, on shared memory.
-template <typename D, typename DeltaSrc, typename Slots>
-__device__ __forceinline__ ClimbEnd climb_from_item(int e, int M, const ItemArrays& A, const DeltaSrc& ds, const Slots& map,
+template <typename D, typename RT, typename DeltaSrc, typename Slots>
+__device__ __forceinline__ ClimbEnd climb_from_item(int e, int M, const ItemArrays<RT>& A, const DeltaSrc& ds, const Slots& map,
                                                     Node* nodes, int n) {
   const int leaf_base = n - 1;
   int a = e, b = e;                                                   // items covered
   const int se = map.slot(e);
   int sa = se;                                                        // slot of item a: where this subtree's box lives
-  int range_left = A.l[se], range_right = A.r[se];                    // L3 (leaves covered)
+  int range_left = A.base + (int)A.l[se], range_right = A.base + (int)A.r[se];   // L3 (leaves covered)
   D delta_left = ds.left(a, range_left), delta_right = ds.right(b, range_right);   // L4
   float lo[3], hi[3];
 #pragma unroll
@@ -209,13 +219,13 @@ __device__ __forceinline__ ClimbEnd climb_from_item(int e, int M, const ItemArra
       p = range_right;                                                // Apetrei index = split
       ssib = map.slot(b + 1);
       b = other;
-      range_right = A.r[map.slot(b)];
+      range_right = A.base + (int)A.r[map.slot(b)];
       delta_right = ds.right(b, range_right);                         // L14
     } else {
       p = range_left - 1;
       a = other;
       sa = ssib = map.slot(a);
-      range_left = A.l[sa];
+      range_left = A.base + (int)A.l[sa];
       delta_left = ds.left(a, range_left);                            // L19
     }
     __threadfence_block();                                            // the sibling's box was written before its CAS
@@ -244,7 +254,8 @@ __device__ __forceinline__ ClimbEnd climb_from_item(int e, int M, const ItemArra
 }
 
 // After a barrier: is the subtree that stopped like this still without its sibling (a maximal subtree of the window)?
-__device__ __forceinline__ bool climb_survives(const ItemArrays& A, const ClimbEnd& c) {
+template <typename RT>
+__device__ __forceinline__ bool climb_survives(const ItemArrays<RT>& A, const ClimbEnd& c) {
   return c.fin == -1 || (c.fin >= 0 && A.store[c.fin] != -2);
 }
 
@@ -270,15 +281,17 @@ __device__ __forceinline__ int block_compact(bool flag, uint32_t* s_wsum, int nw
 template <typename D>
 struct LocalSmem {
   D delta[kHierWindow + 2];      // delta[k] = delta*(c0 - 1 + k)
-  int l[kHierWindow], r[kHierWindow], store[kHierWindow];
+  int store[kHierWindow];
   float box[6 * kHierWindow];
+  uint16_t l[kHierWindow], r[kHierWindow];   // offsets from the window's first leaf
 };
+static_assert(kHierWindow <= 65536, "level-1 item ranges are kept as 16-bit offsets");
 template <typename D>
 struct MergeSmem {
   D bd[kMergeMaxItems + 1], nd[kMergeMaxItems + 1];
   int l[kMergeMaxItems], r[kMergeMaxItems], store[kMergeMaxItems];
   float box[6 * kMergeMaxItems];
-  int pref[kMergeFan + 1];
+  int pref[kMergeFanMax + 1];
 };
 // Windows of every level (level 1 first) and where each level's hand-over segments and arrival counters start.
 struct HierLevels {
@@ -308,7 +321,7 @@ __device__ __forceinline__ void merge_window(MergeSmem<typename Delta<KeyT>::T>&
   const int seg0 = window * kMergeFan;
   const int nseg = min(kMergeFan, in_segs - seg0);
   if (tid < 32) {                                         // exclusive prefix of the segment counts, by one warp
-    constexpr int PER = (kMergeFan + 31) / 32;
+    constexpr int PER = kMergeFanMax / 32;
     int c[PER], sum = 0;
 #pragma unroll
     for (int u = 0; u < PER; ++u) {
@@ -326,16 +339,16 @@ __device__ __forceinline__ void merge_window(MergeSmem<typename Delta<KeyT>::T>&
 #pragma unroll
     for (int u = 0; u < PER; ++u) {
       const int sg = tid * PER + u;
-      if (sg < kMergeFan) S.pref[sg] = run;
+      S.pref[sg] = run;                                   // entries past nseg hold the total
       run += c[u];
     }
-    if (tid == 31) S.pref[kMergeFan] = incl;
+    if (tid == 31) S.pref[kMergeFanMax] = incl;
   }
   __syncthreads();
-  int count = S.pref[kMergeFan];
+  int count = S.pref[kMergeFanMax];
   int2* region = in_items + (size_t)seg0 * kSegCap;       // this window's input segments, contiguous
   bool flat = false;                                      // items compacted at the start of `region`
-  const ItemArrays A{S.l, S.r, S.box, MAXI, S.store};
+  const ItemArrays<int> A{S.l, S.r, 0, S.box, MAXI, S.store};
 
   while (true) {
     const bool last_pass = count <= MAXI;
@@ -356,8 +369,8 @@ __device__ __forceinline__ void merge_window(MergeSmem<typename Delta<KeyT>::T>&
           } else {
             int sg = 0;                                   // segment of item g: the last sg with pref[sg] <= g
 #pragma unroll
-            for (int step = 32; step > 0; step >>= 1)
-              if (step < kMergeFan && sg + step < kMergeFan && S.pref[sg + step] <= g) sg += step;
+            for (int step = kMergeFanMax / 2; step > 0; step >>= 1)
+              if (sg + step < nseg && S.pref[sg + step] <= g) sg += step;
             it[j] = __ldcg(region + (size_t)sg * kSegCap + (g - S.pref[sg]));
           }
         }
@@ -458,8 +471,8 @@ hierarchy_local_kernel(const float* __restrict__ prim, const KeyT* __restrict__ 
   __shared__ uint32_t s_wsum[NW + 1];
   __shared__ int s_wcount[NW];
   D* const s_delta = smem.delta;
-  int* const s_l = smem.l;
-  int* const s_r = smem.r;
+  uint16_t* const s_l = smem.l;
+  uint16_t* const s_r = smem.r;
   int* const s_store = smem.store;
   float* const s_box = smem.box;
 
@@ -607,8 +620,8 @@ hierarchy_local_kernel(const float* __restrict__ prim, const KeyT* __restrict__ 
     const uint32_t am = __ballot_sync(0xffffffffu, active);
     if (active) {
       const int slot = warp * PER_WARP + wcount + __popc(am & lt_mask);
-      s_l[slot] = range_left;
-      s_r[slot] = range_right;
+      s_l[slot] = (uint16_t)(range_left - c0);
+      s_r[slot] = (uint16_t)(range_right - c0);
 #pragma unroll
       for (int a = 0; a < 3; ++a) {
         s_box[a * W + slot] = lo[a];
@@ -631,7 +644,7 @@ hierarchy_local_kernel(const float* __restrict__ prim, const KeyT* __restrict__ 
   map.o2 = 2 * PER_WARP - map.b2;
   map.o3 = 3 * PER_WARP - map.b3;
   const int M = map.b3 + s_wcount[3];
-  const ItemArrays A{s_l, s_r, s_box, W, s_store};
+  const ItemArrays<uint16_t> A{s_l, s_r, c0, s_box, W, s_store};
   ClimbEnd end[G];
 #pragma unroll
   for (int j = 0; j < G; ++j) {
@@ -713,9 +726,9 @@ int hierarchy_total_segments(int n) {
 }
 
 template <typename KeyT>
-static void launch_hierarchy_keys(const float* prim, bool is_box, const KeyT* codes, const uint32_t* perm, char* nodes, int n,
-                                  const Header* header, int2* seg_items, int* seg_count, uint32_t* arrivals,
-                                  cudaStream_t stream) {
+static cudaError_t launch_hierarchy_keys(const float* prim, bool is_box, const KeyT* codes, const uint32_t* perm, char* nodes,
+                                         int n, const Header* header, int2* seg_items, int* seg_count, uint32_t* arrivals,
+                                         cudaStream_t stream) {
   HierLevels lv{};
   lv.levels = hierarchy_levels(n, lv.segs);
   int off = 0;
@@ -723,30 +736,32 @@ static void launch_hierarchy_keys(const float* prim, bool is_box, const KeyT* co
     lv.seg_off[l] = off;
     off += lv.segs[l];
   }
+  cudaError_t e;
   if (is_box)
-    launch_pdl(hierarchy_local_kernel<KeyT, true>, dim3(lv.segs[0]), dim3(kHierThreads), 0, stream, prim, codes, perm, nodes, n, header, seg_items,
-                                                                               seg_count);
+    e = launch_pdl(hierarchy_local_kernel<KeyT, true>, dim3(lv.segs[0]), dim3(kHierThreads), 0, stream, prim, codes, perm, nodes,
+                   n, header, seg_items, seg_count);
   else
-    launch_pdl(hierarchy_local_kernel<KeyT, false>, dim3(lv.segs[0]), dim3(kHierThreads), 0, stream, prim, codes, perm, nodes, n, header, seg_items,
-                                                                                seg_count);
-  if (lv.levels > 1) {
-    using D = typename Delta<KeyT>::T;
-    const size_t smem = sizeof(MergeSmem<D>);
-    cudaFuncSetAttribute(hierarchy_merge_kernel<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    launch_pdl(hierarchy_merge_kernel<KeyT>, dim3(lv.segs[1]), dim3(kMergeThreads), smem, stream, codes, nodes, n, is_box ? kLeafBoxes : kLeafPoints,
-                                                                             seg_items, seg_count, arrivals, lv);
-  }
+    e = launch_pdl(hierarchy_local_kernel<KeyT, false>, dim3(lv.segs[0]), dim3(kHierThreads), 0, stream, prim, codes, perm, nodes,
+                   n, header, seg_items, seg_count);
+  if (e != cudaSuccess || lv.levels <= 1) return e;
+  using D = typename Delta<KeyT>::T;
+  const size_t smem = sizeof(MergeSmem<D>);
+  // the opt-in to more than 48 KB of dynamic shared memory is a property of the function: set once per process
+  static const cudaError_t attr =
+      cudaFuncSetAttribute(hierarchy_merge_kernel<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (attr != cudaSuccess) return attr;
+  return launch_pdl(hierarchy_merge_kernel<KeyT>, dim3(lv.segs[1]), dim3(kMergeThreads), smem, stream, codes, nodes, n,
+                    is_box ? kLeafBoxes : kLeafPoints, seg_items, seg_count, arrivals, lv);
 }
 
-void launch_hierarchy(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
-                      void* nodes, int n, const Header* header, int2* seg_items, int* seg_count, uint32_t* arrivals,
-                      cudaStream_t stream) {
+cudaError_t launch_hierarchy(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
+                             void* nodes, int n, const Header* header, int2* seg_items, int* seg_count, uint32_t* arrivals,
+                             cudaStream_t stream) {
   if (key_bytes == 4)
-    launch_hierarchy_keys<uint32_t>(prim, is_box, static_cast<const uint32_t*>(sorted_codes), perm, static_cast<char*>(nodes), n,
-                                    header, seg_items, seg_count, arrivals, stream);
-  else
-    launch_hierarchy_keys<uint64_t>(prim, is_box, static_cast<const uint64_t*>(sorted_codes), perm, static_cast<char*>(nodes), n,
-                                    header, seg_items, seg_count, arrivals, stream);
+    return launch_hierarchy_keys<uint32_t>(prim, is_box, static_cast<const uint32_t*>(sorted_codes), perm,
+                                           static_cast<char*>(nodes), n, header, seg_items, seg_count, arrivals, stream);
+  return launch_hierarchy_keys<uint64_t>(prim, is_box, static_cast<const uint64_t*>(sorted_codes), perm,
+                                         static_cast<char*>(nodes), n, header, seg_items, seg_count, arrivals, stream);
 }
 
 int hierarchy_seg_capacity() { return kSegCap; }

@@ -328,28 +328,36 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_o
 }
 
 template <typename KeyT>
-static void sort_all(const SortBuffers& B, int n, int passes, cudaStream_t stream, void* const* pass_events) {
+static cudaError_t sort_all(const SortBuffers& B, int n, int passes, cudaStream_t stream, void* const* pass_events) {
   const int tiles = (n + SortCfg<KeyT>::TILE - 1) / SortCfg<KeyT>::TILE;
   KeyT* keys[2] = {static_cast<KeyT*>(B.keys[0]), static_cast<KeyT*>(B.keys[1])};
   const size_t smem = sizeof(SortSmem<KeyT>);
-  cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  // the opt-in to more than 48 KB of dynamic shared memory is a property of the function: set once per process
+  static const cudaError_t attr = [&]() {
+    cudaError_t e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    return e;
+  }();
+  if (attr != cudaSuccess) return attr;
   for (int p = 0; p < passes; ++p) {
     const int in = p & 1, out = in ^ 1;
     uint32_t* st = B.status + (size_t)p * tiles * 256;
     uint32_t* vout = (p == passes - 1 && B.final_vals) ? B.final_vals : B.vals[out];
+    cudaError_t e;
     if (p == 0)
-      launch_pdl(onesweep_pass_kernel<KeyT, true, false>, dim3(tiles), dim3(kSortThreads), smem, stream,
+      e = launch_pdl(onesweep_pass_kernel<KeyT, true, false>, dim3(tiles), dim3(kSortThreads), smem, stream,
                  keys[in], keys[out], nullptr, vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
     else if (p == passes - 1)
-      launch_pdl(onesweep_pass_kernel<KeyT, false, true>, dim3(tiles), dim3(kSortThreads), smem, stream,
+      e = launch_pdl(onesweep_pass_kernel<KeyT, false, true>, dim3(tiles), dim3(kSortThreads), smem, stream,
                  keys[in], keys[out], B.vals[in], vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
     else
-      launch_pdl(onesweep_pass_kernel<KeyT, false, false>, dim3(tiles), dim3(kSortThreads), smem, stream,
+      e = launch_pdl(onesweep_pass_kernel<KeyT, false, false>, dim3(tiles), dim3(kSortThreads), smem, stream,
                  keys[in], keys[out], B.vals[in], vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
+    if (e != cudaSuccess) return e;
     if (pass_events && pass_events[p]) cudaEventRecord(static_cast<cudaEvent_t>(pass_events[p]), stream);
   }
+  return cudaSuccess;
 }
 
 SortBuffers sort_buffers(void* scratch, const ScratchLayout& L) {
@@ -366,11 +374,9 @@ SortBuffers sort_buffers(void* scratch, const ScratchLayout& L) {
   return B;
 }
 
-void launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStream_t stream, void* const* pass_events) {
-  if (key_bytes == 4)
-    sort_all<uint32_t>(B, n, passes, stream, pass_events);
-  else
-    sort_all<uint64_t>(B, n, passes, stream, pass_events);
+cudaError_t launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStream_t stream, void* const* pass_events) {
+  if (key_bytes == 4) return sort_all<uint32_t>(B, n, passes, stream, pass_events);
+  return sort_all<uint64_t>(B, n, passes, stream, pass_events);
 }
 
 }  // namespace bvh
