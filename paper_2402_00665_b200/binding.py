@@ -17,8 +17,7 @@ from ctypes import c_int, c_int64, c_size_t, c_void_p
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# BVH_B200_LIB selects another build of the same library (tuning sweeps); the default is the in-tree product.
-LIB_PATH = os.environ.get("BVH_B200_LIB") or os.path.join(_HERE, "libbvh_b200.so")
+LIB_PATH = os.path.join(_HERE, "libbvh_b200.so")
 
 BVH_OK = 0
 ERRORS = {
