@@ -6,8 +6,9 @@
  * readings and definitions listed in DESIGN.md where the paper is silent or garbled.
  *
  * Conventions for EVERY entry point
- *  - All data pointers are DEVICE pointers (cudaMalloc / torch CUDA memory), 16-byte aligned, owned
- *    by the caller.  The only host pointers are the `size_t*` outputs of the *_sizes functions.
+ *  - All data pointers are DEVICE pointers (cudaMalloc / torch CUDA memory), 16-byte aligned (`nodes`
+ *    and the `rows` of bvh_query_collect: 32-byte aligned), owned by the caller.  The only host
+ *    pointers are the `size_t*` outputs of the *_sizes functions.
  *  - The library never allocates, frees or synchronises; it holds no global state and is re-entrant
  *    across streams.  Every call only enqueues work on `stream` (a cudaStream_t passed as void*;
  *    NULL = the legacy default stream) and returns.
@@ -95,7 +96,10 @@ int bvh_query_order_boxes(const void* nodes, int64_t n, const float* minmax, int
  * Sphere query {x,y,z,r}: squared distance from the centre to the box <= r*r, fp32 round-to-nearest,
  * association of D8.  Box query {min.xyz,max.xyz}: closed-interval overlap on every axis (G12).
  * order: NULL (thread t serves query t) or a permutation of [0,q) from bvh_query_order_*.
- * q = 0 or n = 0: counts (if q > 0) are set to 0. */
+ * q = 0 or n = 0: counts (if q > 0) are set to 0.  `nodes` must hold a finished build over exactly n
+ * primitives; the library cannot synchronise to check that on the host, so the query kernels check the
+ * header the build wrote (magic, n) on the device: a buffer that fails the check yields counts of 0 and no
+ * stores instead of a walk over garbage indices. */
 int bvh_query_spheres_count(const void* nodes, int64_t n, const float* xyzr, int64_t q, const uint32_t* order,
                             int32_t* counts, void* stream);
 int bvh_query_boxes_count(const void* nodes, int64_t n, const float* minmax, int64_t q, const uint32_t* order,
@@ -115,6 +119,27 @@ int bvh_query_spheres_fill(const void* nodes, int64_t n, const float* xyzr, int6
                            const int64_t* offsets, int32_t* indices, void* stream);
 int bvh_query_boxes_fill(const void* nodes, int64_t n, const float* minmax, int64_t q, const uint32_t* order,
                          const int64_t* offsets, int32_t* indices, void* stream);
+
+/* Single-pass variant of count-then-fill (Alg. 1 L5 "Store the result";
+ * the traversal is the expensive, divergent part, so it should run once).  The caller guesses a row
+ * capacity `cap` (entries per query: from an estimate, or from the counts of the previous batch) and provides
+ * rows = int32[q * cap], 32-byte aligned; cap is a multiple of 8, >= 8.
+ *   bvh_query_collect        ONE traversal: counts[j] = number of hits of query j (exact, whatever cap is), and the
+ *                            first min(counts[j], cap) hits of query j, in traversal order, in rows[j*cap ...).
+ *                            query_kind: 0 spheres {x,y,z,r}, 1 boxes {min,max}, 2 rays (8 floats); predicates,
+ *                            `order` and the n = 0 / q = 0 behaviour as in the count calls.
+ *   bvh_scan_counts          (as before) counts -> offsets; the caller reads offsets[q] to size `indices`.
+ *   bvh_rows_to_csr          copies every row that fitted (counts[j] <= cap) to indices[offsets[j] ...).
+ *   bvh_query_fill_overflow  the fill traversal for the rows that did not fit (counts[j] > cap) only; a no-op walk
+ *                            when there are none.
+ * After the three calls `offsets` / `indices` are byte-identical to what count -> scan -> fill produce. */
+int bvh_query_collect(const void* nodes, int64_t n, const float* queries, int query_kind, int64_t q,
+                      const uint32_t* order, int64_t cap, int32_t* rows, int32_t* counts, void* stream);
+int bvh_rows_to_csr(const int32_t* rows, int64_t cap, const int32_t* counts, const int64_t* offsets, int64_t q,
+                    int32_t* indices, void* stream);
+int bvh_query_fill_overflow(const void* nodes, int64_t n, const float* queries, int query_kind, int64_t q,
+                            const uint32_t* order, int64_t cap, const int32_t* counts, const int64_t* offsets,
+                            int32_t* indices, void* stream);
 
 /* NEXT-1: ray queries, "all [primitives] that a ray intersects", through the same
  * Algorithm 1 kernel with a third predicate.  A ray is 8 floats {origin.xyz, direction.xyz, tmin, tmax}: the points

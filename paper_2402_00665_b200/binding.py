@@ -45,6 +45,9 @@ SYMBOLS = {
     "bvh_scan_counts": [_P, c_int64, _P, _P, c_size_t, _P],
     "bvh_query_spheres_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
     "bvh_query_boxes_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
+    "bvh_query_collect": [_P, c_int64, _P, c_int, c_int64, _P, c_int64, _P, _P, _P],
+    "bvh_rows_to_csr": [_P, c_int64, _P, _P, c_int64, _P, _P],
+    "bvh_query_fill_overflow": [_P, c_int64, _P, c_int, c_int64, _P, c_int64, _P, _P, _P, _P],
     "bvh_query_order_rays": [_P, c_int64, _P, c_int64, _P, _P, c_size_t, _P],
     "bvh_query_rays_count": [_P, c_int64, _P, c_int64, _P, _P, _P],
     "bvh_query_rays_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
@@ -160,6 +163,23 @@ def bvh_query_boxes_count(nodes, n: int, minmax, q: int, order, counts) -> None:
            "bvh_query_boxes_count")
 
 
+def bvh_query_collect(nodes, n: int, queries, query_kind: int, q: int, order, cap: int, rows, counts) -> None:
+    _check(load_library().bvh_query_collect(_ptr(nodes), n, _ptr(queries), query_kind, q, _ptr(order), cap, _ptr(rows),
+                                            _ptr(counts), _stream()), "bvh_query_collect")
+
+
+def bvh_rows_to_csr(rows, cap: int, counts, offsets, q: int, indices) -> None:
+    _check(load_library().bvh_rows_to_csr(_ptr(rows), cap, _ptr(counts), _ptr(offsets), q, _ptr(indices), _stream()),
+           "bvh_rows_to_csr")
+
+
+def bvh_query_fill_overflow(nodes, n: int, queries, query_kind: int, q: int, order, cap: int, counts, offsets,
+                            indices) -> None:
+    _check(load_library().bvh_query_fill_overflow(_ptr(nodes), n, _ptr(queries), query_kind, q, _ptr(order), cap,
+                                                  _ptr(counts), _ptr(offsets), _ptr(indices), _stream()),
+           "bvh_query_fill_overflow")
+
+
 def bvh_query_order_rays(nodes, n: int, rays, q: int, order, scratch) -> None:
     _check(load_library().bvh_query_order_rays(_ptr(nodes), n, _ptr(rays), q, _ptr(order), _ptr(scratch),
                                                scratch.numel() * scratch.element_size(), _stream()),
@@ -268,18 +288,30 @@ class QueryWorkspace:
         self.order_scratch = torch.empty(bvh_query_order_sizes(self.q), dtype=torch.uint8, device=device)
 
 
+QUERY_KINDS = {4: 0, 6: 1, 8: 2}   # floats per query -> query_kind of the C ABI
+
+
 def query(bvh: Bvh, queries: torch.Tensor, ws: QueryWorkspace | None = None, indices: torch.Tensor | None = None,
-          ordered: bool = True):
+          ordered: bool = True, row_capacity: int | None = None, rows: torch.Tensor | None = None):
     """Range search.  queries: float32 CUDA [q,4] spheres {x,y,z,r}, [q,6] boxes {min,max} or [q,8] rays
     {origin, direction, tmin, tmax}.
 
     order (Morton schedule of the queries) -> count -> scan -> fill.  Returns (offsets int64[q+1], indices
     int32[nnz]) on the device.  Reads nnz back once (the path's only device->host sync) unless ``indices`` is
-    passed in with enough room."""
+    passed in with enough room.
+
+    ``row_capacity`` (a multiple of 8) selects the single-pass variant instead: order -> collect (one traversal
+    into rows of that many entries + exact counts) -> scan -> rows_to_csr -> fill_overflow (only the rows that
+    did not fit are traversed again).  Same result, byte for byte.  ``rows``: optional int32 buffer of
+    q * row_capacity entries to reuse."""
     if queries.dtype != torch.float32 or queries.dim() != 2 or queries.shape[1] not in (4, 6, 8):
         raise BvhError(f"expected float32 [q,4], [q,6] or [q,8], got {queries.dtype} {tuple(queries.shape)}")
     q = int(queries.shape[0])
+    if bvh.prim_kind is None:
+        raise BvhError("query() on a Bvh that has not been built")
     ws = ws or QueryWorkspace(q, queries.device)
+    if ws.q < q:
+        raise BvhError(f"QueryWorkspace holds {ws.q} queries, {q} given")
     order_fn, count, fill = {
         4: (bvh_query_order_spheres, bvh_query_spheres_count, bvh_query_spheres_fill),
         6: (bvh_query_order_boxes, bvh_query_boxes_count, bvh_query_boxes_fill),
@@ -289,13 +321,26 @@ def query(bvh: Bvh, queries: torch.Tensor, ws: QueryWorkspace | None = None, ind
     if ordered and q > 0:
         order_fn(bvh.nodes, bvh.n, queries, q, ws.order, ws.order_scratch)
         order = ws.order
-    count(bvh.nodes, bvh.n, queries, q, order, ws.counts)
+    kind = QUERY_KINDS[int(queries.shape[1])]
+    if row_capacity is not None:
+        cap = int(row_capacity)
+        if rows is None:
+            rows = torch.empty(max(q, 1) * cap, dtype=torch.int32, device=queries.device)
+        elif rows.numel() < q * cap:
+            raise BvhError(f"rows holds {rows.numel()} entries, {q * cap} needed")
+        bvh_query_collect(bvh.nodes, bvh.n, queries, kind, q, order, cap, rows, ws.counts)
+    else:
+        count(bvh.nodes, bvh.n, queries, q, order, ws.counts)
     bvh_scan_counts(ws.counts, q, ws.offsets, ws.scan_scratch)
     if indices is None:
         nnz = int(ws.offsets[q].item())
         indices = torch.empty(max(nnz, 1), dtype=torch.int32, device=queries.device)
     else:
-        nnz = None
-    fill(bvh.nodes, bvh.n, queries, q, order, ws.offsets, indices)
+        nnz = None   # the caller vouches for the size (reading offsets[q] back here would be the sync it avoids)
+    if row_capacity is not None:
+        bvh_rows_to_csr(rows, cap, ws.counts, ws.offsets, q, indices)
+        bvh_query_fill_overflow(bvh.nodes, bvh.n, queries, kind, q, order, cap, ws.counts, ws.offsets, indices)
+    else:
+        fill(bvh.nodes, bvh.n, queries, q, order, ws.offsets, indices)
     offsets = ws.offsets[: q + 1]
     return offsets, (indices if nnz is None else indices[:nnz])

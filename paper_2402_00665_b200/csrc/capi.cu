@@ -7,6 +7,16 @@ namespace bvh {
 
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+int sm_count() {
+  static const int sms = []() {
+    int dev = 0, v = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0)
+      v = kNumSMs;
+    return v;
+  }();
+  return sms;
+}
+
 ScratchLayout scratch_layout(int64_t n, int morton_bits) {
   ScratchLayout L{};
   L.key_bytes = (morton_bits == 30) ? 4 : 8;
@@ -168,28 +178,38 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   return check_launch();
 }
 
-static int query(const void* nodes, int64_t n, const float* queries, int64_t q, int kind, bool fill,
-                 const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* indices, void* stream_) {
+static inline bool misaligned32(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 31u) != 0; }
+
+// mode: kModeCount / kModeFill / kModeCollect of traverse.cu (0 / 1 / 2).  cap: collect: entries per row; fill with
+// only_over: rows with counts[j] > cap.  Whether `nodes` holds a finished hierarchy over n primitives is checked on the
+// device (NodesHeader), since the library may not synchronise: a stale buffer yields counts of 0 and no stores.
+static int query(const void* nodes, int64_t n, const float* queries, int64_t q, int kind, int mode,
+                 const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* out, int64_t cap, bool only_over,
+                 void* stream_) {
   if (n < 0 || q < 0) return BVH_ERR_INVALID_ARGUMENT;
   if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
+  if (kind < 0 || kind > 2) return BVH_ERR_INVALID_ARGUMENT;
   if (q == 0) return BVH_OK;
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-  if (fill) {
-    if (!offsets) return BVH_ERR_INVALID_ARGUMENT;
+  if (mode == 1) {
+    if (!offsets || (only_over && !counts)) return BVH_ERR_INVALID_ARGUMENT;
   } else {
     if (!counts) return BVH_ERR_INVALID_ARGUMENT;
   }
+  if (mode == 2 && (cap < 8 || cap % 8 != 0 || cap > 0x7fffffff || !out || misaligned32(out))) return BVH_ERR_INVALID_ARGUMENT;
   if (n == 0) {
-    if (!fill) {
+    if (mode != 1) {
       zero_counts_kernel<<<(unsigned)((q + 255) / 256), 256, 0, stream>>>(counts, q);
       return check_launch();
     }
     return BVH_OK;
   }
-  if (!nodes || !queries || misaligned(nodes) || misaligned(queries)) return BVH_ERR_INVALID_ARGUMENT;
-  if (fill && !indices) return BVH_ERR_INVALID_ARGUMENT;  // nnz = 0 callers still pass a valid pointer
-  launch_traverse(nodes, (int)n, queries, q, kind, fill, order, counts, offsets, indices, stream);
-  return check_launch();
+  // node records are read with 256-bit loads: 32-byte alignment
+  if (!nodes || !queries || misaligned32(nodes) || misaligned(queries)) return BVH_ERR_INVALID_ARGUMENT;
+  if (mode == 1 && !out) return BVH_ERR_INVALID_ARGUMENT;  // nnz = 0 callers still pass a valid pointer
+  if (launch_traverse(nodes, (int)n, queries, q, kind, mode, order, counts, offsets, out, cap, only_over, stream) != cudaSuccess)
+    return BVH_ERR_CUDA;
+  return BVH_OK;
 }
 
 __global__ void iota_kernel(uint32_t* order, int64_t q) {
@@ -293,22 +313,22 @@ int bvh_query_order_rays(const void* nodes, int64_t n, const float* rays, int64_
 
 int bvh_query_rays_count(const void* nodes, int64_t n, const float* rays, int64_t q, const uint32_t* order,
                          int32_t* counts, void* stream) {
-  return bvh::query(nodes, n, rays, q, 2, false, order, counts, nullptr, nullptr, stream);
+  return bvh::query(nodes, n, rays, q, 2, 0, order, counts, nullptr, nullptr, 0, false, stream);
 }
 
 int bvh_query_rays_fill(const void* nodes, int64_t n, const float* rays, int64_t q, const uint32_t* order,
                         const int64_t* offsets, int32_t* indices, void* stream) {
-  return bvh::query(nodes, n, rays, q, 2, true, order, nullptr, offsets, indices, stream);
+  return bvh::query(nodes, n, rays, q, 2, 1, order, nullptr, offsets, indices, 0, false, stream);
 }
 
 int bvh_query_spheres_count(const void* nodes, int64_t n, const float* xyzr, int64_t q, const uint32_t* order,
                             int32_t* counts, void* stream) {
-  return bvh::query(nodes, n, xyzr, q, 0, false, order, counts, nullptr, nullptr, stream);
+  return bvh::query(nodes, n, xyzr, q, 0, 0, order, counts, nullptr, nullptr, 0, false, stream);
 }
 
 int bvh_query_boxes_count(const void* nodes, int64_t n, const float* minmax, int64_t q, const uint32_t* order,
                           int32_t* counts, void* stream) {
-  return bvh::query(nodes, n, minmax, q, 1, false, order, counts, nullptr, nullptr, stream);
+  return bvh::query(nodes, n, minmax, q, 1, 0, order, counts, nullptr, nullptr, 0, false, stream);
 }
 
 int bvh_scan_sizes(int64_t q, size_t* scratch_bytes) {
@@ -328,12 +348,34 @@ int bvh_scan_counts(const int32_t* counts, int64_t q, int64_t* offsets, void* sc
 
 int bvh_query_spheres_fill(const void* nodes, int64_t n, const float* xyzr, int64_t q, const uint32_t* order,
                            const int64_t* offsets, int32_t* indices, void* stream) {
-  return bvh::query(nodes, n, xyzr, q, 0, true, order, nullptr, offsets, indices, stream);
+  return bvh::query(nodes, n, xyzr, q, 0, 1, order, nullptr, offsets, indices, 0, false, stream);
 }
 
 int bvh_query_boxes_fill(const void* nodes, int64_t n, const float* minmax, int64_t q, const uint32_t* order,
                          const int64_t* offsets, int32_t* indices, void* stream) {
-  return bvh::query(nodes, n, minmax, q, 1, true, order, nullptr, offsets, indices, stream);
+  return bvh::query(nodes, n, minmax, q, 1, 1, order, nullptr, offsets, indices, 0, false, stream);
+}
+
+int bvh_query_collect(const void* nodes, int64_t n, const float* queries, int query_kind, int64_t q, const uint32_t* order,
+                      int64_t cap, int32_t* rows, int32_t* counts, void* stream) {
+  return bvh::query(nodes, n, queries, q, query_kind, 2, order, counts, nullptr, rows, cap, false, stream);
+}
+
+int bvh_rows_to_csr(const int32_t* rows, int64_t cap, const int32_t* counts, const int64_t* offsets, int64_t q,
+                    int32_t* indices, void* stream) {
+  if (q < 0 || cap < 8 || cap % 8 != 0) return BVH_ERR_INVALID_ARGUMENT;
+  if (q == 0) return BVH_OK;
+  if (!rows || !counts || !offsets || !indices) return BVH_ERR_INVALID_ARGUMENT;
+  if (bvh::launch_rows_to_csr(rows, cap, counts, offsets, q, indices, static_cast<cudaStream_t>(stream)) != cudaSuccess)
+    return BVH_ERR_CUDA;
+  return BVH_OK;
+}
+
+int bvh_query_fill_overflow(const void* nodes, int64_t n, const float* queries, int query_kind, int64_t q,
+                            const uint32_t* order, int64_t cap, const int32_t* counts, const int64_t* offsets,
+                            int32_t* indices, void* stream) {
+  if (cap < 0) return BVH_ERR_INVALID_ARGUMENT;
+  return bvh::query(nodes, n, queries, q, query_kind, 1, order, const_cast<int32_t*>(counts), offsets, indices, cap, true, stream);
 }
 
 int bvh_export(const void* nodes, const void* scratch, int64_t n, int morton_bits, void* sorted_codes, uint32_t* perm,

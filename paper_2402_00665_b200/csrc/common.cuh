@@ -9,7 +9,7 @@ namespace bvh {
 
 constexpr int kSentinel = -1;   // the paper's sentinel node; reading G9
 constexpr int kInvalid = -1;    // the paper's "invalid entry value (e.g., -1)" in `store`
-constexpr int kNumSMs = 148;    // B200
+constexpr int kNumSMs = 148;    // B200: compile-time grid sizing of the streaming kernels (a performance choice, not a limit)
 
 // 32-byte node record, read and written as two float4 (one 32-byte sector per node visit).
 //   lo = {min.x, min.y, min.z, bitcast(left_child)}   hi = {max.x, max.y, max.z, bitcast(rope)}
@@ -169,11 +169,15 @@ size_t variant_extra_bytes(int64_t n);
 int launch_variant_karras(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
                           void* nodes, int n, const Header* header, void* extra, cudaStream_t stream);
 // K6/K8: stackless traversal.  kind 0 = spheres (xyzr), 1 = boxes (minmax), 2 = rays (o.xyz, d.xyz, tmin, tmax).
-// fill: offsets/indices used.
+// mode 0 = count (counts out), 1 = fill (offsets in, out = indices; only_over: only rows with counts[j] > cap),
+// 2 = collect (out = rows of cap entries, counts out).
 // order (optional): thread t serves query order[t] (results still land in row order[t]).
-void launch_traverse(const void* nodes, int n, const float* queries, int64_t q, int kind, bool fill,
-                     const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* indices,
-                     cudaStream_t stream);
+cudaError_t launch_traverse(const void* nodes, int n, const float* queries, int64_t q, int kind, int mode,
+                            const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* out, int64_t cap,
+                            bool only_over, cudaStream_t stream);
+cudaError_t launch_rows_to_csr(const int32_t* rows, int64_t cap, const int32_t* counts, const int64_t* offsets, int64_t q,
+                               int32_t* indices, cudaStream_t stream);
+int sm_count();   // multiprocessors of the current device (cached)
 // K7: exclusive scan of int32 counts into int64 offsets[q+1].
 size_t scan_scratch_bytes(int64_t q);
 void launch_scan(const int32_t* counts, int64_t q, int64_t* offsets, void* scratch, cudaStream_t stream);

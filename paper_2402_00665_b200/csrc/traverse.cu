@@ -209,37 +209,102 @@ struct LeafRec<false> {
 #define BVH_SCAN_UNROLL 4
 #endif
 
-template <typename Query, bool FILL, bool POINT_LEAF>
-__device__ __forceinline__ void traverse_body(const char* __restrict__ nodes, int n, const float* __restrict__ queries,
-                                              int64_t q, const uint32_t* __restrict__ order, int32_t* __restrict__ counts,
-                                              const int64_t* __restrict__ offsets, int32_t* __restrict__ indices,
-                                              int64_t num_chunks, int ctas_per_sm) {
+// What a pass does with a leaf that satisfies the predicate (Alg. 1 L5, "Store the result or perform an operation"):
+//   kModeCount    count it (K6);
+//   kModeFill     store its primitive at offsets[query] + k (K8);
+//   kModeCollect  single-pass variant: store it in the query's own slice of `cap` entries of a
+//                 caller-provided buffer (rows + query * cap; hits past cap are dropped) AND count it, so that one
+//                 traversal yields counts and, for every row that fits, its content.
+enum { kModeCount = 0, kModeFill = 1, kModeCollect = 2 };
+
+struct TraverseArgs {
+  const char* nodes;
+  int n;
+  const float* queries;
+  int64_t q;
+  const uint32_t* order;     // optional: thread t serves query order[t]
+  int32_t* counts;           // count, collect: out.  fill with only_over: in
+  const int64_t* offsets;    // fill
+  int32_t* out;              // fill: indices; collect: rows
+  int64_t cap;               // collect: entries per row.  fill with only_over: only rows with counts[j] > cap are filled
+  int only_over;
+  int64_t num_chunks;
+  int ctas_per_sm;
+  int num_sms;
+};
+
+// Row output of the fill / collect passes.  The hits of a row arrive a few at a time (one scan step of 32 leaves gives
+// ~8 on C3), at whatever alignment the row has: stored as they come, almost every 32-byte sector of the result would
+// be written in two or three pieces, and a sector that reaches L2 in pieces costs a DRAM read to complete it (round 1:
+// 1.78 x the algorithmic DRAM traffic).  So hits are staged: each query keeps the tail of its row that does not fill a
+// sector yet (< 8 entries) in shared memory; the hits of a posted range are appended to it in a per-warp buffer, and
+// the warp writes out what is complete up to the last 32-byte boundary of the global address, as consecutive lanes =
+// whole sectors, and keeps the rest.  Only the first and last sector of a row can be partial.
+#ifndef BVH_FILL_STAGE
+#define BVH_FILL_STAGE 0
+#endif
+constexpr int kFillStage = BVH_FILL_STAGE;        // 0: store hits as they come; 1: per posted range, coalesced; 2: whole sectors
+constexpr int kStageInts = 8;                      // one sector
+constexpr int kRangeBufInts = kScanLeaves + kStageInts;
+
+__device__ __forceinline__ void store_sector(int32_t* p, const int* v) {   // 32-byte aligned: one full sector
+  asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]),
+               "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
+               : "memory");
+}
+
+// Shared memory of a block: what a lane posts for the warp to read (its query, the leaf range to scan, where its row
+// starts) and the staging of the row output.
+template <typename Query, bool STORE>
+struct TravSmem {
+  __align__(16) float query[kTravThreads * Query::kSlotWords];
+  int2 range[kTravThreads];
+  int32_t* row[STORE ? kTravThreads : 1];
+  __align__(32) int stage[STORE ? kTravThreads * kStageInts : 8];
+  int buf[STORE ? (kTravThreads / 32) * kRangeBufInts : 1];
+};
+
+template <typename Query, int MODE, bool POINT_LEAF>
+__device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Query, MODE != kModeCount>& S) {
+  constexpr bool STORE = MODE != kModeCount;
   constexpr int U = POINT_LEAF ? BVH_SCAN_UNROLL : (BVH_SCAN_UNROLL > 2 ? 2 : BVH_SCAN_UNROLL);   // leaf loads in flight per lane
-  // what a lane posts for the warp to read: its query, the leaf range to scan, (fill) where its row starts
-  __shared__ __align__(16) float s_query[kTravThreads * Query::kSlotWords];
-  __shared__ int2 s_range[kTravThreads];
-  __shared__ int64_t s_row[FILL ? kTravThreads : 1];
+  float* const s_query = S.query;
+  int2* const s_range = S.range;
+  int32_t** const s_row = S.row;
+  int* const s_stage = S.stage;
+  int* const s_buf = S.buf;
+  const char* __restrict__ nodes = A.nodes;
+  const int n = A.n;
+  const float* __restrict__ queries = A.queries;
+  const uint32_t* __restrict__ order = A.order;
   const Node* __restrict__ internal = reinterpret_cast<const Node*>(nodes + kNodesHeaderBytes);
   const char* __restrict__ leaves = nodes + leaf_offset_bytes(n);
   const int leaf_base = n - 1;
   const int lane = threadIdx.x & 31;
   const int warp_first = threadIdx.x - lane;               // slot of lane 0 of this warp
   const uint32_t lt_mask = (1u << lane) - 1u;
-  const int64_t sm_slot = blockIdx.x % kNumSMs;
-  const int64_t r = blockIdx.x / kNumSMs;
+  int* const buf = s_buf + (STORE ? (threadIdx.x >> 5) * kRangeBufInts : 0);
+  const int cap = (MODE == kModeCollect) ? (int)A.cap : 0x7fffffff;   // row positions >= cap are not stored
+  const int64_t sm_slot = blockIdx.x % A.num_sms;
+  const int64_t r = blockIdx.x / A.num_sms;
   for (int64_t k = 0;; ++k) {
-    const int64_t chunk = (k * kNumSMs + sm_slot) * ctas_per_sm + r;
-    if (chunk >= num_chunks) break;
+    const int64_t chunk = (k * A.num_sms + sm_slot) * A.ctas_per_sm + r;
+    if (chunk >= A.num_chunks) break;
     const int64_t t = chunk * kTravThreads + threadIdx.x;
-    const bool have = t < q;
+    bool have = t < A.q;
     const int64_t j = have ? (order ? (int64_t)order[t] : t) : 0;
+    if (MODE == kModeFill && A.only_over) have = have && (int64_t)A.counts[j] > A.cap;
     Query query;
     query.load(queries, j);
     __syncwarp();                                            // the previous chunk's scans are over
     query.to_shared(s_query + threadIdx.x * Query::kSlotWords);
-    if (FILL) s_row[threadIdx.x] = have ? offsets[j] : 0;    // this query's CSR row
+    int32_t* row = nullptr;
+    if (STORE) {
+      row = (MODE == kModeFill) ? A.out + (have ? A.offsets[j] : 0) : A.out + j * A.cap;   // this query's row
+      s_row[threadIdx.x] = row;
+    }
     __syncwarp();
-    int32_t* const row = FILL ? indices + s_row[FILL ? threadIdx.x : 0] : nullptr;
+    const int align = STORE ? (int)((reinterpret_cast<uintptr_t>(row) >> 2) & (kStageInts - 1)) : 0;
     int count = 0;
     int node = have ? 0 : kSentinel;                         // L1: start from the root
     int first = 0;                                           // first leaf below `node`
@@ -262,11 +327,22 @@ __device__ __forceinline__ void traverse_body(const char* __restrict__ nodes, in
         oq.from_shared(s_query + (warp_first + o) * Query::kSlotWords);
         const int2 range = s_range[warp_first + o];
         const int end = range.y;
-        int ocount = 0;                                    // count: this lane's hits; fill: the row's running length
+        int ocount = 0;                                    // count: this lane's hits; store: entries in `buf`
         int32_t* orow = nullptr;
-        if (FILL) {
-          ocount = __shfl_sync(0xffffffffu, count, o);
-          orow = indices + s_row[warp_first + o];
+        int p0 = 0, oalign = 0;
+        if (STORE) {
+          const int oc = __shfl_sync(0xffffffffu, count, o);
+          orow = s_row[warp_first + o];
+          if (kFillStage == 2) {
+            // the row's staged tail comes first in the range buffer
+            oalign = __shfl_sync(0xffffffffu, align, o);
+            const int carry = min(oc, (oalign + oc) & (kStageInts - 1));
+            p0 = oc - carry;                               // row position of buf[0]: sector-aligned, or the row's start
+            if (lane < carry) buf[lane] = s_stage[(warp_first + o) * kStageInts + lane];
+            ocount = carry;
+          } else {
+            p0 = oc;
+          }
         }
         for (int c = range.x + lane; c < end + lane; c += 32 * U) {   // c - lane is warp-uniform
           LeafRec<POINT_LEAF> leaf[U];
@@ -278,17 +354,37 @@ __device__ __forceinline__ void traverse_body(const char* __restrict__ nodes, in
             const bool inside = c + 32 * u < end;
             const bool sat = leaf[u].hit(oq);              // evaluated on every lane (no branch); masked below
             const bool hit = inside & sat;                 // L3-5 on leaf c + 32u
-            if (FILL) {
+            if (STORE) {
               const uint32_t m = __ballot_sync(0xffffffffu, hit);
-              if (hit) orow[ocount + __popc(m & lt_mask)] = (int)(leaf[u].payload() & kLeafPrimMask);
+              const int at = ocount + __popc(m & lt_mask);
+              if (kFillStage == 0) {
+                if (hit && p0 + at < cap) orow[p0 + at] = (int)(leaf[u].payload() & kLeafPrimMask);
+              } else {
+                if (hit) buf[at] = (int)(leaf[u].payload() & kLeafPrimMask);
+              }
               ocount += __popc(m);
             } else {
               ocount += hit ? 1 : 0;
             }
           }
         }
-        if (FILL) {
-          if (lane == o) count = ocount;
+        if (STORE) {
+          if (kFillStage == 2) {
+            __syncwarp();
+            // write out up to the last sector boundary of the global address; keep the rest staged
+            const int rem = (oalign + p0 + ocount) & (kStageInts - 1);
+            const int flush = ocount - rem > 0 ? ocount - rem : 0;
+            for (int e = lane; e < flush; e += 32)
+              if (p0 + e < cap) orow[p0 + e] = buf[e];
+            if (lane < ocount - flush) s_stage[(warp_first + o) * kStageInts + lane] = buf[flush + lane];
+            __syncwarp();
+          } else if (kFillStage == 1) {
+            __syncwarp();
+            for (int e = lane; e < ocount; e += 32)
+              if (p0 + e < cap) orow[p0 + e] = buf[e];
+            __syncwarp();
+          }
+          if (lane == o) count = p0 + ocount;
         } else {
           const int total = __reduce_add_sync(0xffffffffu, ocount);   // one REDUX per range instead of a ballot per step
           if (lane == o) count += total;
@@ -302,7 +398,22 @@ __device__ __forceinline__ void traverse_body(const char* __restrict__ nodes, in
           leaf.load(leaves, i);
           const uint32_t payload = leaf.payload();
           if (leaf.hit(query)) {                             // L3-5
-            if (FILL) row[count] = (int)(payload & kLeafPrimMask);
+            if (STORE && kFillStage != 2) {
+              if (count < cap) row[count] = (int)(payload & kLeafPrimMask);
+            } else if (STORE) {
+              int* st = s_stage + threadIdx.x * kStageInts;
+              const int carry = min(count, (align + count) & (kStageInts - 1));
+              st[carry] = (int)(payload & kLeafPrimMask);
+              if (((align + count + 1) & (kStageInts - 1)) == 0) {   // the sector is complete
+                const int p = count - carry;
+                if (carry + 1 == kStageInts) {
+                  if (p < cap) store_sector(row + p, st);    // (cap is a multiple of 8: a sector is inside or outside)
+                } else {
+                  for (int e = 0; e <= carry; ++e)
+                    if (p + e < cap) row[p + e] = st[e];
+                }
+              }
+            }
             ++count;
           }
           // L6: N_skip of leaf i (Algorithm 2): leaf i+1 or internal node i+1, one bit in the record
@@ -327,51 +438,116 @@ __device__ __forceinline__ void traverse_body(const char* __restrict__ nodes, in
       }
       __syncwarp();                                          // posted ranges are visible to the warp
     }
-    if (!FILL && have) counts[j] = count;
+    if (STORE && kFillStage == 2) {                          // what is still staged: the row's last, partial sector
+      const int carry = min(count, (align + count) & (kStageInts - 1));
+      const int* st = s_stage + threadIdx.x * kStageInts;
+      for (int e = 0; e < carry; ++e)
+        if (count - carry + e < cap) row[count - carry + e] = st[e];
+    }
+    if (MODE != kModeFill && have) A.counts[j] = count;
   }
 }
 
 // The leaf format (point or box records) is a property of the hierarchy, recorded in its header by the build;
-// the kernel reads it there (one uniform branch), so the query entry points need no extra argument.
-template <typename Query, bool FILL>
-__global__ void __launch_bounds__(kTravThreads, Query::kCtasPerSm)
-traverse_kernel(const char* __restrict__ nodes, int n, const float* __restrict__ queries, int64_t q,
-                const uint32_t* __restrict__ order, int32_t* __restrict__ counts, const int64_t* __restrict__ offsets,
-                int32_t* __restrict__ indices, int64_t num_chunks, int ctas_per_sm) {
-  if (reinterpret_cast<const NodesHeader*>(nodes)->leaf_kind == kLeafPoints)
-    traverse_body<Query, FILL, true>(nodes, n, queries, q, order, counts, offsets, indices, num_chunks, ctas_per_sm);
+// the kernel reads it there (one uniform branch), so the query entry points need no extra argument.  The same
+// header tells whether `nodes` holds a finished hierarchy over n primitives at all: if not (never built, built for
+// another n, overwritten), nothing is traversed -- counts come out as 0, nothing is stored -- instead of following
+// garbage indices.
+template <typename Query, int MODE>
+__global__ void __launch_bounds__(kTravThreads, Query::kCtasPerSm) traverse_kernel(const TraverseArgs A) {
+  const NodesHeader* h = reinterpret_cast<const NodesHeader*>(A.nodes);
+  if (h->magic != kNodesMagic || h->n != A.n) {
+    if (MODE != kModeFill)
+      for (int64_t t = (int64_t)blockIdx.x * kTravThreads + threadIdx.x; t < A.q; t += (int64_t)gridDim.x * kTravThreads)
+        A.counts[t] = 0;
+    return;
+  }
+  __shared__ TravSmem<Query, MODE != kModeCount> S;
+  if (h->leaf_kind == kLeafPoints)
+    traverse_body<Query, MODE, true>(A, S);
   else
-    traverse_body<Query, FILL, false>(nodes, n, queries, q, order, counts, offsets, indices, num_chunks, ctas_per_sm);
+    traverse_body<Query, MODE, false>(A, S);
 }
 
 template <typename Query>
-static void launch_traverse_kind(const char* nodes, int n, const float* queries, int64_t q, bool fill,
-                                 const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* indices,
-                                 cudaStream_t stream) {
-  const int64_t num_chunks = (q + kTravThreads - 1) / kTravThreads;
-  // persistent grid: up to 148 x Query::kCtasPerSm CTAs; fewer CTAs per SM when there is not enough work to fill them
-  int ctas_per_sm = (int)((num_chunks + kNumSMs - 1) / kNumSMs);
+static cudaError_t launch_traverse_kind(TraverseArgs A, int mode, cudaStream_t stream) {
+  A.num_chunks = (A.q + kTravThreads - 1) / kTravThreads;
+  A.num_sms = sm_count();
+  // persistent grid: up to SMs x Query::kCtasPerSm CTAs; fewer CTAs per SM when there is not enough work to fill them
+  int ctas_per_sm = (int)((A.num_chunks + A.num_sms - 1) / A.num_sms);
   if (ctas_per_sm > Query::kCtasPerSm) ctas_per_sm = Query::kCtasPerSm;
   if (ctas_per_sm < 1) ctas_per_sm = 1;
-  const unsigned g = (unsigned)(kNumSMs * ctas_per_sm);
-  if (fill)
-    traverse_kernel<Query, true><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, order, counts, offsets, indices,
-                                                                num_chunks, ctas_per_sm);
+  A.ctas_per_sm = ctas_per_sm;
+  const unsigned g = (unsigned)(A.num_sms * ctas_per_sm);
+  if (mode == kModeCount)
+    traverse_kernel<Query, kModeCount><<<g, kTravThreads, 0, stream>>>(A);
+  else if (mode == kModeFill)
+    traverse_kernel<Query, kModeFill><<<g, kTravThreads, 0, stream>>>(A);
   else
-    traverse_kernel<Query, false><<<g, kTravThreads, 0, stream>>>(nodes, n, queries, q, order, counts, offsets, indices,
-                                                                 num_chunks, ctas_per_sm);
+    traverse_kernel<Query, kModeCollect><<<g, kTravThreads, 0, stream>>>(A);
+  return cudaGetLastError();
 }
 
-void launch_traverse(const void* nodes, int n, const float* queries, int64_t q, int kind, bool fill,
-                     const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* indices,
-                     cudaStream_t stream) {
-  const char* base = static_cast<const char*>(nodes);
-  if (kind == 0)
-    launch_traverse_kind<SphereQuery>(base, n, queries, q, fill, order, counts, offsets, indices, stream);
-  else if (kind == 1)
-    launch_traverse_kind<BoxQuery>(base, n, queries, q, fill, order, counts, offsets, indices, stream);
-  else
-    launch_traverse_kind<RayQuery>(base, n, queries, q, fill, order, counts, offsets, indices, stream);
+cudaError_t launch_traverse(const void* nodes, int n, const float* queries, int64_t q, int kind, int mode,
+                            const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* out, int64_t cap,
+                            bool only_over, cudaStream_t stream) {
+  TraverseArgs A{};
+  A.nodes = static_cast<const char*>(nodes);
+  A.n = n;
+  A.queries = queries;
+  A.q = q;
+  A.order = order;
+  A.counts = counts;
+  A.offsets = offsets;
+  A.out = out;
+  A.cap = cap;
+  A.only_over = only_over ? 1 : 0;
+  if (kind == 0) return launch_traverse_kind<SphereQuery>(A, mode, stream);
+  if (kind == 1) return launch_traverse_kind<BoxQuery>(A, mode, stream);
+  return launch_traverse_kind<RayQuery>(A, mode, stream);
+}
+
+// rows -> CSR (single-pass variant): row j of `rows` (cap entries, counts[j] of them valid if counts[j] <= cap) is copied
+// to indices[offsets[j] ...).  Rows that did not fit (counts[j] > cap) are skipped: the fill pass restricted to them
+// (only_over) writes those.  One group of G lanes per row.
+template <int G>
+__global__ void __launch_bounds__(256) rows_to_csr_kernel(const int32_t* __restrict__ rows, int64_t cap,
+                                                          const int32_t* __restrict__ counts,
+                                                          const int64_t* __restrict__ offsets, int64_t q,
+                                                          int32_t* __restrict__ indices) {
+  const int64_t group = ((int64_t)blockIdx.x * 256 + threadIdx.x) / G;
+  const int64_t groups = (int64_t)gridDim.x * 256 / G;
+  const int gl = threadIdx.x % G;
+  for (int64_t j = group; j < q; j += groups) {
+    const int c = counts[j];
+    if (c <= 0 || c > cap) continue;
+    const int32_t* __restrict__ src = rows + j * cap;
+    int32_t* __restrict__ dst = indices + offsets[j];
+    int e = gl;
+    for (; e + 3 * G < c; e += 4 * G) {                     // four loads in flight per lane
+      const int v0 = __ldcs(src + e), v1 = __ldcs(src + e + G), v2 = __ldcs(src + e + 2 * G), v3 = __ldcs(src + e + 3 * G);
+      dst[e] = v0;
+      dst[e + G] = v1;
+      dst[e + 2 * G] = v2;
+      dst[e + 3 * G] = v3;
+    }
+    for (; e < c; e += G) dst[e] = __ldcs(src + e);
+  }
+}
+
+cudaError_t launch_rows_to_csr(const int32_t* rows, int64_t cap, const int32_t* counts, const int64_t* offsets, int64_t q,
+                               int32_t* indices, cudaStream_t stream) {
+  const int sms = sm_count();
+  if (cap >= 128) {
+    int64_t blocks = (q * 32 + 255) / 256;
+    if (blocks > (int64_t)sms * 16) blocks = (int64_t)sms * 16;
+    rows_to_csr_kernel<32><<<(unsigned)blocks, 256, 0, stream>>>(rows, cap, counts, offsets, q, indices);
+  } else {
+    int64_t blocks = (q * 8 + 255) / 256;
+    if (blocks > (int64_t)sms * 16) blocks = (int64_t)sms * 16;
+    rows_to_csr_kernel<8><<<(unsigned)blocks, 256, 0, stream>>>(rows, cap, counts, offsets, q, indices);
+  }
+  return cudaGetLastError();
 }
 
 }  // namespace bvh

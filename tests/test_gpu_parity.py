@@ -233,6 +233,131 @@ def test_query_order_is_a_permutation_and_does_not_change_results(B):
     assert int(o1[100]) == 0 and int(o1[-1]) > 0
 
 
+def _oracle_csr(oracle_lib, o, queries):
+    fn = {4: oracle_lib.query_spheres_tree, 6: oracle_lib.query_boxes_tree, 8: oracle_lib.query_rays_tree}[queries.shape[1]]
+    return fn(o, queries)
+
+
+@pytest.mark.parametrize("name,n,q,radius", [("C1", 4096, 4096, None), ("C3", 120_001, 5_000, 0.004),
+                                             ("C4", 70_003, 30_000, 4e-3), ("C5", 65_537, 10_000, 0.04)])
+def test_single_pass_query_equals_oracle(B, oracle_lib, name, n, q, radius):
+    """NEXT-3: collect (one traversal into rows of `cap` entries + exact counts) -> scan -> rows_to_csr -> fill_overflow
+    gives the oracle's CSR byte for byte, whatever the capacity: every row fits / some rows overflow / almost all do."""
+    w = W.make(name, n=n, q=q, radius=radius)
+    o = oracle_lib.build_bvh(w.prims, w.morton_bits)
+    bvh = gpu_build(B, w.prims, w.morton_bits)
+    ooff, oidx = _oracle_csr(oracle_lib, o, w.queries)
+    counts = np.diff(ooff)
+    mx = int(counts.max())
+    caps = sorted({(mx + 7) // 8 * 8, max(8, int(np.median(counts)) // 8 * 8), 8})
+    dq = _dev(w.queries)
+    for cap in caps:
+        for ordered in (True, False):
+            off, idx = B.query(bvh, dq, ordered=ordered, row_capacity=cap)
+            torch.cuda.synchronize()
+            assert np.array_equal(off.cpu().numpy(), ooff), (name, cap, "offsets")
+            assert np.array_equal(idx.cpu().numpy()[: ooff[-1]], oidx), (name, cap, "indices in traversal order")
+    # the rows themselves: the first min(count, cap) hits of every query, counts exact
+    cap = caps[len(caps) // 2]
+    rows = torch.full((w.q * cap,), -7, dtype=torch.int32, device="cuda")
+    cnt = torch.empty(w.q, dtype=torch.int32, device="cuda")
+    B.bvh_query_collect(bvh.nodes, bvh.n, dq, B.QUERY_KINDS[w.queries.shape[1]], w.q, None, cap, rows, cnt)
+    torch.cuda.synchronize()
+    assert np.array_equal(cnt.cpu().numpy(), counts)
+    r = rows.cpu().numpy().reshape(w.q, cap)
+    for j in np.random.default_rng(3).choice(w.q, 200, replace=False):
+        k = min(int(counts[j]), cap)
+        assert np.array_equal(r[j, :k], oidx[ooff[j]: ooff[j] + k]) and np.all(r[j, k:] == -7), j
+
+
+def test_single_pass_rays_and_argument_checks(B, oracle_lib):
+    w = W.make("C4", n=30_000, q=0)
+    bvh = gpu_build(B, w.prims, w.morton_bits)
+    rays = _rays_through(w.prims, 4000, seed=31, tmax=4.0)
+    o = oracle_lib.build_bvh(w.prims, w.morton_bits)
+    ooff, oidx = oracle_lib.query_rays_tree(o, rays)
+    off, idx = B.query(bvh, _dev(rays), row_capacity=16)
+    torch.cuda.synchronize()
+    assert np.array_equal(off.cpu().numpy(), ooff) and np.array_equal(idx.cpu().numpy()[: ooff[-1]], oidx)
+    dq = _dev(rays)
+    cnt = torch.empty(4000, dtype=torch.int32, device="cuda")
+    rows = torch.empty(4000 * 16 + 8, dtype=torch.int32, device="cuda")
+    for bad_cap, bad_rows in ((12, rows), (0, rows), (16, rows[1:])):     # not a multiple of 8 / zero / rows misaligned
+        with pytest.raises(B.BvhError):
+            B.bvh_query_collect(bvh.nodes, bvh.n, dq, 2, 4000, None, bad_cap, bad_rows, cnt)
+    with pytest.raises(B.BvhError):
+        B.bvh_query_collect(bvh.nodes, bvh.n, dq, 3, 4000, None, 16, rows, cnt)      # unknown query kind
+    with pytest.raises(B.BvhError):
+        B.query(B.Bvh(100, 30), _dev(W.spheres_at(W.uniform_cube(4, seed=1), 0.1)))    # never built
+
+
+def test_stale_or_mismatched_nodes_buffer_is_not_traversed(B):
+    """The query kernels check the header the build wrote (magic, n) on the device: a buffer that was never built, was
+    built for another n or was overwritten gives counts of 0 and stores nothing, instead of a walk over garbage."""
+    pts = W.uniform_cube(5000, seed=9)
+    bvh = gpu_build(B, pts, 30)
+    qs = _dev(W.spheres_at(pts[:512], 0.2))
+    cnt = torch.full((512,), -1, dtype=torch.int32, device="cuda")
+    B.bvh_query_spheres_count(bvh.nodes, 5000, qs, 512, None, cnt)
+    torch.cuda.synchronize()
+    assert int(cnt.min()) > 0
+    # wrong n for this buffer
+    cnt.fill_(-1)
+    B.bvh_query_spheres_count(bvh.nodes, 4999, qs, 512, None, cnt)
+    torch.cuda.synchronize()
+    assert cnt.cpu().tolist() == [0] * 512
+    # garbage where the hierarchy should be
+    junk = torch.randint(0, 255, (bvh.nodes.numel(),), dtype=torch.uint8, device="cuda")
+    junk[:4] = 0
+    cnt.fill_(-1)
+    B.bvh_query_spheres_count(junk, 5000, qs, 512, None, cnt)
+    rows = torch.full((512 * 8,), -7, dtype=torch.int32, device="cuda")
+    cnt2 = torch.full((512,), -1, dtype=torch.int32, device="cuda")
+    B.bvh_query_collect(junk, 5000, qs, 0, 512, None, 8, rows, cnt2)
+    idx = torch.full((64,), -7, dtype=torch.int32, device="cuda")
+    off = torch.zeros(513, dtype=torch.int64, device="cuda")
+    B.bvh_query_spheres_fill(junk, 5000, qs, 512, None, off, idx)
+    torch.cuda.synchronize()
+    assert cnt.cpu().tolist() == [0] * 512 and cnt2.cpu().tolist() == [0] * 512
+    assert int((rows != -7).sum()) == 0 and int((idx != -7).sum()) == 0
+    with pytest.raises(B.BvhError):                      # 256-bit node loads: 32-byte alignment
+        B.bvh_query_spheres_count(bvh.nodes[16:], 5000, qs, 512, None, cnt)
+
+
+def test_touching_counts_as_intersecting_boxes_and_rays(B, oracle_lib):
+    """G12: closed comparisons.  Box queries that share exactly a face / an edge / a corner with a primitive box hit
+    it, one ulp away they miss; rays that graze a face or end exactly on it (tmax) hit, one ulp short they miss."""
+    f = np.float32
+    prims = np.array([[0.25, 0.25, 0.25, 0.5, 0.5, 0.5], [0.75, 0.75, 0.75, 0.875, 0.875, 0.875],
+                      [-1.0, -1.0, -1.0, -0.5, -0.5, -0.5]], f)
+    up, dn = (lambda x: np.nextafter(f(x), f(np.inf))), (lambda x: np.nextafter(f(x), f(-np.inf)))
+    qb = np.array([
+        [0.5, 0.25, 0.25, 0.625, 0.5, 0.5],              # shares the face x = 0.5
+        [up(0.5), 0.25, 0.25, 0.625, 0.5, 0.5],          # one ulp off
+        [0.5, 0.5, 0.25, 0.625, 0.625, 0.5],             # shares an edge
+        [0.5, 0.5, 0.5, 0.75, 0.75, 0.75],               # corner of the first, corner of the second
+        [0.5, 0.5, up(0.5), 0.75, 0.75, dn(0.75)],       # neither
+        [-0.5, -0.5, -0.5, 0.25, 0.25, 0.25],            # corner of the third and of the first
+    ], f)
+    o = oracle_lib.build_bvh(prims, 63)
+    bvh = gpu_build(B, prims, 63)
+    goff, gidx = assert_query_equal(B, bvh, o, oracle_lib, qb, "touching boxes")
+    assert list(np.diff(goff)) == [1, 0, 1, 2, 0, 2]
+    rays = np.array([
+        [0.0, 0.5, 0.375, 1, 0, 0, 0.0, 8.0],            # runs in the face y = 0.5 of the first box
+        [0.0, up(0.5), 0.375, 1, 0, 0, 0.0, 8.0],        # one ulp above it
+        [0.0, 0.375, 0.375, 1, 0, 0, 0.0, 0.25],         # ends exactly on the face x = 0.25 (tmax)
+        [0.0, 0.375, 0.375, 1, 0, 0, 0.0, dn(0.25)],     # ends one ulp short
+        [1.0, 0.375, 0.375, -1, 0, 0, 0.5, 8.0],         # starts exactly on the face x = 0.5 (tmin)
+        [0.0, 0.0, 0.0, 1, 1, 1, 0.0, 8.0],              # through the corners of the first two boxes
+    ], f)
+    ooff, oidx = oracle_lib.query_rays_tree(o, rays)
+    off, idx = B.query(bvh, _dev(rays))
+    torch.cuda.synchronize()
+    assert np.array_equal(off.cpu().numpy(), ooff) and np.array_equal(idx.cpu().numpy()[: ooff[-1]], oidx)
+    assert list(np.diff(ooff)) == [1, 0, 1, 0, 1, 2]
+
+
 def test_empty_inputs(B):
     bvh = B.Bvh(0, 30)
     bvh.build(torch.zeros((0, 3), dtype=torch.float32, device="cuda"))
