@@ -358,6 +358,49 @@ def test_touching_counts_as_intersecting_boxes_and_rays(B, oracle_lib):
     assert list(np.diff(ooff)) == [1, 0, 1, 0, 1, 2]
 
 
+def test_containment_shortcut_large_queries(B, oracle_lib):
+    """A subtree whose box lies inside the query is reported without walking it (traverse.cu, contains_box).  The result
+    must not change: queries that swallow whole subtrees (up to the whole scene), queries for which the farthest-corner
+    distance of a node equals r*r exactly, and one ulp less -- on a dyadic lattice, where that arithmetic is exact."""
+    f = np.float32
+    g = np.arange(32, dtype=f) / f(32.0)
+    pts = np.stack(np.meshgrid(g, g, g, indexing="ij"), axis=-1).reshape(-1, 3).astype(f)     # 32768 lattice points
+    for bits in (30, 63):
+        o = oracle_lib.build_bvh(pts, bits)
+        bvh = gpu_build(B, pts, bits)
+        c = f(0.5) - f(1.0 / 64.0)                      # centre of the lattice
+        # farthest corner of the whole scene from the centre: (31/64)^2 * 3, exactly representable
+        r2 = f(3.0) * f(31.0 / 64.0) * f(31.0 / 64.0)
+        r = f(np.sqrt(np.float64(r2)))
+        qs = [[c, c, c, 2.0], [c, c, c, r], [c, c, c, np.nextafter(r, f(0))], [c, c, c, np.nextafter(r, f(2))],
+              [0.25, 0.25, 0.25, 0.25], [0.25, 0.25, 0.25, np.nextafter(f(0.25), f(0))], [0.0, 0.0, 0.0, 0.5],
+              [0.75, 0.5, 0.25, 0.3], [5.0, 5.0, 5.0, 1.0]]
+        # spheres whose radius is exactly the farthest-corner distance of an octant [0, 15/32]^3 from its own centre
+        h = f(15.0 / 64.0)
+        rr = f(np.sqrt(np.float64(f(3.0) * h * h)))
+        for dr in (rr, np.nextafter(rr, f(0)), np.nextafter(rr, f(1))):
+            qs.append([h, h, h, dr])
+        qs = np.array(qs, f)
+        goff, gidx = assert_query_equal(B, bvh, o, oracle_lib, qs, f"containment {bits}")
+        assert np.diff(goff)[0] == len(pts) and np.diff(goff)[-4] == 0
+        off, idx = B.query(bvh, _dev(qs), row_capacity=32768)
+        torch.cuda.synchronize()
+        assert np.array_equal(off.cpu().numpy(), goff) and np.array_equal(idx.cpu().numpy()[: goff[-1]], gidx)
+        off, idx = B.query(bvh, _dev(qs), row_capacity=1024)            # contained subtrees larger than the row: truncated, refilled
+        torch.cuda.synchronize()
+        assert np.array_equal(off.cpu().numpy(), goff) and np.array_equal(idx.cpu().numpy()[: goff[-1]], gidx)
+    # box queries and box leaves
+    boxes = W.boxes_around(pts[::2], 1.0 / 256.0)
+    o = oracle_lib.build_bvh(boxes, 63)
+    bvh = gpu_build(B, boxes, 63)
+    lo, hi = boxes[:, :3].min(axis=0), boxes[:, 3:].max(axis=0)
+    qb = np.array([[*lo, *hi], [*np.nextafter(lo, f(1)), *hi], [-1, -1, -1, 2, 2, 2], [*lo, 0.5, 0.5, 0.5],
+                   [0.25, 0.25, 0.25, 0.75, 0.75, 0.75], [*lo, *lo]], f)
+    goff, gidx = assert_query_equal(B, bvh, o, oracle_lib, qb, "containment boxes")
+    assert np.diff(goff)[0] == len(boxes) and np.diff(goff)[2] == len(boxes)
+    assert_query_equal(B, bvh, o, oracle_lib, np.array([[0.5, 0.5, 0.5, 0.45], [0.5, 0.5, 0.5, 5.0]], f), "containment sphere/box leaves")
+
+
 def test_empty_inputs(B):
     bvh = B.Bvh(0, 30)
     bvh.build(torch.zeros((0, 3), dtype=torch.float32, device="cuda"))
