@@ -64,6 +64,20 @@ def _L():
         lib.oracle_result_free.argtypes = [c_void_p]
         lib.oracle_walk_all.argtypes = [i32p, i32p, i64, i32p, i64]
         lib.oracle_walk_all.restype = c_int64
+        for name in ("oracle_nearest_spheres_brute", "oracle_first_hit_rays_brute"):
+            f = getattr(lib, name)
+            f.argtypes = [fp, i64, c_int, fp, i64, i32p, fp]
+            f.restype = None
+        for name in ("oracle_nearest_spheres_tree", "oracle_first_hit_rays_tree"):
+            f = getattr(lib, name)
+            f.argtypes = [fp, i32p, i32p, i64, fp, i64, i32p, fp]
+            f.restype = None
+        lib.oracle_apetrei.argtypes = [u64p, i64, i32p, i32p, i32p]
+        lib.oracle_apetrei.restype = None
+        lib.oracle_ropes_from.argtypes = [i32p, i32p, i64, c_int32, i32p]
+        lib.oracle_ropes_from.restype = None
+        lib.oracle_boxes_from.argtypes = [fp, c_int, u32p, i32p, i32p, i64, c_int32, fp]
+        lib.oracle_boxes_from.restype = None
         for name in ("oracle_scene_bounds", "oracle_morton", "oracle_sort", "oracle_hierarchy", "oracle_ropes",
                      "oracle_ropes_alg2", "oracle_boxes", "oracle_build", "oracle_result_copy", "oracle_result_free"):
             getattr(lib, name).restype = None
@@ -250,3 +264,68 @@ def walk_all(left_child, rope, n: int) -> np.ndarray:
     if k < 0:
         raise RuntimeError("stackless walk did not terminate within 2n+8 visits")
     return order[:k].copy()
+
+
+# ---- D10 / D11: an operation at the leaf instead of a stored row ----------------------------------
+
+def _reduce(fn_brute, fn_tree, queries, width, prim=None, bvh=None):
+    qa = np.ascontiguousarray(queries, np.float32)
+    assert qa.ndim == 2 and qa.shape[1] == width
+    idx = np.empty(qa.shape[0], np.int32)
+    key = np.empty(qa.shape[0], np.float32)
+    if bvh is not None:
+        fn_tree(_p(bvh.aabb, c_float), _p(bvh.left_child, c_int32), _p(bvh.right_child, c_int32), bvh.n, _p(qa, c_float),
+                qa.shape[0], _p(idx, c_int32), _p(key, c_float))
+    else:
+        a, n, is_box = _prims(prim)
+        fn_brute(_p(a, c_float), n, is_box, _p(qa, c_float), qa.shape[0], _p(idx, c_int32), _p(key, c_float))
+    return idx, key
+
+
+def nearest_spheres_brute(prim, xyzr):
+    """D10: per sphere {x,y,z,r}, the primitive with the smallest D8 distance d2 <= r*r (ties: smallest index);
+    returns (index or -1, d2 or +inf).  Tests every primitive."""
+    return _reduce(_L().oracle_nearest_spheres_brute, None, xyzr, 4, prim=prim)
+
+
+def nearest_spheres_tree(bvh: Bvh, xyzr):
+    return _reduce(None, _L().oracle_nearest_spheres_tree, xyzr, 4, bvh=bvh)
+
+
+def first_hit_rays_brute(prim, rays):
+    """D11: per ray, the primitive whose box the ray enters first (smallest t_enter; ties: smallest index);
+    returns (index or -1, t_enter or +inf).  Tests every primitive."""
+    return _reduce(_L().oracle_first_hit_rays_brute, None, rays, 8, prim=prim)
+
+
+def first_hit_rays_tree(bvh: Bvh, rays):
+    return _reduce(None, _L().oracle_first_hit_rays_tree, rays, 8, bvh=bvh)
+
+
+# ---- Algorithm 3: Apetrei's numbering (NEXT-2 a) ------------------------------------------------------------------
+
+class ApetreiTree:
+    """The hierarchy as the unmodified Algorithm 3 numbers it: internal node index = split position, root stored."""
+
+    __slots__ = ("n", "root", "left", "right", "rope", "aabb")
+
+
+def apetrei_tree(prim, bvh: Bvh) -> ApetreiTree:
+    """Runs Algorithm 3 serially over bvh.sorted_codes, then skip-connections by their
+    definition (a walk from the stored root) and boxes by post-order union."""
+    a, n, is_box = _prims(prim)
+    t = ApetreiTree()
+    t.n = n
+    m = max(n - 1, 0)
+    t.left, t.right = np.empty(m, np.int32), np.empty(m, np.int32)
+    root = np.zeros(1, np.int32)
+    if n >= 2:
+        _L().oracle_apetrei(_p(bvh.sorted_codes, c_uint64), n, _p(t.left, c_int32), _p(t.right, c_int32), _p(root, c_int32))
+    t.root = int(root[0])
+    t.rope = np.empty(max(2 * n - 1, 0), np.int32)
+    t.aabb = np.empty((max(2 * n - 1, 0), 6), np.float32)
+    if n >= 1:
+        _L().oracle_ropes_from(_p(t.left, c_int32), _p(t.right, c_int32), n, t.root, _p(t.rope, c_int32))
+        _L().oracle_boxes_from(_p(a, c_float), is_box, _p(bvh.perm, c_uint32), _p(t.left, c_int32), _p(t.right, c_int32),
+                               n, t.root, _p(t.aabb, c_float))
+    return t

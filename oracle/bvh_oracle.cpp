@@ -21,6 +21,10 @@
 //   oracle_boxes          D7  step 4 "compute the bounding boxes of the internal nodes"
 //   oracle_query_*_tree   D8  range search with a STACK on {left,right}
 //   oracle_query_*_brute  D8  the plain definition: test every primitive
+//   oracle_nearest_*      D10 "perform an operation" (Alg. 1 L5): nearest primitive within the radius
+//   oracle_first_hit_*    D11 the same for rays: the primitive a ray enters first
+//   oracle_apetrei        Algorithm 3 run serially: Apetrei's node numbering (index = split)
+//   oracle_ropes_from / oracle_boxes_from   D6 / D7 on a hierarchy whose root is not node 0
 //
 // Parity pins (tests/test_oracle_*.py): P1 worked example reconstructed from PAPER.md:120/166,
 // P2 Algorithm 2, P3 invariants, P4 closed forms, P5 brute force, P6 numpy stable sort, P7 Morton
@@ -79,8 +83,8 @@ inline int highest_differing_bit(uint64_t cf, uint32_t f, uint64_t cl, uint32_t 
   return -1;
 }
 
-// D8 sphere-vs-box, exact association fixed in DESIGN.md.
-inline bool sphere_hits_box(const float c[3], float r, const float lo[3], const float hi[3]) {
+// D8 squared distance from a point to a box, exact association fixed in DESIGN.md.
+inline float sphere_d2(const float c[3], const float lo[3], const float hi[3]) {
   float s[3];
   for (int a = 0; a < 3; ++a) {
     float u = lo[a] - c[a];
@@ -90,6 +94,12 @@ inline bool sphere_hits_box(const float c[3], float r, const float lo[3], const 
   }
   float d2 = s[0] + s[1];
   d2 = d2 + s[2];
+  return d2;
+}
+
+// D8 sphere-vs-box.
+inline bool sphere_hits_box(const float c[3], float r, const float lo[3], const float hi[3]) {
+  float d2 = sphere_d2(c, lo, hi);
   float r2 = r * r;
   return d2 <= r2;
 }
@@ -108,7 +118,14 @@ inline bool box_hits_box(const float qlo[3], const float qhi[3], const float lo[
 // per axis with d != 0: inv = 1 / d, t1 = (lo - o) * inv, t2 = (hi - o) * inv, the ray's interval is clipped to
 // [min(t1,t2), max(t1,t2)]; per axis with d == 0 the ray never leaves the slab or never enters it: lo <= o <= hi
 // (closed, G12).  Hit iff the clipped interval is not empty (tn <= tf: touching counts).
+inline bool ray_enters_box(const float ray[8], const float lo[3], const float hi[3], float* t_enter);
 inline bool ray_hits_box(const float ray[8], const float lo[3], const float hi[3]) {
+  float t;
+  return ray_enters_box(ray, lo, hi, &t);
+}
+// ... and where the clipped interval starts (D11: the parameter at which the ray is inside all three slabs for the
+// first time, never less than tmin).
+inline bool ray_enters_box(const float ray[8], const float lo[3], const float hi[3], float* t_enter) {
   float tn = ray[6], tf = ray[7];
   for (int a = 0; a < 3; ++a) {
     const float o = ray[a], d = ray[3 + a];
@@ -126,6 +143,7 @@ inline bool ray_hits_box(const float ray[8], const float lo[3], const float hi[3
       tf = tf < tmax_a ? tf : tmax_a;
     }
   }
+  *t_enter = tn;
   return tn <= tf;
 }
 
@@ -257,10 +275,16 @@ void oracle_hierarchy(const uint64_t* sorted, int64_t n, int32_t* left, int32_t*
 // is in the left subtree of ... the nodes on the right-most path (including the root node) ... all
 // point to the sentinel".  Pre-order walk carrying that right child down.
 // rope has 2n-1 entries (unified index).  Works for n = 1 (single leaf = node 0).
+void oracle_ropes_from(const int32_t* left, const int32_t* right, int64_t n, int32_t root, int32_t* rope);
 void oracle_ropes(const int32_t* left, const int32_t* right, int64_t n, int32_t* rope) {
+  oracle_ropes_from(left, right, n, 0, rope);   // Karras numbering: "The root node is assigned index 0" PAPER.md:101
+}
+// The same walk from a root that is not node 0 (Apetrei numbering: "the root node is no longer guaranteed to be I_0,
+// and its index now needs to be stored in the hierarchy").
+void oracle_ropes_from(const int32_t* left, const int32_t* right, int64_t n, int32_t root, int32_t* rope) {
   const int32_t leaf_base = (int32_t)(n - 1);
   std::vector<std::pair<int32_t, int32_t>> stack;
-  stack.push_back({0, SENTINEL});
+  stack.push_back({n >= 2 ? root : 0, SENTINEL});
   while (!stack.empty()) {
     auto [node, r] = stack.back();
     stack.pop_back();
@@ -296,8 +320,14 @@ void oracle_ropes_alg2(const uint64_t* sorted, const int32_t* first, const int32
 
 // D7.  aabb[node][6] = {lo.xyz, hi.xyz}.  Leaf (n-1)+i = box of primitive perm[i]; internal =
 // component-wise min / max of its two children, post-order.
+void oracle_boxes_from(const float* prim, int is_box, const uint32_t* perm, const int32_t* left,
+                       const int32_t* right, int64_t n, int32_t root, float* aabb);
 void oracle_boxes(const float* prim, int is_box, const uint32_t* perm, const int32_t* left,
                   const int32_t* right, int64_t n, float* aabb) {
+  oracle_boxes_from(prim, is_box, perm, left, right, n, 0, aabb);
+}
+void oracle_boxes_from(const float* prim, int is_box, const uint32_t* perm, const int32_t* left,
+                       const int32_t* right, int64_t n, int32_t root, float* aabb) {
   const int32_t leaf_base = (int32_t)(n - 1);
   for (int64_t i = 0; i < n; ++i) {
     Box b = prim_box(prim, perm[i], is_box);
@@ -308,7 +338,7 @@ void oracle_boxes(const float* prim, int is_box, const uint32_t* perm, const int
   }
   if (n < 2) return;
   std::vector<std::pair<int32_t, int>> stack;  // (node, children_done)
-  stack.push_back({0, 0});
+  stack.push_back({root, 0});
   while (!stack.empty()) {
     auto [node, done] = stack.back();
     stack.pop_back();
@@ -427,6 +457,155 @@ void* oracle_query_boxes_brute(const float* prim, int64_t n, int is_box, const f
 
 void* oracle_query_rays_brute(const float* prim, int64_t n, int is_box, const float* rays, int64_t q) {
   return query_brute(2, prim, n, is_box, rays, q);
+}
+
+// ---- D10 / D11: "Store the result or perform an operation" (Alg. 1 L5) -----------------------------------
+// An operation at the leaf instead of a stored row.  Both are defined over the SAME candidate set as the range search
+// (the primitives whose box satisfies the predicate), so they are reductions of a CSR row, made unique by a tie rule.
+//
+// D10 nearest within the radius (sphere queries): among the primitives with d2 <= r*r (D8), the one with the smallest
+// d2; equal d2: the smallest original index.  idx[j] = that primitive or -1; d2[j] = its d2 or +infinity.
+// D11 first hit (ray queries): among the primitives whose box the ray hits (D9), the one the ray enters first
+// (smallest t_enter, the start of the clipped interval); equal t_enter: the smallest original index.
+// idx[j] = that primitive or -1; t[j] = its t_enter or +infinity.  "Any hit" is idx[j] >= 0.
+static inline float pos_inf() {
+  const uint32_t b = 0x7f800000u;
+  float f;
+  std::memcpy(&f, &b, 4);
+  return f;
+}
+
+static inline bool candidate(int kind, const float* queries, int64_t j, const float lo[3], const float hi[3], float* key) {
+  if (kind == 0) {
+    const float* s = queries + 4 * j;
+    *key = sphere_d2(s, lo, hi);
+    float r2 = s[3] * s[3];
+    return *key <= r2;
+  }
+  return ray_enters_box(queries + 8 * j, lo, hi, key);
+}
+
+// Brute force: the plain definition (every primitive is a candidate test).  kind 0 = spheres (D10), 2 = rays (D11).
+static void reduce_brute(int kind, const float* prim, int64_t n, int is_box, const float* queries, int64_t q,
+                         int32_t* idx, float* key_out) {
+  for (int64_t j = 0; j < q; ++j) {
+    int32_t best = -1;
+    float best_key = pos_inf();
+    for (int64_t i = 0; i < n; ++i) {      // ascending original index: a strict "<" keeps the smallest index on ties
+      Box b = prim_box(prim, i, is_box);
+      float key;
+      if (candidate(kind, queries, j, b.lo, b.hi, &key) && (best < 0 || key < best_key)) {
+        best = (int32_t)i;
+        best_key = key;
+      }
+    }
+    idx[j] = best;
+    key_out[j] = best_key;
+  }
+}
+
+// The same over the oracle's own tree (stack on {left, right}; no pruning beyond the predicate itself, so it visits
+// exactly the leaves the range search reports).
+static void reduce_tree(int kind, const float* aabb, const int32_t* left_child, const int32_t* right_child, int64_t n,
+                        const float* queries, int64_t q, int32_t* idx, float* key_out) {
+  const int32_t leaf_base = (int32_t)(n - 1);
+  std::vector<int32_t> stack;
+  for (int64_t j = 0; j < q; ++j) {
+    int32_t best = -1;
+    float best_key = pos_inf();
+    if (n > 0) {
+      stack.clear();
+      stack.push_back(0);
+      while (!stack.empty()) {
+        int32_t node = stack.back();
+        stack.pop_back();
+        const float* b = aabb + 6 * (int64_t)node;
+        float key;
+        if (!candidate(kind, queries, j, b, b + 3, &key)) continue;
+        if (node >= leaf_base) {
+          const int32_t prim_index = left_child[node];
+          if (best < 0 || key < best_key || (key == best_key && prim_index < best)) {
+            best = prim_index;
+            best_key = key;
+          }
+        } else {
+          stack.push_back(right_child[node]);
+          stack.push_back(left_child[node]);
+        }
+      }
+    }
+    idx[j] = best;
+    key_out[j] = best_key;
+  }
+}
+
+void oracle_nearest_spheres_brute(const float* prim, int64_t n, int is_box, const float* xyzr, int64_t q, int32_t* idx,
+                                  float* d2) {
+  reduce_brute(0, prim, n, is_box, xyzr, q, idx, d2);
+}
+void oracle_nearest_spheres_tree(const float* aabb, const int32_t* left_child, const int32_t* right_child, int64_t n,
+                                 const float* xyzr, int64_t q, int32_t* idx, float* d2) {
+  reduce_tree(0, aabb, left_child, right_child, n, xyzr, q, idx, d2);
+}
+void oracle_first_hit_rays_brute(const float* prim, int64_t n, int is_box, const float* rays, int64_t q, int32_t* idx,
+                                 float* t) {
+  reduce_brute(2, prim, n, is_box, rays, q, idx, t);
+}
+void oracle_first_hit_rays_tree(const float* aabb, const int32_t* left_child, const int32_t* right_child, int64_t n,
+                                const float* rays, int64_t q, int32_t* idx, float* t) {
+  reduce_tree(2, aabb, left_child, right_child, n, rays, q, idx, t);
+}
+
+// ---- Algorithm 3, "Apetrei's algorithm", run serially --------------------------------------------
+// The leaf "threads" run one after the other; a thread that finds store[p] empty (ATOMICCAS returned the invalid
+// value) stops, the second one to arrive carries on.  Internal nodes are numbered by their split
+// position p ("indexed using the split positions gamma"), both children write themselves into the parent
+// (L7, L13), and the root -- the node whose range is [0, n-1] -- is wherever the last merge happened: its index is
+// returned in *root.  delta* is the XOR magnitude of adjacent augmented keys (G1), compared through its
+// highest set bit; +infinity outside [0, n-2].  Unified child indices: I_p -> p, L_i -> (n-1)+i.  n >= 2.
+void oracle_apetrei(const uint64_t* sorted, int64_t n, int32_t* left, int32_t* right, int32_t* root) {
+  const int32_t leaf_base = (int32_t)(n - 1);
+  auto dstar = [&](int64_t i) -> int {
+    if (i < 0 || i >= n - 1) return 1000;
+    return highest_differing_bit(sorted[i], (uint32_t)i, sorted[i + 1], (uint32_t)(i + 1));
+  };
+  std::vector<int32_t> store((size_t)(n - 1), -1);                                    // L1
+  *root = -1;
+  for (int32_t leaf = 0; leaf < n; ++leaf) {                                          // L2
+    int32_t i = leaf;                                                                 // index of the current node
+    int32_t range_left = leaf, range_right = leaf;                                    // L3-4
+    int dl = dstar(range_left - 1), dr = dstar(range_right);
+    while (true) {
+      const bool is_leaf = range_left == range_right;
+      int32_t p;
+      if (dr < dl) {                                                                  // L5: left child of its parent
+        p = range_right;                                                              // L6: Apetrei index
+        left[p] = is_leaf ? leaf_base + i : i;                                        // L7
+        const int32_t old = store[p];                                                 // L8: ATOMICCAS
+        if (old == -1) {
+          store[p] = range_left;
+          break;                                                                      // L9
+        }
+        range_right = old;
+        dr = dstar(range_right);                                                      // L10
+      } else {                                                                        // L12: right child of its parent
+        p = range_left - 1;
+        right[p] = is_leaf ? leaf_base + i : i;                                       // L13
+        const int32_t old = store[p];                                                 // L14
+        if (old == -1) {
+          store[p] = range_right;
+          break;                                                                      // L15
+        }
+        range_left = old;
+        dl = dstar(range_left - 1);                                                   // L16
+      }
+      i = p;                                                                          // L18
+      if (range_left == 0 && range_right == n - 1) {                                  // L19: the range is everything
+        *root = p;
+        break;
+      }
+    }
+  }
 }
 
 int64_t oracle_result_nnz(void* h) { return (int64_t) static_cast<CsrResult*>(h)->indices.size(); }

@@ -474,3 +474,145 @@ def test_d9_ray_tree_equals_brute(oracle_lib, name, n, q):
     boff, bidx = oracle_lib.query_rays_brute(prims, rays)
     assert np.array_equal(toff, boff) and toff[-1] > q
     assert np.array_equal(csr_rows_sorted(toff, tidx), bidx)
+
+
+# ---- NEXT-2 (a): Algorithm 3, Apetrei's numbering ----------------------------------------------------------------
+
+def _renumber_karras_to_apetrei(o_left, o_right, o_last, n):
+    """Test-side renaming of a Karras-ordered tree: every internal node takes its split position as its index
+    (PAPER.md:164).  Returns (root, left, right) in unified indices."""
+    lb = n - 1
+    split = np.array([(o_left[k] - lb) if o_left[k] >= lb else o_last[o_left[k]] for k in range(n - 1)], np.int64)
+    ren = lambda c: c if c >= lb else split[c]  # noqa: E731
+    left, right = np.empty(n - 1, np.int32), np.empty(n - 1, np.int32)
+    for k in range(n - 1):
+        left[split[k]] = ren(o_left[k])
+        right[split[k]] = ren(o_right[k])
+    assert sorted(split.tolist()) == list(range(n - 1))       # every boundary is the split of exactly one node
+    return int(split[0]), left, right, split
+
+
+def test_apetrei_p1_numbering(oracle_lib):
+    """Algorithm 3 on the worked example: the root's children sit at 1 and 4, a gap of 3."""
+    g = {ln.split()[0]: [int(x) for x in ln.split()[1:]] for ln in _read_gold("p1_apetrei_numbering.txt")}
+    keys = _p1()["keys"]
+    pts = np.zeros((8, 3), np.float32)                         # boxes are not looked at here
+
+    class O:                                                   # the part of a Bvh that apetrei_tree reads
+        sorted_codes = keys
+        perm = np.arange(8, dtype=np.uint32)
+
+    t = oracle_lib.apetrei_tree(pts, O)
+    assert t.root == g["root"][0] == 3
+    assert list(t.left) == g["left"] and list(t.right) == g["right"]
+    assert list(t.rope) == g["rope"]
+    assert (t.left[t.root], t.right[t.root]) == (1, 4) and t.right[t.root] - t.left[t.root] == 3
+
+
+@pytest.mark.parametrize("kind", ["distinct", "ties", "wide", "equal"])
+def test_apetrei_equals_renumbered_karras(oracle_lib, kind):
+    """Karras' and Apetrei's constructions "result in an identical hierarchy structure"; only the node
+    indices differ.  Algorithm 3 run serially = the top-down tree with every node renamed to its split."""
+    rng = np.random.default_rng(17)
+    for n in (2, 3, 5, 8, 33, 257, 2000):
+        codes = _random_sorted_codes(rng, n, kind)
+        left, right, first, last = oracle_lib.hierarchy(codes)
+        root, a_left, a_right, split = _renumber_karras_to_apetrei(left, right, last, n)
+        class O:
+            sorted_codes = codes
+            perm = np.arange(n, dtype=np.uint32)
+
+        pts = rng.random((n, 3)).astype(np.float32)
+        t = oracle_lib.apetrei_tree(pts, O)
+        assert t.root == root and np.array_equal(t.left, a_left) and np.array_equal(t.right, a_right), (kind, n)
+        # skip-connections and boxes: the Karras tree's, renamed
+        rope_k = oracle_lib.ropes(left, right, n)
+        box_k = oracle_lib.boxes(pts, O.perm, left, right)
+        lb = n - 1
+        ren = lambda c: c if (c >= lb or c < 0) else split[c]  # noqa: E731
+        for k in range(n - 1):
+            assert t.rope[split[k]] == ren(rope_k[k])
+            assert np.array_equal(t.aabb[split[k]], box_k[k])
+        assert np.array_equal(t.rope[lb:], np.array([ren(c) for c in rope_k[lb:]], np.int32))
+        assert np.array_equal(t.aabb[lb:], box_k[lb:])
+
+
+# ---- D10 / D11: operations at the leaf (PAPER.md:56) -----------------------------------------------------------------
+
+def test_d10_nearest_closed_forms(oracle_lib):
+    """Cases whose answer is known by inspection (coordinates and radii are dyadic: every fp32 step is exact)."""
+    f = np.float32
+    pts = np.array([[0, 0, 0], [1, 0, 0], [3, 0, 0], [1, 0, 0]], f)           # primitives 1 and 3 coincide
+    qs = np.array([
+        [0.875, 0, 0, 1.0],      # nearest is primitive 1 (d2 = 1/64); 3 is as near: the smaller index wins
+        [0.5, 0, 0, 1.0],        # 0 and 1 (and 3) at d2 = 1/4: smallest index 0
+        [2.0, 0, 0, 0.125],      # nothing within the radius
+        [2.0, 0, 0, 1.0],        # primitives 1, 2, 3 exactly AT the radius (closed, G12): smallest index 1
+        [3.0, 0.5, 0, 0.5],      # only primitive 2, at the radius
+        [0, 0, 0, 0.0],          # zero radius on a primitive: d2 = 0 <= 0
+    ], f)
+    idx, d2 = oracle_lib.nearest_spheres_brute(pts, qs)
+    assert idx.tolist() == [1, 0, -1, 1, 2, 0]
+    assert d2[[0, 1, 3, 4, 5]].tolist() == [1 / 64, 0.25, 1.0, 0.25, 0.0] and np.isposinf(d2[2])
+    # box primitives: distance to the box, not to its centre
+    boxes = np.array([[0, 0, 0, 1, 1, 1], [2, 0, 0, 4, 1, 1]], f)
+    idx, d2 = oracle_lib.nearest_spheres_brute(boxes, np.array([[1.5, 0.5, 0.5, 1], [1.75, 0.5, 0.5, 1], [0.5, 0.5, 0.5, 0]], f))
+    assert idx.tolist() == [0, 1, 0] and d2.tolist() == [0.25, 1 / 16, 0.0]
+
+
+@pytest.mark.parametrize("name,n,q", [("C1", 4096, 300), ("C3", 30000, 300), ("C4", 20000, 300)])
+def test_d10_nearest_tree_equals_brute_and_is_the_row_minimum(oracle_lib, name, n, q):
+    w = W.make(name, n=n, q=q, radius=(0.02 if name == "C4" else None))
+    spheres = w.queries if w.queries.shape[1] == 4 else W.spheres_at(w.queries[:, :3], 0.02)
+    o = oracle_lib.build_bvh(w.prims, w.morton_bits)
+    bi, bd = oracle_lib.nearest_spheres_brute(w.prims, spheres)
+    ti, td = oracle_lib.nearest_spheres_tree(o, spheres)
+    assert np.array_equal(bi, ti) and np.array_equal(bd.view(np.uint32), td.view(np.uint32))
+    # the definition again, in numpy on the CSR rows of the range search: minimum of (d2, index) over the row
+    off, idx = oracle_lib.query_spheres_brute(w.prims, spheres)
+    prim6 = w.prims if w.prims.shape[1] == 6 else np.concatenate([w.prims, w.prims], axis=1)
+    some = 0
+    for j in range(q):
+        row = idx[off[j]:off[j + 1]]
+        if len(row) == 0:
+            assert bi[j] == -1 and np.isposinf(bd[j])
+            continue
+        c = spheres[j, :3]
+        d = np.maximum(np.maximum(prim6[row, :3] - c, c - prim6[row, 3:]), np.float32(0))
+        s = d * d
+        d2 = (s[:, 0] + s[:, 1]) + s[:, 2]
+        k = np.lexsort((row, d2))[0]
+        assert bi[j] == row[k] and bd[j] == d2[k]
+        some += 1
+    assert some > q // 2
+
+
+def test_d11_first_hit_closed_forms(oracle_lib):
+    f = np.float32
+    boxes = np.array([[4, -1, -1, 5, 1, 1], [1, -1, -1, 2, 1, 1], [1, -1, -1, 3, 1, 1], [7, 2, 2, 8, 3, 3]], f)
+    rays = np.array([
+        [0, 0, 0, 1, 0, 0, 0, 100],        # enters boxes 1 and 2 at t = 1 (smaller index wins), box 0 at t = 4
+        [0, 0, 0, 1, 0, 0, 2.5, 100],      # tmin inside box 2 only: t_enter = tmin = 2.5; box 1 is behind, box 0 at 4
+        [6, 0, 0, -1, 0, 0, 0, 100],       # from the other side: box 0 first, at t = 1
+        [0, 0, 0, 1, 0, 0, 0, 0.5],        # too short
+        [0, 5, 0, 1, 0, 0, 0, 100],        # misses everything
+        [0, 0, 0, 2, 0, 0, 0, 100],        # direction not normalised: t in units of |d|: box 1 at t = 0.5
+        [1.5, 0, 0, 0, 0, 1, 0, 100],      # starts inside boxes 1 and 2, parallel to two slabs: t_enter = tmin = 0
+    ], f)
+    idx, t = oracle_lib.first_hit_rays_brute(boxes, rays)
+    assert idx.tolist() == [1, 2, 0, -1, -1, 1, 1]
+    assert t[[0, 1, 2, 5, 6]].tolist() == [1.0, 2.5, 1.0, 0.5, 0.0] and np.isposinf(t[3]) and np.isposinf(t[4])
+
+
+@pytest.mark.parametrize("name,n,q", [("C2", 30000, 300), ("C4", 30000, 300)])
+def test_d11_first_hit_tree_equals_brute_and_is_the_row_minimum(oracle_lib, name, n, q):
+    prims, rays = _ray_case(name, n, q)
+    o = oracle_lib.build_bvh(prims, 63)
+    bi, bt = oracle_lib.first_hit_rays_brute(prims, rays)
+    ti, tt = oracle_lib.first_hit_rays_tree(o, rays)
+    assert np.array_equal(bi, ti) and np.array_equal(bt.view(np.uint32), tt.view(np.uint32))
+    off, idx = oracle_lib.query_rays_brute(prims, rays)
+    assert np.array_equal(bi >= 0, np.diff(off) > 0)                      # "any hit" = the row is not empty
+    for j in range(q):                                                     # the winner is a member of the row
+        assert bi[j] == -1 or bi[j] in idx[off[j]:off[j + 1]]
+    assert (bi >= 0).sum() > 10
