@@ -156,6 +156,26 @@ int bvh_query_rays_count(const void* nodes, int64_t n, const float* rays, int64_
 int bvh_query_rays_fill(const void* nodes, int64_t n, const float* rays, int64_t q, const uint32_t* order,
                         const int64_t* offsets, int32_t* indices, void* stream);
 
+/* NEXT-1, second half: "Store the result or perform an operation" (Algorithm 1 L5).  Operations that
+ * replace the stored row; same kernel, same walk, no CSR, one call.  Each is a reduction over the set of primitives the
+ * range search would report, made unique by a tie rule on the ORIGINAL primitive index.
+ *   bvh_query_spheres_nearest (D10)  index[j] = the primitive with the smallest squared distance d2 (the D8 arithmetic)
+ *       among those with d2 <= r*r; equal d2: the smallest index; -1 if there is none.  d2[j] = that distance, +infinity
+ *       if none.  The radius shrinks to the best distance found so far, so the walk prunes as it goes.
+ *   bvh_query_rays_first_hit (D11)   index[j] = the primitive whose box the ray enters first: smallest t_enter, the
+ *       start of the clipped interval of D9 (never less than tmin; a ray that starts inside a box enters it at tmin);
+ *       equal t_enter: the smallest index; -1 if none.  t[j] = that parameter, +infinity if none.
+ *   bvh_query_any_hit                hit[j] = 1 if some primitive satisfies the predicate of query j, else 0
+ *       (query_kind 0 spheres, 1 boxes, 2 rays); the walk of a query stops at its first hit.
+ * index, hit: int32[q]; d2, t: float[q]; `order` and the n = 0 / q = 0 behaviour as in the count calls (n = 0:
+ * index = -1, keys = +infinity, hit = 0). */
+int bvh_query_spheres_nearest(const void* nodes, int64_t n, const float* xyzr, int64_t q, const uint32_t* order,
+                              int32_t* index, float* d2, void* stream);
+int bvh_query_rays_first_hit(const void* nodes, int64_t n, const float* rays, int64_t q, const uint32_t* order,
+                             int32_t* index, float* t, void* stream);
+int bvh_query_any_hit(const void* nodes, int64_t n, const float* queries, int query_kind, int64_t q,
+                      const uint32_t* order, int32_t* hit, void* stream);
+
 /* NEXT-2: a MEASUREMENT variant of the build, not a product path.  variant = 1 replaces the last step
  * (the single bottom-up pass of Algorithm 4) by what the paper compares itself with: Karras' top-down construction,
  * one thread per internal node searching its range and split on the common-prefix length of the augmented keys

@@ -45,6 +45,9 @@ SYMBOLS = {
     "bvh_scan_counts": [_P, c_int64, _P, _P, c_size_t, _P],
     "bvh_query_spheres_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
     "bvh_query_boxes_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
+    "bvh_query_spheres_nearest": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
+    "bvh_query_rays_first_hit": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
+    "bvh_query_any_hit": [_P, c_int64, _P, c_int, c_int64, _P, _P, _P],
     "bvh_query_collect": [_P, c_int64, _P, c_int, c_int64, _P, c_int64, _P, _P, _P],
     "bvh_rows_to_csr": [_P, c_int64, _P, _P, c_int64, _P, _P],
     "bvh_query_fill_overflow": [_P, c_int64, _P, c_int, c_int64, _P, c_int64, _P, _P, _P, _P],
@@ -161,6 +164,21 @@ def bvh_query_spheres_count(nodes, n: int, xyzr, q: int, order, counts) -> None:
 def bvh_query_boxes_count(nodes, n: int, minmax, q: int, order, counts) -> None:
     _check(load_library().bvh_query_boxes_count(_ptr(nodes), n, _ptr(minmax), q, _ptr(order), _ptr(counts), _stream()),
            "bvh_query_boxes_count")
+
+
+def bvh_query_spheres_nearest(nodes, n: int, xyzr, q: int, order, index, d2) -> None:
+    _check(load_library().bvh_query_spheres_nearest(_ptr(nodes), n, _ptr(xyzr), q, _ptr(order), _ptr(index), _ptr(d2),
+                                                    _stream()), "bvh_query_spheres_nearest")
+
+
+def bvh_query_rays_first_hit(nodes, n: int, rays, q: int, order, index, t) -> None:
+    _check(load_library().bvh_query_rays_first_hit(_ptr(nodes), n, _ptr(rays), q, _ptr(order), _ptr(index), _ptr(t),
+                                                   _stream()), "bvh_query_rays_first_hit")
+
+
+def bvh_query_any_hit(nodes, n: int, queries, query_kind: int, q: int, order, hit) -> None:
+    _check(load_library().bvh_query_any_hit(_ptr(nodes), n, _ptr(queries), query_kind, q, _ptr(order), _ptr(hit),
+                                            _stream()), "bvh_query_any_hit")
 
 
 def bvh_query_collect(nodes, n: int, queries, query_kind: int, q: int, order, cap: int, rows, counts) -> None:
@@ -344,3 +362,33 @@ def query(bvh: Bvh, queries: torch.Tensor, ws: QueryWorkspace | None = None, ind
         fill(bvh.nodes, bvh.n, queries, q, order, ws.offsets, indices)
     offsets = ws.offsets[: q + 1]
     return offsets, (indices if nnz is None else indices[:nnz])
+
+
+def reduce_query(bvh: Bvh, queries: torch.Tensor, op: str, ws: QueryWorkspace | None = None, ordered: bool = True):
+    """"Perform an operation" at the leaves instead of storing rows.  op = "nearest" (spheres: index and
+    squared distance of the nearest primitive within the radius), "first_hit" (rays: index and entry parameter of the
+    first box the ray enters) or "any_hit" (any query kind: 0 / 1).  Returns device tensors."""
+    q = int(queries.shape[0])
+    if bvh.prim_kind is None:
+        raise BvhError("reduce_query() on a Bvh that has not been built")
+    if queries.dtype != torch.float32 or queries.dim() != 2 or int(queries.shape[1]) not in QUERY_KINDS:
+        raise BvhError(f"expected float32 [q,4], [q,6] or [q,8], got {queries.dtype} {tuple(queries.shape)}")
+    kind = QUERY_KINDS[int(queries.shape[1])]
+    ws = ws or QueryWorkspace(q, queries.device)
+    order = None
+    if ordered and q > 0:
+        (bvh_query_order_spheres, bvh_query_order_boxes, bvh_query_order_rays)[kind](bvh.nodes, bvh.n, queries, q, ws.order,
+                                                                                   ws.order_scratch)
+        order = ws.order
+    index = torch.empty(max(q, 1), dtype=torch.int32, device=queries.device)
+    if op == "any_hit":
+        bvh_query_any_hit(bvh.nodes, bvh.n, queries, kind, q, order, index)
+        return index[:q]
+    key = torch.empty(max(q, 1), dtype=torch.float32, device=queries.device)
+    if op == "nearest" and kind == 0:
+        bvh_query_spheres_nearest(bvh.nodes, bvh.n, queries, q, order, index, key)
+    elif op == "first_hit" and kind == 2:
+        bvh_query_rays_first_hit(bvh.nodes, bvh.n, queries, q, order, index, key)
+    else:
+        raise BvhError(f"operation {op!r} is not defined for {tuple(queries.shape)} queries")
+    return index[:q], key[:q]

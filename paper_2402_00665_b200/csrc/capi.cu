@@ -183,9 +183,17 @@ static inline bool misaligned32(const void* p) { return (reinterpret_cast<uintpt
 // mode: kModeCount / kModeFill / kModeCollect of traverse.cu (0 / 1 / 2).  cap: collect: entries per row; fill with
 // only_over: rows with counts[j] > cap.  Whether `nodes` holds a finished hierarchy over n primitives is checked on the
 // device (NodesHeader), since the library may not synchronise: a stale buffer yields counts of 0 and no stores.
+__global__ void fill_reduce_none_kernel(int32_t* index, float* keys, int64_t q) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < q) {
+    index[i] = -1;
+    keys[i] = __int_as_float(0x7f800000);
+  }
+}
+
 static int query(const void* nodes, int64_t n, const float* queries, int64_t q, int kind, int mode,
                  const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* out, int64_t cap, bool only_over,
-                 void* stream_) {
+                 void* stream_, float* keys = nullptr) {
   if (n < 0 || q < 0) return BVH_ERR_INVALID_ARGUMENT;
   if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
   if (kind < 0 || kind > 2) return BVH_ERR_INVALID_ARGUMENT;
@@ -197,7 +205,12 @@ static int query(const void* nodes, int64_t n, const float* queries, int64_t q, 
     if (!counts) return BVH_ERR_INVALID_ARGUMENT;
   }
   if (mode == 2 && (cap < 8 || cap % 8 != 0 || cap > 0x7fffffff || !out || misaligned32(out))) return BVH_ERR_INVALID_ARGUMENT;
+  if (mode == 3 && (!keys || kind == 1)) return BVH_ERR_INVALID_ARGUMENT;
   if (n == 0) {
+    if (mode == 3) {
+      fill_reduce_none_kernel<<<(unsigned)((q + 255) / 256), 256, 0, stream>>>(counts, keys, q);
+      return check_launch();
+    }
     if (mode != 1) {
       zero_counts_kernel<<<(unsigned)((q + 255) / 256), 256, 0, stream>>>(counts, q);
       return check_launch();
@@ -207,7 +220,7 @@ static int query(const void* nodes, int64_t n, const float* queries, int64_t q, 
   // node records are read with 256-bit loads: 32-byte alignment
   if (!nodes || !queries || misaligned32(nodes) || misaligned(queries)) return BVH_ERR_INVALID_ARGUMENT;
   if (mode == 1 && !out) return BVH_ERR_INVALID_ARGUMENT;  // nnz = 0 callers still pass a valid pointer
-  if (launch_traverse(nodes, (int)n, queries, q, kind, mode, order, counts, offsets, out, cap, only_over, stream) != cudaSuccess)
+  if (launch_traverse(nodes, (int)n, queries, q, kind, mode, order, counts, offsets, out, cap, only_over, keys, stream) != cudaSuccess)
     return BVH_ERR_CUDA;
   return BVH_OK;
 }
@@ -354,6 +367,21 @@ int bvh_query_spheres_fill(const void* nodes, int64_t n, const float* xyzr, int6
 int bvh_query_boxes_fill(const void* nodes, int64_t n, const float* minmax, int64_t q, const uint32_t* order,
                          const int64_t* offsets, int32_t* indices, void* stream) {
   return bvh::query(nodes, n, minmax, q, 1, 1, order, nullptr, offsets, indices, 0, false, stream);
+}
+
+int bvh_query_spheres_nearest(const void* nodes, int64_t n, const float* xyzr, int64_t q, const uint32_t* order,
+                              int32_t* index, float* d2, void* stream) {
+  return bvh::query(nodes, n, xyzr, q, 0, 3, order, index, nullptr, nullptr, 0, false, stream, d2);
+}
+
+int bvh_query_rays_first_hit(const void* nodes, int64_t n, const float* rays, int64_t q, const uint32_t* order,
+                             int32_t* index, float* t, void* stream) {
+  return bvh::query(nodes, n, rays, q, 2, 3, order, index, nullptr, nullptr, 0, false, stream, t);
+}
+
+int bvh_query_any_hit(const void* nodes, int64_t n, const float* queries, int query_kind, int64_t q, const uint32_t* order,
+                      int32_t* hit, void* stream) {
+  return bvh::query(nodes, n, queries, q, query_kind, 4, order, hit, nullptr, nullptr, 0, false, stream);
 }
 
 int bvh_query_collect(const void* nodes, int64_t n, const float* queries, int query_kind, int64_t q, const uint32_t* order,

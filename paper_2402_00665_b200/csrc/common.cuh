@@ -170,11 +170,12 @@ int launch_variant_karras(const float* prim, bool is_box, const void* sorted_cod
                           void* nodes, int n, const Header* header, void* extra, cudaStream_t stream);
 // K6/K8: stackless traversal.  kind 0 = spheres (xyzr), 1 = boxes (minmax), 2 = rays (o.xyz, d.xyz, tmin, tmax).
 // mode 0 = count (counts out), 1 = fill (offsets in, out = indices; only_over: only rows with counts[j] > cap),
-// 2 = collect (out = rows of cap entries, counts out).
+// 2 = collect (out = rows of cap entries, counts out), 3 = reduce (counts = primitive with the smallest key, keys out;
+// spheres and rays), 4 = any hit (counts = 0 / 1).
 // order (optional): thread t serves query order[t] (results still land in row order[t]).
 cudaError_t launch_traverse(const void* nodes, int n, const float* queries, int64_t q, int kind, int mode,
                             const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* out, int64_t cap,
-                            bool only_over, cudaStream_t stream);
+                            bool only_over, float* keys, cudaStream_t stream);
 cudaError_t launch_rows_to_csr(const int32_t* rows, int64_t cap, const int32_t* counts, const int64_t* offsets, int64_t q,
                                int32_t* indices, cudaStream_t stream);
 int sm_count();   // multiprocessors of the current device (cached)

@@ -61,6 +61,7 @@ __device__ __forceinline__ NodeRec load_rec(const Node* __restrict__ p) {
 }
 
 struct SphereQuery {
+  static constexpr bool kHasKey = true;                    // D10: candidates are ranked by their distance
   static constexpr int kWords = 4;
   static constexpr int kCtasPerSm = kTravCtasPerSm;
   float cx, cy, cz, r2;
@@ -95,6 +96,21 @@ struct SphereQuery {
   // the predicate: per axis its distance term max(max(B.lo - c, c - B.hi), 0) <= f because B.lo <= hi, B.hi >= lo and
   // round-to-nearest subtraction is monotone (and f >= 0 since lo <= hi); squaring non-negatives and rounded addition
   // are monotone too, so d2(B) <= F2 <= r*r -- the argument SURVEY.md 8(c) D8 uses for "a hit leaf has hit ancestors".
+  // D10 (nearest within the radius): the key of a candidate is its D8 distance; a found candidate shrinks the radius
+  // to its distance (closed comparisons keep candidates at the same distance in play for the index tie rule).
+  __device__ __forceinline__ bool cand_box(float lox, float loy, float loz, float hix, float hiy, float hiz, float& key) const {
+    const float dx = fmaxf(fmaxf(__fsub_rn(lox, cx), __fsub_rn(cx, hix)), 0.0f);
+    const float dy = fmaxf(fmaxf(__fsub_rn(loy, cy), __fsub_rn(cy, hiy)), 0.0f);
+    const float dz = fmaxf(fmaxf(__fsub_rn(loz, cz), __fsub_rn(cz, hiz)), 0.0f);
+    key = __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+    return key <= r2;
+  }
+  __device__ __forceinline__ bool cand_point(float x, float y, float z, float& key) const {
+    const float dx = fabsf(__fsub_rn(x, cx)), dy = fabsf(__fsub_rn(y, cy)), dz = fabsf(__fsub_rn(z, cz));
+    key = __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+    return key <= r2;
+  }
+  __device__ __forceinline__ void shrink(float key) { r2 = key; }
   __device__ __forceinline__ float extent() const { return 2.0f * sqrtf(r2); }   // only gates the shortcut: any value is safe
   __device__ __forceinline__ bool contains_box(float lox, float loy, float loz, float hix, float hiy, float hiz) const {
     const float fx = fmaxf(__fsub_rn(cx, lox), __fsub_rn(hix, cx));
@@ -106,6 +122,7 @@ struct SphereQuery {
 };
 
 struct BoxQuery {
+  static constexpr bool kHasKey = false;                   // overlap has no ranking: count / fill / any only
   static constexpr int kWords = 6;
   static constexpr int kCtasPerSm = kTravCtasPerSm;
   float lo[3], hi[3];
@@ -146,6 +163,7 @@ struct BoxQuery {
 #define BVH_TRAV_CTAS_RAYS 6
 #endif
 struct RayQuery {
+  static constexpr bool kHasKey = true;                    // D11: candidates are ranked by where the ray enters them
   static constexpr int kWords = 8;
   static constexpr int kCtasPerSm = BVH_TRAV_CTAS_RAYS;   // the ray state does not fit the 64 registers of 8 CTAs per SM
   float o[3], inv[3], tmin, tmax;
@@ -181,6 +199,15 @@ struct RayQuery {
     par = reinterpret_cast<const uint32_t*>(slot)[8];
   }
   __device__ __forceinline__ bool hit_box(float lox, float loy, float loz, float hix, float hiy, float hiz) const {
+    float key;
+    return cand_box(lox, loy, loz, hix, hiy, hiz, key);
+  }
+  // D11 (first hit): the key of a candidate is where the clipped interval starts; a found candidate shortens the
+  // segment to end there (tmax is only the start value of the interval's end, so the entry parameters of the boxes
+  // still in play do not change, and boxes entered at the same parameter stay in play for the index tie rule).
+  __device__ __forceinline__ void shrink(float key) { tmax = key; }
+  __device__ __forceinline__ bool cand_point(float x, float y, float z, float& key) const { return cand_box(x, y, z, x, y, z, key); }
+  __device__ __forceinline__ bool cand_box(float lox, float loy, float loz, float hix, float hiy, float hiz, float& key) const {
     const float lo[3] = {lox, loy, loz}, hi[3] = {hix, hiy, hiz};
     float tn = tmin, tf = tmax;
     bool ok = true;
@@ -195,6 +222,7 @@ struct RayQuery {
         tf = fminf(tf, fmaxf(t1, t2));
       }
     }
+    key = tn;
     return ok && (tn <= tf);
   }
   __device__ __forceinline__ bool hit_point(float x, float y, float z) const { return hit_box(x, y, z, x, y, z); }
@@ -215,6 +243,8 @@ struct LeafRec<true> {
   __device__ __forceinline__ uint32_t payload() const { return __float_as_uint(v.w); }
   template <typename Query>
   __device__ __forceinline__ bool hit(const Query& q) const { return q.hit_point(v.x, v.y, v.z); }
+  template <typename Query>
+  __device__ __forceinline__ bool cand(const Query& q, float& key) const { return q.cand_point(v.x, v.y, v.z, key); }
 };
 template <>
 struct LeafRec<false> {
@@ -225,6 +255,8 @@ struct LeafRec<false> {
   __device__ __forceinline__ uint32_t payload() const { return (uint32_t)r.left; }
   template <typename Query>
   __device__ __forceinline__ bool hit(const Query& q) const { return q.hit_box(r.lox, r.loy, r.loz, r.hix, r.hiy, r.hiz); }
+  template <typename Query>
+  __device__ __forceinline__ bool cand(const Query& q, float& key) const { return q.cand_box(r.lox, r.loy, r.loz, r.hix, r.hiy, r.hiz, key); }
 };
 
 #ifndef BVH_SCAN_UNROLL
@@ -237,7 +269,11 @@ struct LeafRec<false> {
 //   kModeCollect  single-pass variant: store it in the query's own slice of `cap` entries of a
 //                 caller-provided buffer (rows + query * cap; hits past cap are dropped) AND count it, so that one
 //                 traversal yields counts and, for every row that fits, its content.
-enum { kModeCount = 0, kModeFill = 1, kModeCollect = 2 };
+//   kModeReduce   "perform an operation" (NEXT-1): keep the candidate with the smallest key -- its D8 distance for sphere
+//                 queries (D10, nearest within the radius), the parameter at which the ray enters its box for rays (D11,
+//                 first hit) -- smallest primitive index among equal keys; the query shrinks as candidates are found.
+//   kModeAny      "any hit": 1 if some leaf satisfies the predicate, found or not; the walk stops at the first one.
+enum { kModeCount = 0, kModeFill = 1, kModeCollect = 2, kModeReduce = 3, kModeAny = 4 };
 
 struct TraverseArgs {
   const char* nodes;
@@ -245,7 +281,8 @@ struct TraverseArgs {
   const float* queries;
   int64_t q;
   const uint32_t* order;     // optional: thread t serves query order[t]
-  int32_t* counts;           // count, collect: out.  fill with only_over: in
+  int32_t* counts;           // count, collect: out.  fill with only_over: in.  reduce: primitive index out; any: flag out
+  float* keys;               // reduce: key of that primitive (d2 / t_enter), +infinity if none
   const int64_t* offsets;    // fill
   int32_t* out;              // fill: indices; collect: rows
   int64_t cap;               // collect: entries per row.  fill with only_over: only rows with counts[j] > cap are filled
@@ -306,9 +343,12 @@ struct TravSmem {
   int buf[STORE ? (kTravThreads / 32) * kRangeBufInts : 1];
 };
 
+__host__ __device__ constexpr bool mode_stores(int mode) { return mode == kModeFill || mode == kModeCollect; }
+
 template <typename Query, int MODE, bool POINT_LEAF>
-__device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Query, MODE != kModeCount>& S) {
-  constexpr bool STORE = MODE != kModeCount;
+__device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Query, mode_stores(MODE)>& S) {
+  constexpr bool STORE = mode_stores(MODE);
+  constexpr bool REDUCE = MODE == kModeReduce, ANY = MODE == kModeAny;
   constexpr int U = POINT_LEAF ? BVH_SCAN_UNROLL : (BVH_SCAN_UNROLL > 2 ? 2 : BVH_SCAN_UNROLL);   // leaf loads in flight per lane
   float* const s_query = S.query;
   int2* const s_range = S.range;
@@ -356,7 +396,9 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
     // The containment test is only worth its instructions for queries that can contain a subtree of kContainMinLeaves
     // leaves at all; warps whose 32 queries are all smaller than the typical box of such a subtree skip it (a
     // heuristic gate: it changes which nodes are tested for containment, never a result).
-    const bool try_contain = kContainment && !STORE && __any_sync(0xffffffffu, have && query.extent() >= contain_extent);
+    const bool try_contain = kContainment && MODE == kModeCount && __any_sync(0xffffffffu, have && query.extent() >= contain_extent);
+    float best_key = __int_as_float(0x7f800000);             // reduce: key and primitive of the best candidate so far
+    int best_idx = -1;
     int count = 0;
     int node = have ? 0 : kSentinel;                         // L1: start from the root
     int first = 0;                                           // first leaf below `node`
@@ -379,6 +421,58 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
         oq.from_shared(s_query + (warp_first + o) * Query::kSlotWords);
         const int2 range = s_range[warp_first + o];
         const int end = range.y;
+        if constexpr (REDUCE) {
+          // the best candidate of the range: smallest key, then smallest primitive index (two warp reductions per step)
+          uint32_t rk = 0xFFFFFFFFu;                       // order-preserving image of the key; all ones: none
+          int ri = 0x7fffffff;
+          for (int c = range.x + lane; c < end + lane; c += 32) {
+            LeafRec<POINT_LEAF> leaf;
+            float key = 0.0f;
+            bool hit = false;
+            if (c < end) {
+              leaf.load(leaves, c);
+              hit = leaf.cand(oq, key);
+            }
+            const uint32_t kb = hit ? float_to_ordered(key) : 0xFFFFFFFFu;
+            const uint32_t kmin = __reduce_min_sync(0xffffffffu, kb);
+            if (kmin != 0xFFFFFFFFu && kmin <= rk) {       // warp-uniform
+              const int ci = (hit && kb == kmin) ? (int)(leaf.payload() & kLeafPrimMask) : 0x7fffffff;
+              const int imin = __reduce_min_sync(0xffffffffu, ci);
+              if (kmin < rk || imin < ri) {
+                rk = kmin;
+                ri = imin;
+              }
+            }
+          }
+          if (lane == o && rk != 0xFFFFFFFFu) {
+            const float k = ordered_to_float(rk);
+            if (best_idx < 0 || k < best_key || (k == best_key && ri < best_idx)) {
+              best_key = k;
+              best_idx = ri;
+              query.shrink(k);
+              query.to_shared(s_query + threadIdx.x * Query::kSlotWords);
+            }
+          }
+          __syncwarp();
+          continue;
+        }
+        if constexpr (ANY) {
+          bool found = false;
+          for (int c = range.x + lane; c < end + lane && !found; c += 32) {
+            LeafRec<POINT_LEAF> leaf;
+            bool hit = false;
+            if (c < end) {
+              leaf.load(leaves, c);
+              hit = leaf.hit(oq);
+            }
+            found = __any_sync(0xffffffffu, hit);
+          }
+          if (lane == o && found) {
+            count = 1;
+            node = kSentinel;                              // nothing more to learn for this query
+          }
+          continue;
+        }
         int ocount = 0;                                    // count: this lane's hits; store: entries in `buf`
         int32_t* orow = nullptr;
         int p0 = 0, oalign = 0;
@@ -443,13 +537,24 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
         }
       }
       // ---- WALK, second half: one step of Algorithm 1 per lane ---------------------------------------------------
-      if (walking) {
+      if (walking && !(ANY && count != 0)) {               // (any hit: a lane whose scan just found one is done)
         if (!at_internal) {                                  // a single leaf (reached as a child or through a rope)
           const int i = node - leaf_base;
           LeafRec<POINT_LEAF> leaf;
           leaf.load(leaves, i);
           const uint32_t payload = leaf.payload();
-          if (leaf.hit(query)) {                             // L3-5
+          if constexpr (REDUCE) {
+            float key;
+            if (leaf.cand(query, key)) {                     // L3-5, "perform an operation"
+              const int pi = (int)(payload & kLeafPrimMask);
+              if (best_idx < 0 || key < best_key || (key == best_key && pi < best_idx)) {
+                best_key = key;
+                best_idx = pi;
+                query.shrink(key);
+                query.to_shared(s_query + threadIdx.x * Query::kSlotWords);
+              }
+            }
+          } else if (leaf.hit(query)) {                      // L3-5
             if (STORE && kFillStage != 2) {
               if (count < cap) row[count] = (int)(payload & kLeafPrimMask);
             } else if (STORE) {
@@ -470,6 +575,7 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
           }
           // L6: N_skip of leaf i (Algorithm 2): leaf i+1 or internal node i+1, one bit in the record
           node = (i == n - 1) ? kSentinel : ((payload & kLeafRopeInternal) ? i + 1 : leaf_base + i + 1);
+          if (ANY && count) node = kSentinel;
           first = i + 1;
         } else {
           const int rope = rec.rope;
@@ -500,7 +606,14 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
       for (int e = 0; e < carry; ++e)
         if (count - carry + e < cap) row[count - carry + e] = st[e];
     }
-    if (MODE != kModeFill && have) A.counts[j] = count;
+    if constexpr (REDUCE) {
+      if (have) {
+        A.counts[j] = best_idx;
+        A.keys[j] = best_key;
+      }
+    } else if (MODE != kModeFill && have) {
+      A.counts[j] = count;
+    }
   }
 }
 
@@ -514,11 +627,13 @@ __global__ void __launch_bounds__(kTravThreads, Query::kCtasPerSm) traverse_kern
   const NodesHeader* h = reinterpret_cast<const NodesHeader*>(A.nodes);
   if (h->magic != kNodesMagic || h->n != A.n) {
     if (MODE != kModeFill)
-      for (int64_t t = (int64_t)blockIdx.x * kTravThreads + threadIdx.x; t < A.q; t += (int64_t)gridDim.x * kTravThreads)
-        A.counts[t] = 0;
+      for (int64_t t = (int64_t)blockIdx.x * kTravThreads + threadIdx.x; t < A.q; t += (int64_t)gridDim.x * kTravThreads) {
+        A.counts[t] = (MODE == kModeReduce) ? -1 : 0;
+        if (MODE == kModeReduce) A.keys[t] = __int_as_float(0x7f800000);
+      }
     return;
   }
-  __shared__ TravSmem<Query, MODE != kModeCount> S;
+  __shared__ TravSmem<Query, mode_stores(MODE)> S;
   if (h->leaf_kind == kLeafPoints)
     traverse_body<Query, MODE, true>(A, S);
   else
@@ -539,15 +654,22 @@ static cudaError_t launch_traverse_kind(TraverseArgs A, int mode, cudaStream_t s
     traverse_kernel<Query, kModeCount><<<g, kTravThreads, 0, stream>>>(A);
   else if (mode == kModeFill)
     traverse_kernel<Query, kModeFill><<<g, kTravThreads, 0, stream>>>(A);
-  else
+  else if (mode == kModeCollect)
     traverse_kernel<Query, kModeCollect><<<g, kTravThreads, 0, stream>>>(A);
+  else if (mode == kModeAny)
+    traverse_kernel<Query, kModeAny><<<g, kTravThreads, 0, stream>>>(A);
+  else if constexpr (Query::kHasKey)
+    traverse_kernel<Query, kModeReduce><<<g, kTravThreads, 0, stream>>>(A);
+  else
+    return cudaErrorInvalidValue;
   return cudaGetLastError();
 }
 
 cudaError_t launch_traverse(const void* nodes, int n, const float* queries, int64_t q, int kind, int mode,
                             const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* out, int64_t cap,
-                            bool only_over, cudaStream_t stream) {
+                            bool only_over, float* keys, cudaStream_t stream) {
   TraverseArgs A{};
+  A.keys = keys;
   A.nodes = static_cast<const char*>(nodes);
   A.n = n;
   A.queries = queries;

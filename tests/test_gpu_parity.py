@@ -401,6 +401,95 @@ def test_containment_shortcut_large_queries(B, oracle_lib):
     assert_query_equal(B, bvh, o, oracle_lib, np.array([[0.5, 0.5, 0.5, 0.45], [0.5, 0.5, 0.5, 5.0]], f), "containment sphere/box leaves")
 
 
+# ---- NEXT-1: operations at the leaf (D10 nearest, D11 first hit, any hit) -----------------------------------------
+
+@pytest.mark.parametrize("name,n,q,radius", [("C1", 4096, 4096, None), ("C3", 120_001, 6_000, 0.004),
+                                             ("C5", 65_537, 6_000, 0.04), ("C4", 70_003, 6_000, None)])
+def test_nearest_within_radius_equals_oracle(B, oracle_lib, name, n, q, radius):
+    w = W.make(name, n=n, q=q, radius=radius)
+    spheres = w.queries if w.queries.shape[1] == 4 else W.spheres_at(w.queries[:, :3], 0.01)   # C4: box leaves
+    spheres = spheres.copy()
+    spheres[::7, 3] = 0.0                                     # some queries that (almost surely) find nothing
+    o = oracle_lib.build_bvh(w.prims, w.morton_bits)
+    oi, od = oracle_lib.nearest_spheres_tree(o, spheres)
+    bvh = gpu_build(B, w.prims, w.morton_bits)
+    for ordered in (True, False):
+        gi, gd = B.reduce_query(bvh, _dev(spheres), "nearest", ordered=ordered)
+        torch.cuda.synchronize()
+        assert np.array_equal(gi.cpu().numpy(), oi), name
+        assert np.array_equal(gd.cpu().numpy().view(np.uint32), od.view(np.uint32)), name     # distances: same bits
+    assert (oi >= 0).sum() > q // 4 and (name == "C1" or (oi < 0).sum() > 0)   # (C1's queries sit on the points)
+    hit = B.reduce_query(bvh, _dev(spheres), "any_hit")
+    torch.cuda.synchronize()
+    assert np.array_equal(hit.cpu().numpy(), (oi >= 0).astype(np.int32))
+
+
+def test_nearest_ties_and_duplicates(B, oracle_lib):
+    """Coincident primitives and lattice points at equal distance: the smallest ORIGINAL index wins, whatever the tree
+    order; zero radius; the radius exactly at a point (closed)."""
+    f = np.float32
+    g = np.arange(8, dtype=f) / f(8.0)
+    pts = np.stack(np.meshgrid(g, g, g, indexing="ij"), axis=-1).reshape(-1, 3).astype(f)
+    pts = np.concatenate([pts, pts[::3], pts[::5]])           # duplicates with larger indices
+    rng = np.random.default_rng(5)
+    pts = pts[rng.permutation(len(pts))]
+    qc = (np.stack(np.meshgrid(g, g, g, indexing="ij"), axis=-1).reshape(-1, 3) + f(1.0 / 16.0)).astype(f)   # cell centres: 8 equidistant corners
+    qs = np.concatenate([W.spheres_at(qc, 0.25), W.spheres_at(pts[:200], 0.0), W.spheres_at(qc[:100], float(np.sqrt(3.0) / 16.0))])
+    for bits in (30, 63):
+        o = oracle_lib.build_bvh(pts, bits)
+        bi, bd = oracle_lib.nearest_spheres_brute(pts, qs)
+        bvh = gpu_build(B, pts, bits)
+        gi, gd = B.reduce_query(bvh, _dev(qs), "nearest")
+        torch.cuda.synchronize()
+        assert np.array_equal(gi.cpu().numpy(), bi) and np.array_equal(gd.cpu().numpy().view(np.uint32), bd.view(np.uint32))
+        assert (bi[:512] >= 0).all() and (bi[512:712] >= 0).all()
+
+
+@pytest.mark.parametrize("name,n", [("C4", 60_000), ("C2", 40_000)])
+def test_first_hit_and_any_hit_rays_equal_oracle(B, oracle_lib, name, n):
+    w = W.make(name, n=n, q=0, radius=0.02 if name == "C4" else None)      # C4: boxes large enough to be hit often
+    prims = w.prims if w.prims.shape[1] == 6 else W.boxes_around(w.prims, 0.004)
+    rays = _rays_through(prims, 8000, seed=41, tmax=4.0)
+    rays[::9, 6] = np.float32(-0.5)                            # negative tmin: entry parameters may be negative
+    o = oracle_lib.build_bvh(prims, 63)
+    oi, ot = oracle_lib.first_hit_rays_tree(o, rays)
+    bvh = gpu_build(B, prims, 63)
+    for ordered in (True, False):
+        gi, gt = B.reduce_query(bvh, _dev(rays), "first_hit", ordered=ordered)
+        torch.cuda.synchronize()
+        assert np.array_equal(gi.cpu().numpy(), oi), name
+        assert np.array_equal(gt.cpu().numpy(), ot), name      # numeric equality (-0.0 == +0.0)
+    assert (oi >= 0).sum() > 500
+    hit = B.reduce_query(bvh, _dev(rays), "any_hit")
+    torch.cuda.synchronize()
+    assert np.array_equal(hit.cpu().numpy(), (oi >= 0).astype(np.int32))
+    # any hit with box queries = "the row is not empty"
+    qb = W.boxes_around(W.uniform_cube(5000, seed=3) * np.float32(2.4) - np.float32(1.2), 0.01)
+    ooff, _ = oracle_lib.query_boxes_tree(o, qb)
+    hit = B.reduce_query(bvh, _dev(qb), "any_hit")
+    torch.cuda.synchronize()
+    assert np.array_equal(hit.cpu().numpy(), (np.diff(ooff) > 0).astype(np.int32))
+    with pytest.raises(B.BvhError):
+        B.reduce_query(bvh, _dev(qb), "nearest")
+
+
+def test_reduce_modes_empty_and_stale(B):
+    bvh = B.Bvh(0, 30)
+    bvh.build(torch.zeros((0, 3), dtype=torch.float32, device="cuda"))
+    qs = _dev(np.array([[0.5, 0.5, 0.5, 1.0], [0, 0, 0, 2.0]], np.float32))
+    i, d = B.reduce_query(bvh, qs, "nearest")
+    h = B.reduce_query(bvh, qs, "any_hit")
+    torch.cuda.synchronize()
+    assert i.cpu().tolist() == [-1, -1] and bool(torch.isinf(d).all()) and h.cpu().tolist() == [0, 0]
+    pts = W.uniform_cube(3000, seed=2)
+    bvh = gpu_build(B, pts, 30)
+    idx = torch.zeros(2, dtype=torch.int32, device="cuda")
+    key = torch.zeros(2, dtype=torch.float32, device="cuda")
+    B.bvh_query_spheres_nearest(bvh.nodes, 2999, qs, 2, None, idx, key)      # n does not match the buffer's header
+    torch.cuda.synchronize()
+    assert idx.cpu().tolist() == [-1, -1] and bool(torch.isinf(key).all())
+
+
 def test_empty_inputs(B):
     bvh = B.Bvh(0, 30)
     bvh.build(torch.zeros((0, 3), dtype=torch.float32, device="cuda"))
