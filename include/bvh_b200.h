@@ -176,17 +176,27 @@ int bvh_query_rays_first_hit(const void* nodes, int64_t n, const float* rays, in
 int bvh_query_any_hit(const void* nodes, int64_t n, const float* queries, int query_kind, int64_t q,
                       const uint32_t* order, int32_t* hit, void* stream);
 
-/* NEXT-2: a MEASUREMENT variant of the build, not a product path.  variant = 1 replaces the last step
- * (the single bottom-up pass of Algorithm 4) by what the paper compares itself with: Karras' top-down construction,
- * one thread per internal node searching its range and split on the common-prefix length of the augmented keys
- * (PAPER.md:99-101), skip-connections by Algorithm 2, and a separate bottom-up pass for the boxes
- * with atomic arrival counters in global memory.  Bounds, Morton codes, sort and the layout of `nodes`
- * are unchanged, and `nodes` comes out byte-identical to bvh_build_points / bvh_build_boxes.  scratch must hold
- * bvh_variant_sizes bytes (the product's scratch plus parent / child / counter arrays).  stage_events as in
- * bvh_build_staged (may be NULL); event [12] closes the replaced step.  bvh_variant_sizes is a host call. */
+/* NEXT-2: MEASUREMENT variants of the build, not product paths.  They replace the last step (the single
+ * bottom-up pass of Algorithm 4) by what the paper compares itself with; bounds, Morton codes, sort and the record
+ * layout are unchanged.
+ *   variant = 1  Karras' top-down construction, one thread per internal node searching its range and split on the
+ *                common-prefix length of the augmented keys, skip-connections by Algorithm 2
+ *                (PAPER.md:105-116), and a separate bottom-up pass for the boxes with atomic arrival counters in global
+ *                memory.  `nodes` comes out byte-identical to bvh_build_points / bvh_build_boxes.
+ *   variant = 2  the unmodified Algorithm 3: bottom-up with ATOMICCAS on a global `store`, internal
+ *                nodes numbered by their split position (Apetrei numbering), root index stored, followed by
+ *                "an extra tree traversal pass" for the skip-connections.  The hierarchy is the same
+ *                tree with other node indices; it is NOT traversable by bvh_query_* (which rely on Karras numbering;
+ *                the buffer is marked and the query kernels refuse it) and is read back with bvh_variant_export:
+ *                left, right: int32[n-1] by Apetrei index (unified child indices: internal p -> p, leaf i -> n-1+i);
+ *                rope: int32[2n-1]; aabb: float[2n-1][6]; root: int32[1].  Any output may be NULL.
+ * scratch must hold bvh_variant_sizes bytes (the product's scratch plus parent / child / counter arrays).  stage_events
+ * as in bvh_build_staged (may be NULL); event [12] closes the replaced step.  bvh_variant_sizes is a host call. */
 int bvh_variant_sizes(int64_t n, int morton_bits, int variant, size_t* scratch_bytes);
 int bvh_build_variant(const float* prim, int prim_is_box, int64_t n, int morton_bits, void* nodes, void* scratch,
                       size_t scratch_bytes, int variant, void* stream, void* const* stage_events);
+int bvh_variant_export(const void* nodes, void* scratch, int64_t n, int morton_bits, int variant, int32_t* left,
+                       int32_t* right, int32_t* rope, float* aabb, int32_t* root, void* stream);
 
 /* Parity export: the canonical arrays of a finished build, for bit-exact comparison.
  * sorted_codes: uint32[n] when morton_bits = 30, uint64[n] when 63.  perm: uint32[n], original

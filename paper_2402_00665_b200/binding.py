@@ -56,6 +56,7 @@ SYMBOLS = {
     "bvh_query_rays_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
     "bvh_variant_sizes": [c_int64, c_int, c_int, ctypes.POINTER(c_size_t)],
     "bvh_build_variant": [_P, c_int, c_int64, c_int, _P, _P, c_size_t, c_int, _P, ctypes.POINTER(c_void_p)],
+    "bvh_variant_export": [_P, _P, c_int64, c_int, c_int, _P, _P, _P, _P, _P, _P],
     "bvh_export": [_P, _P, c_int64, c_int, _P, _P, _P, _P, _P, _P, _P],
 }
 
@@ -221,10 +222,18 @@ def bvh_variant_sizes(n: int, morton_bits: int, variant: int) -> int:
 
 
 def bvh_build_variant(prim, prim_is_box: int, n: int, morton_bits: int, nodes, scratch, variant: int) -> None:
-    """NEXT-2 measurement variant (1 = Karras top-down + Algorithm 2 + separate box pass); same `nodes` bytes."""
+    """NEXT-2 measurement variants: 1 = Karras top-down + Algorithm 2 + separate box pass (same `nodes` bytes as the
+    product); 2 = unmodified Algorithm 3 (Apetrei numbering) + separate skip-connection pass (read with
+    bvh_variant_export)."""
     _check(load_library().bvh_build_variant(_ptr(prim), prim_is_box, n, morton_bits, _ptr(nodes), _ptr(scratch),
                                             scratch.numel() * scratch.element_size(), variant, _stream(), None),
            "bvh_build_variant")
+
+
+def bvh_variant_export(nodes, scratch, n: int, morton_bits: int, variant: int, left=None, right=None, rope=None, aabb=None,
+                       root=None) -> None:
+    _check(load_library().bvh_variant_export(_ptr(nodes), _ptr(scratch), n, morton_bits, variant, _ptr(left), _ptr(right),
+                                             _ptr(rope), _ptr(aabb), _ptr(root), _stream()), "bvh_variant_export")
 
 
 def bvh_scan_sizes(q: int) -> int:

@@ -144,8 +144,8 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   if (misaligned(prim) || misaligned(nodes) || misaligned(scratch)) return BVH_ERR_INVALID_ARGUMENT;
   if ((reinterpret_cast<uintptr_t>(nodes) & 31u) != 0) return BVH_ERR_INVALID_ARGUMENT;
   const ScratchLayout L = scratch_layout(n, morton_bits);
-  if (variant != 0 && variant != 1) return BVH_ERR_INVALID_ARGUMENT;
-  if (scratch_bytes < L.total + (variant == 1 ? variant_extra_bytes(n) : 0)) return BVH_ERR_SCRATCH;
+  if (variant < 0 || variant > 2) return BVH_ERR_INVALID_ARGUMENT;
+  if (scratch_bytes < L.total + (variant != 0 ? variant_extra_bytes(n) : 0)) return BVH_ERR_SCRATCH;
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   char* base = static_cast<char*>(scratch);
   Header* header = reinterpret_cast<Header*>(base + L.header);
@@ -166,6 +166,13 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   if (variant == 1) {
     if (launch_variant_karras(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
                               nodes, (int)n, header, base + L.total, stream) != 0)
+      return BVH_ERR_CUDA;
+    mark(12);
+    return check_launch();
+  }
+  if (variant == 2) {
+    if (launch_variant_apetrei(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
+                               nodes, (int)n, header, base + L.total, stream) != 0)
       return BVH_ERR_CUDA;
     mark(12);
     return check_launch();
@@ -290,7 +297,7 @@ int bvh_build_staged(const float* prim, int prim_is_box, int64_t n, int morton_b
 }
 
 int bvh_variant_sizes(int64_t n, int morton_bits, int variant, size_t* scratch_bytes) {
-  if (n < 0 || !scratch_bytes || variant != 1) return BVH_ERR_INVALID_ARGUMENT;
+  if (n < 0 || !scratch_bytes || (variant != 1 && variant != 2)) return BVH_ERR_INVALID_ARGUMENT;
   if (morton_bits != 30 && morton_bits != 63) return BVH_ERR_MORTON_BITS;
   if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
   *scratch_bytes = bvh::scratch_layout(n, morton_bits).total + bvh::variant_extra_bytes(n);
@@ -300,6 +307,20 @@ int bvh_variant_sizes(int64_t n, int morton_bits, int variant, size_t* scratch_b
 int bvh_build_variant(const float* prim, int prim_is_box, int64_t n, int morton_bits, void* nodes, void* scratch,
                       size_t scratch_bytes, int variant, void* stream, void* const* stage_events) {
   return bvh::build(prim, prim_is_box != 0, n, morton_bits, nodes, scratch, scratch_bytes, stream, stage_events, variant);
+}
+
+int bvh_variant_export(const void* nodes, void* scratch, int64_t n, int morton_bits, int variant, int32_t* left,
+                       int32_t* right, int32_t* rope, float* aabb, int32_t* root, void* stream) {
+  if (n < 0 || variant != 2) return BVH_ERR_INVALID_ARGUMENT;
+  if (morton_bits != 30 && morton_bits != 63) return BVH_ERR_MORTON_BITS;
+  if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
+  if (n == 0) return BVH_OK;
+  if (!nodes || !scratch) return BVH_ERR_INVALID_ARGUMENT;
+  const bvh::ScratchLayout L = bvh::scratch_layout(n, morton_bits);
+  if (bvh::launch_variant_apetrei_export(nodes, static_cast<char*>(scratch) + L.total, (int)n, left, right, rope, aabb, root,
+                                         static_cast<cudaStream_t>(stream)) != 0)
+    return BVH_ERR_CUDA;
+  return BVH_OK;
 }
 
 int bvh_query_order_sizes(int64_t q, size_t* scratch_bytes) {

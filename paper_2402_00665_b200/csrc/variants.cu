@@ -35,15 +35,16 @@ __device__ __forceinline__ int prefix_len(const KeyT* __restrict__ codes, int n,
 
 struct VariantScratch {
   int32_t* parent;   // [2n-1] parent of every node of the unified index space
-  uint32_t* flags;   // [n-1]   children arrived at each internal node (zeroed)
-  int32_t* left;     // [n-1]   left child, by Karras index
-  int32_t* right;    // [n-1]   right child
-  int32_t* rope;     // [n-1]   skip-connection, by Karras index
+  uint32_t* flags;   // [n-1]   variant 1: children arrived at each internal node (zeroed); variant 2: Algorithm 3's `store`
+  int32_t* left;     // [n-1]   left child, by Karras index (variant 1)
+  int32_t* right;    // [n-1]   right child (variant 1: Karras index; variant 2: Apetrei index)
+  int32_t* rope;     // [n-1]   skip-connection, by Karras index (variant 1)
+  int32_t* leaf_rope;  // [n]   variant 2: skip-connection of every leaf (an Apetrei index does not fit the leaf record's one bit)
 };
 static inline size_t align256(size_t x) { return (x + 255) / 256 * 256; }
 size_t variant_extra_bytes(int64_t n) {
   const size_t nn = (size_t)(n > 0 ? n : 1);
-  return align256(4 * (2 * nn)) + 4 * align256(4 * nn);
+  return align256(4 * (2 * nn)) + 5 * align256(4 * nn);
 }
 static VariantScratch variant_scratch(char* base, int64_t n) {
   const size_t nn = (size_t)(n > 0 ? n : 1);
@@ -57,6 +58,8 @@ static VariantScratch variant_scratch(char* base, int64_t n) {
   v.right = reinterpret_cast<int32_t*>(base);
   base += align256(4 * nn);
   v.rope = reinterpret_cast<int32_t*>(base);
+  base += align256(4 * nn);
+  v.leaf_rope = reinterpret_cast<int32_t*>(base);
   return v;
 }
 
@@ -196,6 +199,177 @@ static void launch_variant_keys(const float* prim, bool is_box, const KeyT* code
   if (n < 2) return;
   launch_pdl(karras_topdown_kernel<KeyT>, dim3((unsigned)((n - 1 + 255) / 256)), dim3(256), 0, stream, codes, n, v);
   launch_pdl(karras_box_kernel, dim3(gl), dim3(256), 0, stream, nodes, n, is_box ? kLeafBoxes : kLeafPoints, v);
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// variant 2: the UNMODIFIED Algorithm 3, followed by what the paper's modification removes: "an
+// extra tree traversal pass" that installs the skip-connections.  Internal nodes are numbered by
+// their split position p, both children write themselves into the parent before the ATOMICCAS on
+// `store` (L7-8, L13-14), the first arrival stops, the second merges the boxes (G10: the sibling's box is read back
+// through L2 after a fence) and carries on; the node whose range is [0, n-1] is the root and its index is stored in
+// the header.  The records are the product's {min, left | max, rope}, indexed by Apetrei index; the
+// right child, which the product never stores (Karras numbering: it is left + 1), goes to the variant's scratch, as
+// do the leaves' skip-connections.  The product's traversal relies on Karras numbering (the skip target's index is
+// the first leaf after the subtree), so this hierarchy is not handed to it: its header carries another magic.
+constexpr uint32_t kNodesMagicApetrei = 0x42564133u;   // "BVA3"
+
+template <typename KeyT>
+__global__ void __launch_bounds__(256)
+apetrei_kernel(const KeyT* __restrict__ codes, char* nodes_base, int n, int leaf_kind, VariantScratch v) {
+  pdl_wait();
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n || n < 2) return;
+  const int leaf_base = n - 1;
+  Node* internal = reinterpret_cast<Node*>(nodes_base + kNodesHeaderBytes);
+  int* store = reinterpret_cast<int*>(v.flags);
+  auto dstar = [&](int a) { return (a < 0 || a >= n - 1) ? -1 : prefix_len(codes, n, codes[a], a, a + 1); };   // larger = more similar
+  int cur = leaf_base + i;                                   // the node this thread has just completed
+  int range_left = i, range_right = i;                       // L3-4
+  int sim_left = dstar(i - 1), sim_right = dstar(i);         // delta*(l-1), delta*(r) as prefix lengths: delta_right < delta_left <=> sim_right > sim_left
+  float lo[3], hi[3];
+  load_box_any(nodes_base, n, leaf_kind, cur, lo, hi);
+  while (true) {
+    const bool is_left = sim_right > sim_left;               // L5
+    const int p = is_left ? range_right : range_left - 1;    // L6 / L12: Apetrei index = split
+    if (is_left)
+      reinterpret_cast<int*>(internal + p)[3] = cur;         // L7: I_p.left
+    else
+      v.right[p] = cur;                                      // L13: I_p.right
+    v.parent[cur] = p;                                       // (for the skip-connection pass)
+    __threadfence();                                         // this child's record and pointer before its arrival
+    const int other = atomicCAS(store + p, kInvalid, is_left ? range_left : range_right);   // L8 / L14
+    if (other == kInvalid) return;                           // L9 / L15: first to arrive
+    __threadfence();
+    int sib;
+    if (is_left) {
+      range_right = other;
+      sim_right = dstar(range_right);                        // L10
+      sib = __ldcg(v.right + p);
+    } else {
+      range_left = other;
+      sim_left = dstar(range_left - 1);                      // L16
+      sib = __ldcg(reinterpret_cast<const int*>(internal + p) + 3);
+    }
+    float lo2[3], hi2[3];
+    load_box_any(nodes_base, n, leaf_kind, sib, lo2, hi2);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      lo[a] = fminf(lo[a], lo2[a]);
+      hi[a] = fmaxf(hi[a], hi2[a]);
+    }
+    Node rec;
+    rec.lo = make_float4(lo[0], lo[1], lo[2], __int_as_float(is_left ? cur : sib));
+    rec.hi = make_float4(hi[0], hi[1], hi[2], __int_as_float(kSentinel));   // the skip-connection comes with the next pass
+    internal[p] = rec;
+    cur = p;                                                 // L18
+    if (range_left == 0 && range_right == n - 1) {           // L19: the root; "its index now needs to be stored"
+      reinterpret_cast<NodesHeader*>(nodes_base)->reserved = p;
+      v.parent[p] = kSentinel;
+      return;
+    }
+  }
+}
+
+// The extra pass: the skip-connection of a node is the right child of the nearest ancestor (itself
+// included) that is a left child's parent ... i.e. walk up while the node is a right child; the sibling of the first
+// left child on the way is the target; the right-most path ends at the sentinel.
+__global__ void __launch_bounds__(256) apetrei_rope_kernel(char* nodes_base, int n, VariantScratch v) {
+  pdl_wait();
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  if (x == 0) reinterpret_cast<NodesHeader*>(nodes_base)->magic = kNodesMagicApetrei;
+  if (x >= 2 * n - 1) return;
+  const int leaf_base = n - 1;
+  const Node* internal = reinterpret_cast<const Node*>(nodes_base + kNodesHeaderBytes);
+  int rope = kSentinel;
+  if (n >= 2) {
+    int c = x;
+    while (true) {
+      const int p = v.parent[c];
+      if (p < 0) break;
+      if (reinterpret_cast<const int*>(internal + p)[3] == c) {   // c is the left child of p
+        rope = v.right[p];
+        break;
+      }
+      c = p;
+    }
+  }
+  if (x < leaf_base)
+    reinterpret_cast<int*>(const_cast<Node*>(internal) + x)[7] = rope;
+  else
+    v.leaf_rope[x - leaf_base] = rope;
+}
+
+template <typename KeyT>
+static cudaError_t launch_apetrei_keys(const float* prim, bool is_box, const KeyT* codes, const uint32_t* perm, char* nodes, int n,
+                                       const Header* header, VariantScratch v, cudaStream_t stream) {
+  const unsigned gl = (unsigned)((n + 255) / 256);
+  cudaError_t e;
+  if (is_box)
+    e = launch_pdl(karras_leaf_kernel<KeyT, true>, dim3(gl), dim3(256), 0, stream, prim, codes, perm, nodes, n, header);
+  else
+    e = launch_pdl(karras_leaf_kernel<KeyT, false>, dim3(gl), dim3(256), 0, stream, prim, codes, perm, nodes, n, header);
+  if (e != cudaSuccess) return e;
+  e = launch_pdl(apetrei_kernel<KeyT>, dim3(gl), dim3(256), 0, stream, codes, nodes, n, is_box ? kLeafBoxes : kLeafPoints, v);
+  if (e != cudaSuccess) return e;
+  return launch_pdl(apetrei_rope_kernel, dim3((unsigned)((2 * (int64_t)n - 1 + 255) / 256)), dim3(256), 0, stream, nodes, n, v);
+}
+
+// variant 2 export: the arrays of the Apetrei-numbered hierarchy in the unified index space (internal I_p -> p).
+__global__ void apetrei_export_kernel(const char* __restrict__ nodes, VariantScratch v, int n, int32_t* left, int32_t* right,
+                                      int32_t* rope, float* aabb, int32_t* root) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int leaf_base = n - 1;
+  const NodesHeader* h = reinterpret_cast<const NodesHeader*>(nodes);
+  if (i == 0 && root) *root = n >= 2 ? h->reserved : 0;
+  if (i >= 2 * (int64_t)n - 1) return;
+  float lo[3], hi[3];
+  if (i < leaf_base) {
+    const Node* rec = reinterpret_cast<const Node*>(nodes + kNodesHeaderBytes) + i;
+    const float4 a = rec->lo, b = rec->hi;
+    lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; hi[0] = b.x; hi[1] = b.y; hi[2] = b.z;
+    if (left) left[i] = __float_as_int(a.w);
+    if (right) right[i] = v.right[i];
+    if (rope) rope[i] = __float_as_int(b.w);
+  } else {
+    const int li = (int)(i - leaf_base);
+    const char* leaves = nodes + leaf_offset_bytes(n);
+    if (h->leaf_kind == kLeafPoints) {
+      const float4 p = reinterpret_cast<const float4*>(leaves)[li];
+      lo[0] = hi[0] = p.x; lo[1] = hi[1] = p.y; lo[2] = hi[2] = p.z;
+    } else {
+      const Node* rec = reinterpret_cast<const Node*>(leaves) + li;
+      const float4 a = rec->lo, b = rec->hi;
+      lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; hi[0] = b.x; hi[1] = b.y; hi[2] = b.z;
+    }
+    if (rope) rope[i] = v.leaf_rope[li];
+  }
+  if (aabb) {
+    float* o = aabb + 6 * i;
+    o[0] = lo[0]; o[1] = lo[1]; o[2] = lo[2]; o[3] = hi[0]; o[4] = hi[1]; o[5] = hi[2];
+  }
+}
+
+int launch_variant_apetrei_export(const void* nodes, void* extra, int n, int32_t* left, int32_t* right, int32_t* rope,
+                                  float* aabb, int32_t* root, cudaStream_t stream) {
+  VariantScratch v = variant_scratch(static_cast<char*>(extra), n);
+  const int64_t total = 2 * (int64_t)n - 1;
+  apetrei_export_kernel<<<(unsigned)((total + 255) / 256), 256, 0, stream>>>(static_cast<const char*>(nodes), v, n, left, right,
+                                                                            rope, aabb, root);
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+int launch_variant_apetrei(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
+                           void* nodes, int n, const Header* header, void* extra, cudaStream_t stream) {
+  VariantScratch v = variant_scratch(static_cast<char*>(extra), n);
+  if (n >= 2 && cudaMemsetAsync(v.flags, 0xFF, sizeof(uint32_t) * (size_t)(n - 1), stream) != cudaSuccess) return -1;   // store <- invalid (L1)
+  cudaError_t e;
+  if (key_bytes == 4)
+    e = launch_apetrei_keys<uint32_t>(prim, is_box, static_cast<const uint32_t*>(sorted_codes), perm, static_cast<char*>(nodes),
+                                      n, header, v, stream);
+  else
+    e = launch_apetrei_keys<uint64_t>(prim, is_box, static_cast<const uint64_t*>(sorted_codes), perm, static_cast<char*>(nodes),
+                                      n, header, v, stream);
+  return e == cudaSuccess ? 0 : -1;
 }
 
 // The last step of the build, Karras-style.  extra: variant_extra_bytes(n) of scratch after the product's layout.

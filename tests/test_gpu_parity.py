@@ -663,3 +663,59 @@ def test_variant_karras_topdown(B, oracle_lib, name, n):
         B.bvh_build_variant(_dev(pts), 0, tiny, 63, t.nodes, t.scratch, 1)
         torch.cuda.synchronize()
         assert_build_equal(export_np(t), oracle_lib.build_bvh(pts, 63), f"tiny {tiny}")
+
+
+def _variant2(B, prims, bits):
+    n = prims.shape[0]
+    v = B.Bvh(n, bits)
+    v.scratch = torch.empty(B.bvh_variant_sizes(n, bits, 2), dtype=torch.uint8, device="cuda")
+    v.nodes.zero_()
+    B.bvh_build_variant(_dev(prims), int(prims.shape[1] == 6), n, bits, v.nodes, v.scratch, 2)
+    out = {"left": torch.zeros(max(n - 1, 1), dtype=torch.int32, device="cuda"),
+           "right": torch.zeros(max(n - 1, 1), dtype=torch.int32, device="cuda"),
+           "rope": torch.zeros(2 * n - 1, dtype=torch.int32, device="cuda"),
+           "aabb": torch.zeros((2 * n - 1, 6), dtype=torch.float32, device="cuda"),
+           "root": torch.zeros(1, dtype=torch.int32, device="cuda")}
+    B.bvh_variant_export(v.nodes, v.scratch, n, bits, 2, **out)
+    torch.cuda.synchronize()
+    return v, {k: t.cpu().numpy() for k, t in out.items()}
+
+
+@pytest.mark.parametrize("name,n", [("C1", 4096), ("C2", 60_001), ("C3", 200_000), ("C4", 50_000), ("C5", 70_000)])
+def test_variant_apetrei_algorithm3(B, oracle_lib, name, n):
+    """NEXT-2 (a): the unmodified Algorithm 3 + a separate skip-connection pass builds the same tree with Apetrei's node
+    numbering (index = split, stored root): every array equals the oracle's serial Algorithm 3 (which is pinned to the
+    top-down tree renamed node-to-split), boxes bit for bit; the product's queries refuse the buffer."""
+    w = W.make(name, n=n, q=0)
+    o = oracle_lib.build_bvh(w.prims, w.morton_bits)
+    t = oracle_lib.apetrei_tree(w.prims, o)
+    v, g = _variant2(B, w.prims, w.morton_bits)
+    assert int(g["root"][0]) == t.root
+    assert np.array_equal(g["left"][: n - 1], t.left) and np.array_equal(g["right"][: n - 1], t.right)
+    assert np.array_equal(g["rope"], t.rope)
+    assert np.array_equal(g["aabb"].view(np.uint32), t.aabb.view(np.uint32))
+    # the same tree as the product's: the always-true walk from the stored root visits the leaves in order
+    lb = n - 1
+    node, seen = t.root, []
+    lc = np.concatenate([g["left"][: n - 1], np.zeros(n, np.int32)])
+    for _ in range(2 * n):
+        if node < 0:
+            break
+        if node >= lb:
+            seen.append(node - lb)
+            node = g["rope"][node]
+        else:
+            node = lc[node]
+    assert seen == list(range(n))
+    cnt = torch.full((4,), -1, dtype=torch.int32, device="cuda")
+    B.bvh_query_spheres_count(v.nodes, n, _dev(W.spheres_at(W.uniform_cube(4, seed=1), 0.5)), 4, None, cnt)
+    torch.cuda.synchronize()
+    assert cnt.cpu().tolist() == [0, 0, 0, 0]                  # not a Karras-ordered hierarchy: refused
+    for tiny in (1, 2, 3, 5):
+        pts = W.uniform_cube(tiny, seed=tiny)
+        ot = oracle_lib.apetrei_tree(pts, oracle_lib.build_bvh(pts, 63))
+        _, gt = _variant2(B, pts, 63)
+        assert np.array_equal(gt["rope"], ot.rope) and np.array_equal(gt["aabb"].view(np.uint32), ot.aabb.view(np.uint32))
+        if tiny >= 2:
+            assert int(gt["root"][0]) == ot.root and np.array_equal(gt["left"][: tiny - 1], ot.left)
+            assert np.array_equal(gt["right"][: tiny - 1], ot.right)
