@@ -3,7 +3,9 @@
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: linear-BVH build (scene
 bounds, Morton codes, one-sweep radix sort, modified-Apetrei bottom-up pass with ropes and boxes) followed
-by stackless sphere range search to CSR (count, scan, fill).  Workload at N=1: BASELINE.json configs[2]
+by stackless sphere range search to CSR.  The query part of the step is the single-pass form of
+count-then-fill (order, collect = one traversal that counts and stores rows, scan, rows -> CSR, overflow
+rows); the two-traversal form (count, scan, fill) is timed beside it as `query_two_pass`.  Workload at N=1: BASELINE.json configs[2]
 ("C3": 10,000,000 Gaussian-mixture points, 30-bit Morton, 1,000,000 sphere queries of radius 0.002), the
 config `north_star` quotes its target on.
 
@@ -13,7 +15,8 @@ config `north_star` quotes its target on.
 `value` = build throughput (Mprims/s) with inputs resident in HBM, CUDA-event time of the build part of the
 step; the query part is reported beside it (`query`), `ms_per_step` covers both.  N > 1 runs N independent
 replicas (one per GPU, different seeds, no collective on the data path: DESIGN.md "Multi-GPU"), timed as
-the max over ranks.  `--impl reference` times the CPU oracle (oracle/) on a bounded sample: for this tier
+the max over ranks; `--multi shard` instead builds the same hierarchy on every rank and splits ONE query batch
+over the ranks (NEXT-4: strong scaling of the query part, one all-gather of result sizes).  `--impl reference` times the CPU oracle (oracle/) on a bounded sample: for this tier
 the oracle is the reference arm.
 """
 from __future__ import annotations
@@ -39,9 +42,11 @@ UNIT = "Mprims/s"
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 NOMINAL_HBM_GBS = 8000.0   # the denominator BASELINE.json north_star names
 
-# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel from the
-# `ncu --set full` capture summarised in profiles/ (None until a capture for that kernel/workload exists).
-NCU_TRAFFIC_BYTES = {"fill": 4_259_000_000, "count": 327_110_000}   # profiles/r01c_ncu.md rows 17, 13 (DRAM rd + wr)
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of a kernel from the `ncu --set full` captures
+# summarised in profiles/, keyed by (workload, n, q): `roofline.traffic` is null for any other workload or size.
+NCU_TRAFFIC_BYTES = {
+    ("C3", 10_000_000, 1_000_000): {"fill": 4_259_000_000, "count": 327_110_000},   # profiles/r01c_ncu.md rows 17, 13
+}
 
 
 # ---- byte model (restated in DESIGN.md "Roofline") ---------------------------------------
@@ -59,6 +64,9 @@ def byte_model(n: int, q: int, nnz: int, prim_floats: int, query_floats: int, bi
         "count": (Sq + 4 + 4) * q,
         "scan": (4 + 8) * q,
         "fill": (Sq + 8 + 4) * q + 4 * nnz,
+        "collect": (Sq + 4 + 4) * q + 4 * nnz,           # query, order, count out, every hit stored once
+        "rows_to_csr": (4 + 8) * q + 8 * nnz,            # counts, offsets, every hit read and written once
+        "overflow": 4 * q,                               # counts (no row overflows when the capacity holds the largest row)
     }
     build_total = (3 * S + 4 * K + (2 * P - 1) * (K + 4) + 100) * n      # SURVEY.md B_build
     query_total = (2 * Sq + 24) * q + 4 * nnz                            # SURVEY.md B_query
@@ -190,7 +198,7 @@ def config_dict(args, w, world: int, extra=None) -> dict:
 def run_ours(args) -> dict | None:
     import torch
 
-    from paper_2402_00665_b200 import binding
+    from paper_2402_00665_b200 import binding, sharded
 
     rank, local_rank, world = dist_init("nccl")
     if not torch.cuda.is_available():
@@ -199,28 +207,34 @@ def run_ours(args) -> dict | None:
     device = torch.device("cuda", local_rank)
     binding.load_library()
 
-    w = make_workload(args, rank)
-    n, q, bits = w.n, w.q, w.morton_bits
+    shard = args.multi == "shard" and world > 1
+    w = make_workload(args, 0 if shard else rank)           # shard: every rank holds the same scene and the same batch
+    n, bits = w.n, w.morton_bits
     is_box = int(w.prim_kind == "boxes")
-    spheres = w.query_kind == "spheres"
+    kind = binding.QUERY_KINDS[w.queries.shape[1]]
+    q_lo, q_hi = sharded.block_bounds(w.q, rank, world) if shard else (0, w.q)
+    q = q_hi - q_lo                                         # queries this rank serves
     h_prims = torch.from_numpy(w.prims).pin_memory()
-    h_queries = torch.from_numpy(w.queries).pin_memory()
+    h_queries = torch.from_numpy(np.ascontiguousarray(w.queries[q_lo:q_hi])).pin_memory()
     d_prims = h_prims.to(device)
     d_queries = h_queries.to(device)
     bvh = binding.Bvh(n, bits, device)
     ws = binding.QueryWorkspace(q, device)
-    order_fn = binding.bvh_query_order_spheres if spheres else binding.bvh_query_order_boxes
-    count_fn = binding.bvh_query_spheres_count if spheres else binding.bvh_query_boxes_count
-    fill_fn = binding.bvh_query_spheres_fill if spheres else binding.bvh_query_boxes_fill
+    order_fn = (binding.bvh_query_order_spheres, binding.bvh_query_order_boxes, binding.bvh_query_order_rays)[kind]
+    count_fn = (binding.bvh_query_spheres_count, binding.bvh_query_boxes_count, binding.bvh_query_rays_count)[kind]
+    fill_fn = (binding.bvh_query_spheres_fill, binding.bvh_query_boxes_fill, binding.bvh_query_rays_fill)[kind]
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)
 
-    # one untimed pass to learn nnz (same inputs every step -> same nnz) and size the result buffer
+    # one untimed pass to learn nnz and the largest row (same inputs every step -> same counts): sizes the result
+    # buffer and the row capacity of the single-pass query ("capacity from the previous batch")
     bvh.build(d_prims)
     order_fn(bvh.nodes, n, d_queries, q, ws.order, ws.order_scratch)
     count_fn(bvh.nodes, n, d_queries, q, ws.order, ws.counts)
     binding.bvh_scan_counts(ws.counts, q, ws.offsets, ws.scan_scratch)
     nnz = int(ws.offsets[q].item())
+    cap = max(8, (int(ws.counts[:q].max().item()) + 7) // 8 * 8) if q > 0 else 8
     d_indices = torch.empty(max(nnz, 1), dtype=torch.int32, device=device)
+    d_rows = torch.empty(max(q, 1) * cap, dtype=torch.int32, device=device)
 
     def ev():
         e = torch.cuda.Event(enable_timing=True)
@@ -228,36 +242,51 @@ def run_ours(args) -> dict | None:
         return e
 
     stage = [ev() for _ in range(binding.NUM_STAGE_EVENTS)]
-    e_b0, e_b1, e_order, e_count, e_scan, e_fill = ev(), ev(), ev(), ev(), ev(), ev()
+    e_b0, e_b1, e_order, e_collect, e_scan, e_rows, e_over = (ev() for _ in range(7))
+    t_c0, t_c1, t_c2, t_c3 = (ev() for _ in range(4))
     P = 4 if bits == 30 else 8
     stage_for_call = [stage[k] if (k < 4 + P or k == 12) else None for k in range(binding.NUM_STAGE_EVENTS)]
     build_fn = binding.bvh_build_boxes if is_box else binding.bvh_build_points
 
     def step():
         """One pass of the hot path through the public entry points: the build as ONE call (no events inside it),
-        then the query stages with an event after each."""
+        then the single-pass query with an event after each stage."""
         e_b0.record()
         build_fn(d_prims, n, bits, bvh.nodes, bvh.scratch)
         e_b1.record()
         order_fn(bvh.nodes, n, d_queries, q, ws.order, ws.order_scratch)
         e_order.record()
-        count_fn(bvh.nodes, n, d_queries, q, ws.order, ws.counts)
-        e_count.record()
+        binding.bvh_query_collect(bvh.nodes, n, d_queries, kind, q, ws.order, cap, d_rows, ws.counts)
+        e_collect.record()
         binding.bvh_scan_counts(ws.counts, q, ws.offsets, ws.scan_scratch)
         e_scan.record()
+        binding.bvh_rows_to_csr(d_rows, cap, ws.counts, ws.offsets, q, d_indices)
+        e_rows.record()
+        binding.bvh_query_fill_overflow(bvh.nodes, n, d_queries, kind, q, ws.order, cap, ws.counts, ws.offsets, d_indices)
+        e_over.record()
+
+    def two_pass():
+        """The two-traversal form of the same query (count, scan, fill), on the hierarchy the last step left."""
+        t_c0.record()
+        count_fn(bvh.nodes, n, d_queries, q, ws.order, ws.counts)
+        t_c1.record()
+        binding.bvh_scan_counts(ws.counts, q, ws.offsets, ws.scan_scratch)
+        t_c2.record()
         fill_fn(bvh.nodes, n, d_queries, q, ws.order, ws.offsets, d_indices)
-        e_fill.record()
+        t_c3.record()
 
     build_names = ["init", "bounds", "morton"] + [f"sort_pass{p}" for p in range(P)] + ["hierarchy"]
-    names = build_names + ["order", "count", "scan", "fill"]
+    query_names = ["order", "collect", "scan", "rows_to_csr", "overflow"]
+    names = build_names + query_names
     launches_per_step = {"init": 0, "bounds": 1, "morton": 1, **{f"sort_pass{p}": 1 for p in range(P)},
-                         "hierarchy": 2 if n > 256 else 1, "order": 5, "count": 1, "scan": 3, "fill": 1}
+                         "hierarchy": 2 if n > 256 else 1, "order": 5, "collect": 1, "scan": 3, "rows_to_csr": 1,
+                         "overflow": 1}
 
     def read_times() -> dict:
         return {"_build": e_b0.elapsed_time(e_b1), "order": e_b1.elapsed_time(e_order),
-                "count": e_order.elapsed_time(e_count), "scan": e_count.elapsed_time(e_scan),
-                "fill": e_scan.elapsed_time(e_fill), "_query": e_b1.elapsed_time(e_fill),
-                "_step": e_b0.elapsed_time(e_fill)}
+                "collect": e_order.elapsed_time(e_collect), "scan": e_collect.elapsed_time(e_scan),
+                "rows_to_csr": e_scan.elapsed_time(e_rows), "overflow": e_rows.elapsed_time(e_over),
+                "_query": e_b1.elapsed_time(e_over), "_step": e_b0.elapsed_time(e_over)}
 
     def read_stage_times() -> dict:
         t = {"init": stage[0].elapsed_time(stage[1]), "bounds": stage[1].elapsed_time(stage[2]),
@@ -294,6 +323,15 @@ def run_ours(args) -> dict | None:
     dist_barrier(world, device)
     clocks = sampler.stop() if rank == 0 else None
 
+    # ---- the two-traversal query, same inputs, same hierarchy (not part of `value` / `ms_per_step`) ------------------
+    for _ in range(args.steps):
+        flush.fill_(1)
+        two_pass()
+        torch.cuda.synchronize()
+        for k, v in (("tp_count", t_c0.elapsed_time(t_c1)), ("tp_scan", t_c1.elapsed_time(t_c2)),
+                     ("tp_fill", t_c2.elapsed_time(t_c3))):
+            acc[k] = acc.get(k, 0.0) + v
+
     # ---- per-kernel breakdown of the build: the same build through bvh_build_staged, which records an event after
     # every kernel.  Separate steps, not part of `value`: an event between two kernels keeps the second from being
     # set up while the first still runs (programmatic dependent launch), so the staged build is a little slower.
@@ -306,9 +344,8 @@ def run_ours(args) -> dict | None:
 
     # ---- end to end: pinned host inputs -> device -> build -> query -> CSR back on the host, public API ----------
     e2e_steps = max(1, min(args.steps, 5))
-    h_offsets = torch.empty(q + 1, dtype=torch.int64).pin_memory()
-    h_indices = torch.empty(max(nnz, 1), dtype=torch.int32).pin_memory()
     h_root = torch.empty(32, dtype=torch.uint8).pin_memory()
+    host_out = binding.HostCsr(q, nnz)
 
     def e2e_step():
         t0 = time.perf_counter()
@@ -317,11 +354,8 @@ def run_ours(args) -> dict | None:
         h_root.copy_(bvh.nodes[64:96], non_blocking=True)   # root record (after the 64-byte header)
         torch.cuda.synchronize()
         t1 = time.perf_counter()
-        dq = h_queries.to(device, non_blocking=True)
-        off, idx = binding.query(bvh, dq, ws)      # reads nnz back, allocates, fills
-        h_offsets.copy_(off, non_blocking=True)
-        h_indices[: idx.numel()].copy_(idx, non_blocking=True)
-        torch.cuda.synchronize()
+        # queries H2D, single-pass search in chunks, each chunk's rows copied to the host while the next one is searched
+        binding.query_to_host(bvh, h_queries, host_out, row_capacity=cap, chunks=args.e2e_chunks)
         t2 = time.perf_counter()
         return t1 - t0, t2 - t1
 
@@ -334,54 +368,73 @@ def run_ours(args) -> dict | None:
         e2e_q += qq
     dist_barrier(world, device)
 
-    # ---- NEXT-1: ray queries through the same traversal kernel (only where a ray can hit something: box primitives)
-    rays_info = None
-    if is_box and rank == 0:
-        qr = int(min(max(q, 1), 1 << 20))
-        lo, hi = w.prims[:, :3].min(axis=0), w.prims[:, 3:].max(axis=0)
-        origins = workloads.uniform_cube(qr, seed=2001) * (hi - lo) * np.float32(1.2) + lo - (hi - lo) * np.float32(0.1)
-        h_rays = workloads.rays_at(origins.astype(np.float32), workloads.sphere_surface(qr, seed=2002), 0.0,
-                                   float(np.linalg.norm(hi - lo)))
-        d_rays = torch.from_numpy(h_rays).to(device)
-        wr = binding.QueryWorkspace(qr, device)
-        off_r, idx_r = binding.query(bvh, d_rays, wr)          # sizes the result
-        ridx = torch.empty(max(int(idx_r.numel()), 1), dtype=torch.int32, device=device)
-        rt = []
-        for _ in range(4):
-            flush.fill_(1)
-            r0 = ev()
-            binding.query(bvh, d_rays, wr, indices=ridx)
-            r1 = ev()
-            torch.cuda.synchronize()
-            rt.append(r0.elapsed_time(r1))
-        rms = float(np.median(rt[1:]))
-        rays_info = {"q": qr, "ms": round(rms, 4), "mrays_per_s": round(qr / (rms * 1e-3) / 1e6, 3),
-                     "hits_per_ray": round(int(off_r[qr].item()) / qr, 3),
-                     "what": "order + count + scan + fill of segments through the scene box, random directions"}
+    # ---- NEXT-1: operations at the leaf through the same traversal kernel (rank 0) -----------------------------------
+    next1 = {}
+    if rank == 0 and not args.no_extras:
+        def timed(fn, reps=4):
+            ts = []
+            for _ in range(reps):
+                flush.fill_(1)
+                a0 = ev()
+                fn()
+                a1 = ev()
+                torch.cuda.synchronize()
+                ts.append(a0.elapsed_time(a1))
+            return float(np.median(ts[1:]))
 
-    # ---- NEXT-2: the construction the paper compares itself with (Karras top-down + Algorithm 2 + separate box pass),
-    # same bounds / Morton / sort, same output bytes: how much the single bottom-up pass saves on this GPU
+        if kind == 0:
+            idx_n = torch.empty(max(q, 1), dtype=torch.int32, device=device)
+            key_n = torch.empty(max(q, 1), dtype=torch.float32, device=device)
+            ms_near = timed(lambda: binding.bvh_query_spheres_nearest(bvh.nodes, n, d_queries, q, ws.order, idx_n, key_n))
+            found = int((idx_n[:q] >= 0).sum().item())
+            ms_any = timed(lambda: binding.bvh_query_any_hit(bvh.nodes, n, d_queries, 0, q, ws.order, idx_n))
+            next1["nearest_within_radius"] = {"ms": round(ms_near, 4), "mqueries_per_s": round(q / (ms_near * 1e-3) / 1e6, 2),
+                                              "found": found}
+            next1["any_hit"] = {"ms": round(ms_any, 4), "mqueries_per_s": round(q / (ms_any * 1e-3) / 1e6, 2)}
+            next1["what"] = "same queries, Morton order from the step; no CSR (PAPER.md:56 'perform an operation')"
+        if is_box:
+            qr = int(min(max(q, 1), 1 << 20))
+            lo, hi = w.prims[:, :3].min(axis=0), w.prims[:, 3:].max(axis=0)
+            origins = workloads.uniform_cube(qr, seed=2001) * (hi - lo) * np.float32(1.2) + lo - (hi - lo) * np.float32(0.1)
+            h_rays = workloads.rays_at(origins.astype(np.float32), workloads.sphere_surface(qr, seed=2002), 0.0,
+                                       float(np.linalg.norm(hi - lo)))
+            d_rays = torch.from_numpy(h_rays).to(device)
+            wr = binding.QueryWorkspace(qr, device)
+            off_r, idx_r = binding.query(bvh, d_rays, wr)          # sizes the result
+            ridx = torch.empty(max(int(idx_r.numel()), 1), dtype=torch.int32, device=device)
+            rms = timed(lambda: binding.query(bvh, d_rays, wr, indices=ridx))
+            fi = torch.empty(qr, dtype=torch.int32, device=device)
+            ft = torch.empty(qr, dtype=torch.float32, device=device)
+            fms = timed(lambda: binding.bvh_query_rays_first_hit(bvh.nodes, n, d_rays, qr, wr.order, fi, ft))
+            next1["rays"] = {"q": qr, "csr_ms": round(rms, 4), "csr_mrays_per_s": round(qr / (rms * 1e-3) / 1e6, 3),
+                             "hits_per_ray": round(int(off_r[qr].item()) / qr, 3), "first_hit_ms": round(fms, 4),
+                             "first_hit_mrays_per_s": round(qr / (fms * 1e-3) / 1e6, 3),
+                             "what": "segments through the scene box, random directions: order + count + scan + fill, "
+                                     "and first hit alone on the same order"}
+
+    # ---- NEXT-2: the constructions the paper compares itself with, same bounds / Morton / sort -----------------------
     variant_info = None
     if rank == 0 and not args.no_variant:
-        vscratch = torch.empty(binding.bvh_variant_sizes(n, bits, 1), dtype=torch.uint8, device=device)
-        vnodes = torch.empty_like(bvh.nodes)
-        vt = []
-        for _ in range(6):
-            flush.fill_(1)
-            v0 = ev()
-            binding.bvh_build_variant(d_prims, is_box, n, bits, vnodes, vscratch, 1)
-            v1 = ev()
-            torch.cuda.synchronize()
-            vt.append(v0.elapsed_time(v1))
-        vms = float(np.median(vt[1:]))
         common = sum(acc[k] for k in build_names if k != "hierarchy") / args.steps     # staged: everything but the last step
-        variant_info = {"variant": "karras_topdown + algorithm2 ropes + separate box pass", "build_ms": round(vms, 4),
-                        "alg4_build_ms": round(acc["_build"] / args.steps, 4),
-                        "last_step_ms_estimate": {"variant": round(vms - common, 4),
-                                                  "alg4": round(acc["_build"] / args.steps - common, 4)},
-                        "what": "whole build as one call, median of 5; the last step = build minus the staged times of "
-                                "memset, bounds, Morton and sort (rank 0)"}
-        del vscratch, vnodes
+        variant_info = {"alg4_build_ms": round(acc["_build"] / args.steps, 4),
+                        "alg4_last_step_ms": round(acc["_build"] / args.steps - common, 4),
+                        "what": "whole build as one call, median of 5; last step = build minus the staged times of memset, "
+                                "bounds, Morton and sort (rank 0)"}
+        for variant, label in ((1, "karras_topdown + algorithm2 ropes + separate box pass"),
+                               (2, "algorithm3 (apetrei numbering, global atomics) + separate rope pass")):
+            vscratch = torch.empty(binding.bvh_variant_sizes(n, bits, variant), dtype=torch.uint8, device=device)
+            vnodes = torch.empty_like(bvh.nodes)
+            vt = []
+            for _ in range(6):
+                flush.fill_(1)
+                v0 = ev()
+                binding.bvh_build_variant(d_prims, is_box, n, bits, vnodes, vscratch, variant)
+                v1 = ev()
+                torch.cuda.synchronize()
+                vt.append(v0.elapsed_time(v1))
+            vms = float(np.median(vt[1:]))
+            variant_info[f"variant{variant}"] = {"what": label, "build_ms": round(vms, 4), "last_step_ms": round(vms - common, 4)}
+            del vscratch, vnodes
 
     # ---- reduce over ranks: time = max, units = sum -----------------------------------------------------------------
     keys = sorted(acc)
@@ -389,6 +442,8 @@ def run_ours(args) -> dict | None:
     acc = dict(zip(keys, mx[: len(keys)]))
     e2e_b, e2e_q = mx[len(keys)], mx[len(keys) + 1]
     n_all, q_all, nnz_all = sm
+    if shard:
+        n_all = float(n)                                    # one scene, replicated: the build does not scale in this mode
     if rank != 0:
         return None
 
@@ -406,12 +461,17 @@ def run_ours(args) -> dict | None:
     dk = kernels[dominant]
     build_gbs = model["build_total"] / (ms["_build"] * 1e-3) / 1e9
     query_gbs = model["query_total"] / (ms["_query"] * 1e-3) / 1e9
+    tp_ms = ms["order"] + ms["tp_count"] + ms["tp_scan"] + ms["tp_fill"]
     value = n_all / (ms["_build"] * 1e-3) / 1e6
+    full = not args.n and not args.q
+    traffic = NCU_TRAFFIC_BYTES.get((w.name, w.n, w.q), {}).get(dominant) if full and world == 1 else None
     line = {
         "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
-        "ms_per_step": round(ms["_step"], 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": round(ms["_step"], 4), "higher_is_better": True, "scaling": "strong" if shard else "weak",
+        "vs_baseline": None,
         "dtype": "u32 Morton codes / f32 boxes" if bits == 30 else "u64 Morton codes / f32 boxes", "data": "synthetic",
-        "config": config_dict(args, w, world, {"hits_per_query": round(nnz / max(q, 1), 2), "nnz": nnz}),
+        "config": config_dict(args, w, world, {"hits_per_query": round(nnz_all / max(q_all, 1), 2), "nnz": int(nnz_all),
+                                               "row_capacity": cap, "multi": args.multi if world > 1 else "single"}),
         "build": {"ms": round(ms["_build"], 4), "mprims_per_s": round(value, 2), "alg_bytes": int(model["build_total"]),
                   "gbs": round(build_gbs, 1), "frac_of_measured_peak": round(build_gbs / peak, 4),
                   "frac_of_8TBs": round(build_gbs / NOMINAL_HBM_GBS, 4),
@@ -419,24 +479,29 @@ def run_ours(args) -> dict | None:
         "query": {"ms": round(ms["_query"], 4), "mqueries_per_s": round(q_all / (ms["_query"] * 1e-3) / 1e6, 3),
                   "alg_bytes": int(model["query_total"]), "gbs": round(query_gbs, 1),
                   "frac_of_measured_peak": round(query_gbs / peak, 4), "frac_of_8TBs": round(query_gbs / NOMINAL_HBM_GBS, 4),
+                  "path": "single pass: order + collect + scan + rows_to_csr + fill_overflow (byte-identical CSR)",
                   "excluded": "nnz read-back and indices allocation (included in e2e)"},
+        "query_two_pass": {"ms": round(tp_ms, 4), "mqueries_per_s": round(q_all / (tp_ms * 1e-3) / 1e6, 3),
+                           "count_ms": round(ms["tp_count"], 4), "scan_ms": round(ms["tp_scan"], 4),
+                           "fill_ms": round(ms["tp_fill"], 4), "path": "order + count + scan + fill"},
         "roofline": {"bound": "hbm", "kernel": dominant, "achieved": dk["gbs"], "peak": peak, "unit": "GB/s",
-                     "frac": dk["frac"], "traffic": NCU_TRAFFIC_BYTES.get(dominant), "peak_source": peak_src,
+                     "frac": dk["frac"], "traffic": traffic, "peak_source": peak_src,
                      "alg_bytes_per_launch": dk["alg_bytes"], "ms_per_launch": dk["ms"]},
         "kernels": kernels,
         "build_staged_ms": round(ms["_build_staged"], 4),
         "gpu_launches": K * sum(launches_per_step.values()),
         "e2e": {"value": round(n_all / (e2e_b / e2e_steps) / 1e6, 2), "unit": UNIT,
                 "h2d_bytes_per_step": int(h_prims.numel() * 4 + h_queries.numel() * 4),
-                "d2h_bytes_per_step": int(32 + 8 + (q + 1) * 8 + nnz * 4), "steps": e2e_steps,
+                "d2h_bytes_per_step": int(32 + (q + 1) * 8 + nnz * 4), "steps": e2e_steps,
                 "build_ms": round(e2e_b / e2e_steps * 1e3, 3), "query_ms": round(e2e_q / e2e_steps * 1e3, 3),
-                "query_mqueries_per_s": round(q_all / (e2e_q / e2e_steps) / 1e6, 3),
-                "what": "pinned host prims -> H2D -> build -> root record D2H | pinned queries -> H2D -> count, scan, "
-                        "nnz read-back, alloc, fill -> CSR offsets+indices D2H; wall clock, through binding.Bvh/query"},
+                "query_mqueries_per_s": round(q_all / (e2e_q / e2e_steps) / 1e6, 3), "query_chunks": args.e2e_chunks,
+                "what": "pinned host prims -> H2D -> build -> root record D2H | pinned queries -> H2D -> single-pass search in "
+                        "chunks, each chunk's CSR rows copied D2H on a second stream while the next chunk is searched -> "
+                        "offsets + indices in pinned host memory; wall clock, through binding.Bvh / binding.query_to_host"},
         "clocks": clocks,
     }
-    if rays_info:
-        line["next1_rays"] = rays_info
+    if next1:
+        line["next1_operations"] = next1
     if variant_info:
         line["next2_variant"] = variant_info
     if world == 1 and not args.no_cpu_baseline:
@@ -474,7 +539,7 @@ def run_reference(args) -> dict | None:
 
     oracle.build()
     w = make_workload(args, 0)
-    ns, qs = min(w.n, 2_500_000), min(w.q, 10_000)
+    ns, qs = w.n, min(w.q, 10_000)          # the whole build (a few seconds for 10^7 primitives); a bounded query sample
     prims, queries = w.prims[:ns], w.queries[:qs]
 
     def step():
@@ -495,7 +560,7 @@ def run_reference(args) -> dict | None:
         tb += b
         tq += qq
     value = round(ns / (tb / args.steps) / 1e6, 3)
-    sample = (f"each step: oracle build of the first {ns} of {w.n} primitives + first {qs} of {w.q} queries on that tree; "
+    sample = (f"each step: oracle build of all {ns} primitives + the first {qs} of {w.q} queries on that tree; "
               f"serial, 1 of {os.cpu_count()} host cores")
     return {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
@@ -520,7 +585,11 @@ def main(argv=None):
     ap.add_argument("--n", type=int, default=0, help="override the primitive count (non-default: for quick checks)")
     ap.add_argument("--q", type=int, default=0, help="override the query count")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-variant", action="store_true", help="skip the NEXT-2 comparison build (Karras top-down)")
+    ap.add_argument("--no-variant", action="store_true", help="skip the NEXT-2 comparison builds (Karras top-down, Algorithm 3)")
+    ap.add_argument("--no-extras", action="store_true", help="skip the NEXT-1 operation timings (nearest, any hit, rays)")
+    ap.add_argument("--multi", choices=["replicas", "shard"], default="replicas",
+                    help="N > 1: independent replicas (weak scaling, default) or one query batch sharded over a replicated tree")
+    ap.add_argument("--e2e-chunks", type=int, default=8, help="query chunks of the end-to-end leg (search / D2H overlap)")
     args = ap.parse_args(argv)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     line = run_reference(args) if args.impl == "reference" else run_ours(args)

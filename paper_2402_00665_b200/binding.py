@@ -373,6 +373,64 @@ def query(bvh: Bvh, queries: torch.Tensor, ws: QueryWorkspace | None = None, ind
     return offsets, (indices if nnz is None else indices[:nnz])
 
 
+class HostCsr:
+    """Pinned host buffers that receive a CSR result: ``offsets`` int64[q + 1], ``indices`` int32[capacity]; ``nnz`` is
+    set by :func:`query_to_host`."""
+
+    def __init__(self, q: int, capacity: int):
+        self.q = int(q)
+        self.offsets = torch.empty(self.q + 1, dtype=torch.int64).pin_memory()
+        self.indices = torch.empty(max(int(capacity), 1), dtype=torch.int32).pin_memory()
+        self.nnz = 0
+
+
+def query_to_host(bvh: Bvh, h_queries: torch.Tensor, out: HostCsr, row_capacity: int, chunks: int = 8, ordered: bool = True):
+    """End-to-end range search from pinned host queries to a CSR in pinned host memory.
+
+    The result (4 bytes per hit) is usually far larger than the queries, and its device->host copy far longer than the
+    search; so the batch is searched in ``chunks`` contiguous blocks (single-pass path: order, collect, scan,
+    rows_to_csr, fill_overflow on the current stream) and each block's rows are copied to the host on a second stream
+    while the next block is searched.  Returns ``out`` with offsets[0..q] and indices[0..nnz) filled, synchronised."""
+    if not (h_queries.is_pinned() and not h_queries.is_cuda):
+        raise BvhError("query_to_host takes the queries in pinned host memory")
+    q = int(h_queries.shape[0])
+    if out.q != q:
+        raise BvhError(f"HostCsr was made for {out.q} queries, {q} given")
+    dev = bvh.nodes.device
+    chunks = max(1, min(int(chunks), max(q, 1)))
+    bounds = [(c * q // chunks, (c + 1) * q // chunks) for c in range(chunks)]
+    qmax = max(hi - lo for lo, hi in bounds) if q > 0 else 0
+    ws = QueryWorkspace(qmax, dev)
+    cap = int(row_capacity)
+    rows = torch.empty(max(qmax, 1) * cap, dtype=torch.int32, device=dev)
+    main = torch.cuda.current_stream()
+    copy = torch.cuda.Stream(device=dev)
+    keep, base = [], 0
+    for lo, hi in bounds:
+        if hi == lo:
+            continue
+        dq = h_queries[lo:hi].to(dev, non_blocking=True)
+        off, idx = query(bvh, dq, ws, ordered=ordered, row_capacity=cap, rows=rows)     # reads this block's nnz back
+        nnz = int(idx.numel())
+        if base + nnz > out.indices.numel():
+            raise BvhError(f"HostCsr holds {out.indices.numel()} indices, more are needed")
+        off_g = off[:-1] + base                                                           # global positions of the block's rows
+        done = torch.cuda.Event()
+        done.record(main)
+        with torch.cuda.stream(copy):
+            copy.wait_event(done)
+            out.offsets[lo:hi].copy_(off_g, non_blocking=True)
+            if nnz:
+                out.indices[base: base + nnz].copy_(idx[:nnz], non_blocking=True)
+        keep.append((off_g, idx, dq))                                                     # alive until the copies are done
+        base += nnz
+    copy.synchronize()
+    main.synchronize()
+    out.offsets[q] = base
+    out.nnz = base
+    return out
+
+
 def reduce_query(bvh: Bvh, queries: torch.Tensor, op: str, ws: QueryWorkspace | None = None, ordered: bool = True):
     """"Perform an operation" at the leaves instead of storing rows.  op = "nearest" (spheres: index and
     squared distance of the nearest primitive within the radius), "first_hit" (rays: index and entry parameter of the

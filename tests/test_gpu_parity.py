@@ -490,6 +490,24 @@ def test_reduce_modes_empty_and_stale(B):
     assert idx.cpu().tolist() == [-1, -1] and bool(torch.isinf(key).all())
 
 
+def test_query_to_host_pipeline_equals_query(B, oracle_lib):
+    """End-to-end helper: pinned host queries -> chunked single-pass search -> CSR in pinned host memory, copies
+    overlapped with the search of the next chunk.  Same CSR as the oracle, whatever the chunking."""
+    w = W.make("C3", n=150_000, q=30_001, radius=0.004)
+    o = oracle_lib.build_bvh(w.prims, w.morton_bits)
+    ooff, oidx = oracle_lib.query_spheres_tree(o, w.queries)
+    bvh = gpu_build(B, w.prims, w.morton_bits)
+    hq = torch.from_numpy(w.queries).pin_memory()
+    cap = (int(np.diff(ooff).max()) + 7) // 8 * 8
+    for chunks, c in ((1, cap), (7, cap), (8, 8)):
+        out = B.HostCsr(w.q, int(ooff[-1]))
+        B.query_to_host(bvh, hq, out, row_capacity=c, chunks=chunks)
+        assert out.nnz == int(ooff[-1])
+        assert np.array_equal(out.offsets.numpy(), ooff) and np.array_equal(out.indices.numpy()[: out.nnz], oidx)
+    with pytest.raises(B.BvhError):
+        B.query_to_host(bvh, hq, B.HostCsr(w.q, 10), row_capacity=cap)          # too small for the result
+
+
 def test_empty_inputs(B):
     bvh = B.Bvh(0, 30)
     bvh.build(torch.zeros((0, 3), dtype=torch.float32, device="cuda"))
