@@ -1,6 +1,7 @@
 // bounds_morton.cu -- K1 scene bounds (D1) and K2 Morton encoding (D2) fused with the
 // digit histograms the one-sweep sort needs.  Both are single streaming passes over the input.
 #include "common.cuh"
+#include "device_helpers.cuh"
 
 namespace bvh {
 
@@ -123,32 +124,6 @@ cudaError_t launch_scene_bounds(const float* prim, int n, bool is_box, Header* h
 // and block: the sort then needs no histogram pass of its own.
 // ---------------------------------------------------------------------------------------------------
 constexpr int kMortonThreads = 256;
-
-__device__ __forceinline__ uint32_t spread10(uint32_t x) {
-  x = (x | (x << 16)) & 0x030000FFu;
-  x = (x | (x << 8)) & 0x0300F00Fu;
-  x = (x | (x << 4)) & 0x030C30C3u;
-  x = (x | (x << 2)) & 0x09249249u;
-  return x;
-}
-__device__ __forceinline__ uint64_t spread21(uint32_t v) {
-  uint64_t x = v & 0x1fffffu;
-  x = (x | (x << 32)) & 0x001f00000000ffffull;
-  x = (x | (x << 16)) & 0x001f0000ff0000ffull;
-  x = (x | (x << 8)) & 0x100f00f00f00f00full;
-  x = (x | (x << 4)) & 0x10c30c30c30c30c3ull;
-  x = (x | (x << 2)) & 0x1249249249249249ull;
-  return x;
-}
-
-__device__ __forceinline__ uint32_t quantise(float lo, float hi, float slo, float shi, float scale, uint32_t cell_max) {
-  const float c = __fmul_rn(__fadd_rn(lo, hi), 0.5f);
-  const float e = __fsub_rn(shi, slo);
-  float t = 0.0f;
-  if (e > 0.0f) t = __fdiv_rn(__fsub_rn(c, slo), e);
-  const uint32_t q = __float2uint_rz(__fmul_rn(t, scale));
-  return min(q, cell_max);
-}
 
 // PRIM_FLOATS: 3 = points, 6 = boxes {min,max}, 4 = sphere queries {x,y,z,r} (centre only; used to order queries),
 // 8 = ray queries {o.xyz, d.xyz, tmin, tmax} (origin only; used to order queries).

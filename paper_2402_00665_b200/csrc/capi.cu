@@ -232,6 +232,11 @@ static int query(const void* nodes, int64_t n, const float* queries, int64_t q, 
   return BVH_OK;
 }
 
+#ifndef BVH_SMALL_ORDER_Q
+#define BVH_SMALL_ORDER_Q 8192
+#endif
+constexpr int64_t kSmallOrderQ = BVH_SMALL_ORDER_Q;
+
 __global__ void iota_kernel(uint32_t* order, int64_t q) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < q) order[i] = (uint32_t)i;
@@ -246,7 +251,9 @@ static int query_order(const void* nodes, int64_t n, const float* queries, int64
   if (q == 0) return BVH_OK;
   if (!order) return BVH_ERR_INVALID_ARGUMENT;
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-  if (n == 0) {  // no frame: identity
+  // no frame (n = 0), or a batch so small that it is bound by the number of dependent launches and gains nothing from
+  // a schedule (the whole hierarchy it touches stays in L2): identity, one launch instead of five
+  if (n == 0 || q <= kSmallOrderQ) {
     iota_kernel<<<(unsigned)((q + 255) / 256), 256, 0, stream>>>(order, q);
     return check_launch();
   }

@@ -111,11 +111,15 @@ __device__ inline void load_scene_bounds(const Header* h, float out[6]) {
 // costs more than it gains on the large configs (C3 765 us), because waiting blocks of the next kernel then hold
 // registers and shared memory the tail of the running one needs.
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-#ifdef BVH_PDL_EARLY_TRIGGER
-__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
-#else
-__device__ __forceinline__ void pdl_trigger() {}
+// Small grids (the launch-bound regime: n up to a few 10^5) do trigger their dependents, right after their own wait:
+// the next kernel's blocks then sit resident at their pdl_wait() while this grid runs, and start the moment it has
+// completed, instead of being launched then.  A grid that fills the GPU does not (see above).
+#ifndef BVH_PDL_TRIGGER_MAX_BLOCKS
+#define BVH_PDL_TRIGGER_MAX_BLOCKS 296
 #endif
+__device__ __forceinline__ void pdl_trigger() {
+  if (gridDim.x <= BVH_PDL_TRIGGER_MAX_BLOCKS) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
 template <typename... KArgs, typename... Args>
 inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args&&... args) {
   cudaLaunchConfig_t cfg{};

@@ -8,6 +8,7 @@
 //
 // Line references "L#" are the pseudo-code line numbers of Algorithm 4 in the paper.
 #include "common.cuh"
+#include "device_helpers.cuh"
 
 namespace bvh {
 
@@ -20,58 +21,6 @@ namespace bvh {
 constexpr int kHierThreads = 128;               // threads of a level-1 block
 constexpr int kHierWindow = BVH_HIER_WINDOW;    // leaves of a level-1 window (one block); a multiple of kHierThreads
 static_assert(kHierWindow % kHierThreads == 0, "a level-1 window is a whole number of 32-leaf groups per warp");
-
-// delta*(i): XOR of adjacent sorted codes; equal codes fall back to the XOR of the
-// sorted positions (augmented key, readings G1/G5); +infinity outside [0, n-2].  The
-// value is packed so that one unsigned compare orders it (G14): position band < code band < infinity.
-template <typename KeyT>
-struct Delta;
-template <>
-struct Delta<uint32_t> {
-  using T = uint32_t;
-  static constexpr T kInf = 0xFFFFFFFFu;
-  __device__ static __forceinline__ T make(uint32_t a, uint32_t b, int i) {
-    const uint32_t x = a ^ b;                              // < 2^30
-    return x ? (x + 0x40000000u) : (uint32_t)(i ^ (i + 1));  // codes and positions < 2^30 (capi.cu rejects n >= 2^30)
-  }
-};
-// 64-bit codes: the value kept is the INDEX of the highest differing bit, not the XOR itself.  Every comparison
-// Algorithm 4 makes is between delta*(l-1) and delta*(r) of a node's range [l, r], or between delta*(r) and
-// delta*(r+1) (L8, L26); in both cases the two XORs cannot share their highest set bit (sorted keys: a key cannot
-// have that bit both set, as the upper key of one pair, and clear, as the lower key of the other, under the
-// same prefix), so the order of the XORs is the order of their highest bits -- Karras' common-prefix length
-// (PAPER.md:97).  One 32-bit word instead of two: half the shuffles and shared memory of the 63-bit build.
-template <>
-struct Delta<uint64_t> {
-  using T = uint32_t;
-  static constexpr T kInf = 0xFFFFFFFFu;
-  __device__ static __forceinline__ T make(uint64_t a, uint64_t b, int i) {
-    const uint64_t x = a ^ b;                              // <= 2^63 - 1
-    return x ? (0x40000000u + (uint32_t)(63 - __clzll((long long)x))) : (uint32_t)(i ^ (i + 1));
-  }
-};
-
-template <typename KeyT>
-__device__ __forceinline__ typename Delta<KeyT>::T delta_star(const KeyT* __restrict__ codes, int i, int n) {
-  if (i < 0 || i >= n - 1) return Delta<KeyT>::kInf;
-  return Delta<KeyT>::make(codes[i], codes[i + 1], i);
-}
-
-__device__ __forceinline__ void store_node(Node* nodes, int idx, const float lo[3], const float hi[3], int left, int rope) {
-  // one 256-bit store = one full 32-byte sector (STG.E.ENL2.256, sm_100)
-  asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(nodes + idx), "f"(lo[0]), "f"(lo[1]), "f"(lo[2]),
-               "f"(__int_as_float(left)), "f"(hi[0]), "f"(hi[1]), "f"(hi[2]), "f"(__int_as_float(rope))
-               : "memory");
-}
-
-// Leaf record i (layout in common.cuh): a point leaf stores the point once.
-template <bool IS_BOX>
-__device__ __forceinline__ void store_leaf(char* leaves, int i, const float lo[3], const float hi[3], uint32_t payload) {
-  if (IS_BOX)
-    store_node(reinterpret_cast<Node*>(leaves), i, lo, hi, (int)payload, 0);
-  else
-    reinterpret_cast<float4*>(leaves)[i] = make_float4(lo[0], lo[1], lo[2], __uint_as_float(payload));
-}
 
 // Box of node `idx` of the unified index space, through L2 (written by another block or an earlier kernel).
 __device__ __forceinline__ void load_box_cg(const char* nodes, int n, int leaf_kind, int idx, float lo[3], float hi[3]) {

@@ -17,6 +17,7 @@
 // a path without bounds predicates, positions are 32-bit, values are loaded after the ranking so that
 // fewer registers are live (4 CTAs of 256 threads per SM).
 #include "common.cuh"
+#include "device_helpers.cuh"
 
 namespace bvh {
 
@@ -74,37 +75,6 @@ struct SortSmem {
   KeyT keys[SortCfg<KeyT>::TILE];
   uint32_t vals[SortCfg<KeyT>::TILE];
 };
-
-// Lanes of the warp whose digit equals this lane's: AND over the 8 digit bits of (ballot of the bit) or its
-// complement.  `peers` enters as the mask of participating lanes.  MATCH_ANY: one MATCH.ANY instruction instead;
-// its cost grows with the number of distinct digits in the warp, so it only pays for the most significant
-// digit (few distinct values among 32 keys that are neighbours in the input; measured on C3: 59 vs 68 us for
-// that pass, but 105 vs 75 us for the least significant one).
-template <bool MATCH_ANY>
-__device__ __forceinline__ uint32_t match_digit(uint32_t d, uint32_t peers) {
-  if (MATCH_ANY) {
-    peers &= __match_any_sync(0xffffffffu, d);
-  } else {
-#pragma unroll
-    for (int b = 0; b < 8; ++b) {
-      // four SASS instructions per bit: bit test -> predicate, VOTE, and one predicated LOP3 per polarity
-      asm volatile(
-          "{\n\t"
-          ".reg .pred p;\n\t"
-          ".reg .b32 t, bal;\n\t"
-          "and.b32 t, %1, %2;\n\t"
-          "setp.ne.u32 p, t, 0;\n\t"
-          "vote.sync.ballot.b32 bal, p, 0xffffffff;\n\t"
-          "@p and.b32 %0, %0, bal;\n\t"
-          "@!p not.b32 bal, bal;\n\t"
-          "@!p and.b32 %0, %0, bal;\n\t"
-          "}"
-          : "+r"(peers)
-          : "r"(d), "r"(1u << b));
-    }
-  }
-  return peers;
-}
 
 template <typename KeyT, bool IOTA, bool FULL, bool TOP>
 __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_out,

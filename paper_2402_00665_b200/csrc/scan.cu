@@ -81,6 +81,28 @@ __global__ void __launch_bounds__(kScanThreads) scan_apply_kernel(const int32_t*
   }
 }
 
+// q <= kScanTile: the whole scan in one block (small batches are bound by the number of dependent launches).
+__global__ void __launch_bounds__(kScanThreads) scan_single_tile_kernel(const int32_t* __restrict__ counts, int64_t q,
+                                                                        int64_t* __restrict__ offsets) {
+  __shared__ int64_t s_warp[kScanThreads / 32];
+  const int64_t base = (int64_t)threadIdx.x * kScanItems;   // blocked arrangement
+  int32_t c[kScanItems];
+  int64_t v = 0;
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) {
+    c[k] = (base + k < q) ? counts[base + k] : 0;
+    v += c[k];
+  }
+  int64_t total;
+  int64_t run = block_exclusive_scan(v, &total, s_warp);
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) {
+    if (base + k < q) offsets[base + k] = run;
+    run += c[k];
+  }
+  if (threadIdx.x == 0) offsets[q] = total;
+}
+
 __global__ void scan_empty_kernel(int64_t* offsets) { offsets[0] = 0; }
 
 size_t scan_scratch_bytes(int64_t q) {
@@ -91,6 +113,10 @@ size_t scan_scratch_bytes(int64_t q) {
 void launch_scan(const int32_t* counts, int64_t q, int64_t* offsets, void* scratch, cudaStream_t stream) {
   if (q == 0) {
     scan_empty_kernel<<<1, 1, 0, stream>>>(offsets);
+    return;
+  }
+  if (q <= kScanTile) {
+    scan_single_tile_kernel<<<1, kScanThreads, 0, stream>>>(counts, q, offsets);
     return;
   }
   const int64_t tiles = (q + kScanTile - 1) / kScanTile;
