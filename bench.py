@@ -45,7 +45,9 @@ NOMINAL_HBM_GBS = 8000.0   # the denominator BASELINE.json north_star names
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of a kernel from the `ncu --set full` captures
 # summarised in profiles/, keyed by (workload, n, q): `roofline.traffic` is null for any other workload or size.
 NCU_TRAFFIC_BYTES = {
-    ("C3", 10_000_000, 1_000_000): {"fill": 4_259_000_000, "count": 327_110_000},   # profiles/r01c_ncu.md rows 17, 13
+    # profiles/r02_ncu.md rows 13 (collect), 17 (rows_to_csr), 19 (count), 23 (fill), 6 (hierarchy, level 1): DRAM rd + wr
+    ("C3", 10_000_000, 1_000_000): {"collect": 4_324_314_000, "rows_to_csr": 5_007_352_000, "count": 390_046_000,
+                                    "fill": 4_343_356_000, "hierarchy": 1_330_786_000},
 }
 
 
