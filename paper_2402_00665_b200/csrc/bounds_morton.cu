@@ -37,38 +37,55 @@ __global__ void __launch_bounds__(kBoundsThreads) scene_bounds_kernel(const floa
   pdl_wait();
   pdl_trigger();
   const float inf = __int_as_float(0x7f800000);
-  float mn[3][4], mx[3][4];
+  // (load slot j, component c) of a lane sees the scalar with flat index 4 * (32 j + lane) + c of the chunk, whose role is
+  // that index modulo 6 = (2 j + c + 4 lane) mod 6: the twelve (j, c) fall into six classes k = (2 j + c) mod 6 of two
+  // members each, whatever the lane.  Six running mins and six maxes per thread.
+  float mn[6], mx[6];
 #pragma unroll
-  for (int j = 0; j < 3; ++j)
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-      mn[j][c] = inf;
-      mx[j][c] = -inf;
-    }
+  for (int k = 0; k < 6; ++k) {
+    mn[k] = inf;
+    mx[k] = -inf;
+  }
   const int lane = threadIdx.x & 31;
   const int64_t warp_global = ((int64_t)blockIdx.x * kBoundsThreads + threadIdx.x) >> 5;
   const int64_t num_warps = ((int64_t)gridDim.x * kBoundsThreads) >> 5;
   const int64_t nvec = nfloats >> 2;          // whole float4s
   const int64_t nchunks = nvec / 96;          // whole 96-float4 chunks
   const float4* __restrict__ v = reinterpret_cast<const float4*>(prim);
-  for (int64_t ch = warp_global; ch < nchunks; ch += num_warps) {
+  auto fold = [&](const float4 (&x)[3]) {
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      const float f[4] = {x[j].x, x[j].y, x[j].z, x[j].w};
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const int k = (2 * j + c) % 6;
+        mn[k] = fminf(mn[k], f[c]);
+        mx[k] = fmaxf(mx[k], f[c]);
+      }
+    }
+  };
+  int64_t ch = warp_global;
+  for (; ch + num_warps < nchunks; ch += 2 * num_warps) {   // two chunks per turn: six 128-bit loads in flight per lane
     const float4* p = v + ch * 96 + lane;
-    float4 x[3];
+    const float4* p2 = v + (ch + num_warps) * 96 + lane;
+    float4 x[3], y[3];
 #pragma unroll
     for (int j = 0; j < 3; ++j) x[j] = __ldcs(p + j * 32);   // streaming: read exactly once
 #pragma unroll
-    for (int j = 0; j < 3; ++j) {
-      mn[j][0] = fminf(mn[j][0], x[j].x); mx[j][0] = fmaxf(mx[j][0], x[j].x);
-      mn[j][1] = fminf(mn[j][1], x[j].y); mx[j][1] = fmaxf(mx[j][1], x[j].y);
-      mn[j][2] = fminf(mn[j][2], x[j].z); mx[j][2] = fmaxf(mx[j][2], x[j].z);
-      mn[j][3] = fminf(mn[j][3], x[j].w); mx[j][3] = fmaxf(mx[j][3], x[j].w);
-    }
+    for (int j = 0; j < 3; ++j) y[j] = __ldcs(p2 + j * 32);
+    fold(x);
+    fold(y);
+  }
+  for (; ch < nchunks; ch += num_warps) {
+    const float4* p = v + ch * 96 + lane;
+    float4 x[3];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) x[j] = __ldcs(p + j * 32);
+    fold(x);
   }
   float lo[3] = {inf, inf, inf}, hi[3] = {-inf, -inf, -inf};
 #pragma unroll
-  for (int j = 0; j < 3; ++j)
-#pragma unroll
-    for (int c = 0; c < 4; ++c) fold_role((4 * (j * 32 + lane) + c) % 6, is_box, mn[j][c], mx[j][c], lo, hi);
+  for (int k = 0; k < 6; ++k) fold_role((k + 4 * lane) % 6, is_box, mn[k], mx[k], lo, hi);
   // tail: scalars after the last whole chunk
   const int64_t tail0 = nchunks * 96 * 4;
   for (int64_t e = tail0 + (int64_t)blockIdx.x * kBoundsThreads + threadIdx.x; e < nfloats;
@@ -116,7 +133,7 @@ cudaError_t launch_scene_bounds(const float* prim, int n, bool is_box, Header* h
 }
 
 // ---------------------------------------------------------------------------------------------------
-// K2.  One thread per primitive.  D2: centroid c = (min + max) * 0.5, t = (c - lo) / (hi - lo) (0 when
+// K2.  One thread per group of four points / two boxes (one query in the query-ordering variants).  D2: centroid c = (min + max) * 0.5, t = (c - lo) / (hi - lo) (0 when
 // the extent is 0), cell = min(trunc(t * 2^b), 2^b - 1), all fp32 round-to-nearest with explicit
 // intrinsics so that nvcc cannot contract them.  Bits are spread with magic-number masks; x is the
 // most significant axis of each triple.  The same pass accumulates the 256-bin histogram of every
@@ -151,21 +168,8 @@ __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __r
   constexpr int B = (sizeof(KeyT) == 4) ? 10 : 21;
   const float scale = (float)(1u << B);
   const uint32_t cell_max = (1u << B) - 1u;
-  for (int64_t i = (int64_t)blockIdx.x * kMortonThreads + threadIdx.x; i < n; i += (int64_t)gridDim.x * kMortonThreads) {
-    float lo[3], hi[3];
-    if (PRIM_FLOATS == 6) {
-      const float2* p = reinterpret_cast<const float2*>(prim + 6 * i);
-      const float2 a = __ldcs(p), b = __ldcs(p + 1), c = __ldcs(p + 2);
-      lo[0] = a.x; lo[1] = a.y; lo[2] = b.x; hi[0] = b.y; hi[1] = c.x; hi[2] = c.y;
-    } else if (PRIM_FLOATS == 4 || PRIM_FLOATS == 8) {
-      const float4 v = __ldg(reinterpret_cast<const float4*>(prim) + (PRIM_FLOATS / 4) * i);
-      lo[0] = hi[0] = v.x; lo[1] = hi[1] = v.y; lo[2] = hi[2] = v.z;
-    } else {
-      const float* p = prim + 3 * i;
-      lo[0] = hi[0] = __ldcs(p);
-      lo[1] = hi[1] = __ldcs(p + 1);
-      lo[2] = hi[2] = __ldcs(p + 2);
-    }
+  // code of one primitive (D2) + its digits into the block's histograms
+  auto encode = [&](float lo[3], float hi[3]) -> KeyT {
     uint32_t cell[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
@@ -175,14 +179,62 @@ __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __r
       }
       cell[a] = quantise(lo[a], hi[a], scene[a], scene[3 + a], scale, cell_max);
     }
-    KeyT code;
-    if (sizeof(KeyT) == 4)
-      code = (KeyT)((spread10(cell[0]) << 2) | (spread10(cell[1]) << 1) | spread10(cell[2]));
-    else
-      code = (KeyT)((spread21(cell[0]) << 2) | (spread21(cell[1]) << 1) | spread21(cell[2]));
-    codes[i] = code;
+    const KeyT code = morton_code<KeyT>(cell);
 #pragma unroll
     for (int p = 0; p < PASSES; ++p) atomicAdd(&s_hist[p * 256 + (int)((code >> (8 * p)) & 0xFF)], 1u);
+    return code;
+  };
+  const int64_t tid0 = (int64_t)blockIdx.x * kMortonThreads + threadIdx.x, stride = (int64_t)gridDim.x * kMortonThreads;
+  int64_t done = 0;                                       // primitives [0, done) are covered by the vector loop
+  if (PRIM_FLOATS == 3 || PRIM_FLOATS == 6) {
+    // 12 consecutive floats = three 128-bit loads per thread = four points or two boxes: a quarter of the load
+    // instructions of one scalar load per coordinate, and 48 bytes in flight per thread instead of 12 (the kernel
+    // waits on its loads, not on its arithmetic).  The codes leave as one or two 128-bit stores.
+    constexpr int PG = (PRIM_FLOATS == 3) ? 4 : 2;        // primitives per group
+    const int64_t groups = n / PG;
+    const float4* __restrict__ v = reinterpret_cast<const float4*>(prim);
+    for (int64_t g = tid0; g < groups; g += stride) {
+      const float4 x0 = __ldcs(v + 3 * g), x1 = __ldcs(v + 3 * g + 1), x2 = __ldcs(v + 3 * g + 2);
+      const float f[12] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w, x2.x, x2.y, x2.z, x2.w};
+      KeyT c[PG];
+#pragma unroll
+      for (int k = 0; k < PG; ++k) {
+        float lo[3], hi[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+          lo[a] = f[(PRIM_FLOATS == 3 ? 3 : 6) * k + a];
+          hi[a] = f[(PRIM_FLOATS == 3 ? 3 : 6) * k + (PRIM_FLOATS == 3 ? 0 : 3) + a];
+        }
+        c[k] = encode(lo, hi);
+      }
+      if (sizeof(KeyT) == 4) {
+        if (PG == 4)
+          reinterpret_cast<uint4*>(codes)[g] = make_uint4((uint32_t)c[0], (uint32_t)c[1], (uint32_t)c[2], (uint32_t)c[PG - 1]);
+        else
+          reinterpret_cast<uint2*>(codes)[g] = make_uint2((uint32_t)c[0], (uint32_t)c[1]);
+      } else {
+#pragma unroll
+        for (int k = 0; k < PG; k += 2)
+          reinterpret_cast<ulonglong2*>(codes)[(PG / 2) * g + k / 2] = make_ulonglong2((unsigned long long)c[k], (unsigned long long)c[k + 1]);
+      }
+    }
+    done = groups * PG;
+  }
+  for (int64_t i = done + tid0; i < n; i += stride) {     // the last n % PG primitives; every query of the FROM_ROOT variants
+    float lo[3], hi[3];
+    if (PRIM_FLOATS == 6) {
+      const float* p = prim + 6 * i;
+      lo[0] = p[0]; lo[1] = p[1]; lo[2] = p[2]; hi[0] = p[3]; hi[1] = p[4]; hi[2] = p[5];
+    } else if (PRIM_FLOATS == 4 || PRIM_FLOATS == 8) {
+      const float4 q4 = __ldg(reinterpret_cast<const float4*>(prim) + (PRIM_FLOATS / 4) * i);
+      lo[0] = hi[0] = q4.x; lo[1] = hi[1] = q4.y; lo[2] = hi[2] = q4.z;
+    } else {
+      const float* p = prim + 3 * i;
+      lo[0] = hi[0] = p[0];
+      lo[1] = hi[1] = p[1];
+      lo[2] = hi[2] = p[2];
+    }
+    codes[i] = encode(lo, hi);
   }
   __syncthreads();
   for (int i = threadIdx.x; i < PASSES * 256; i += kMortonThreads) {
@@ -191,16 +243,18 @@ __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __r
   }
 }
 
-static unsigned morton_grid(int n) {
-  int64_t blocks = ((int64_t)n + kMortonThreads - 1) / kMortonThreads;
+static unsigned morton_grid(int n, int per_thread = 1) {
+  const int64_t units = ((int64_t)n + per_thread - 1) / per_thread;
+  int64_t blocks = (units + kMortonThreads - 1) / kMortonThreads;
   const int64_t cap = (int64_t)kNumSMs * 8;
   if (blocks > cap) blocks = cap;
+  if (blocks < 1) blocks = 1;
   return (unsigned)blocks;
 }
 
 cudaError_t launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
                    uint32_t* hist, cudaStream_t stream) {
-  const unsigned g = morton_grid(n);
+  const unsigned g = morton_grid(n, is_box ? 2 : 4);
   if (morton_bits == 30) {
     if (is_box)
       return launch_pdl(morton_kernel<uint32_t, 4, 6, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint32_t*)codes, hist);
