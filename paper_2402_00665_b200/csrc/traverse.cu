@@ -32,14 +32,18 @@
 
 namespace bvh {
 
-#ifndef BVH_TRAV_CTAS
-#define BVH_TRAV_CTAS 8
+#ifndef BVH_TRAV_THREADS
+#define BVH_TRAV_THREADS 128
+#endif
+#ifndef BVH_TRAV_WARPS_PER_SM
+#define BVH_TRAV_WARPS_PER_SM 32
 #endif
 #ifndef BVH_SCAN_LEAVES
 #define BVH_SCAN_LEAVES 128
 #endif
-constexpr int kTravThreads = 128;
-constexpr int kTravCtasPerSm = BVH_TRAV_CTAS;
+constexpr int kTravThreads = BVH_TRAV_THREADS;         // queries of a block (one per thread)
+static_assert(kTravThreads % 32 == 0 && kTravThreads >= 32 && kTravThreads <= 1024, "whole warps");
+constexpr int kTravCtasPerSm = BVH_TRAV_WARPS_PER_SM * 32 / kTravThreads;   // resident blocks asked of the register allocator
 constexpr int kScanLeaves = BVH_SCAN_LEAVES;
 
 struct NodeRec {
@@ -159,13 +163,13 @@ struct BoxQuery {
 // with d != 0: inv = 1 / d, t1 = (lo - o) * inv, t2 = (hi - o) * inv clip [tmin, tmax] to [min(t1,t2), max(t1,t2)];
 // per axis with d == 0: lo <= o <= hi.  Hit iff the clipped interval is not empty.  1 / d is computed once per ray
 // (the same IEEE division the oracle does per test); an axis with d == 0 keeps inv = 0 and is tested by bounds.
-#ifndef BVH_TRAV_CTAS_RAYS
-#define BVH_TRAV_CTAS_RAYS 6
+#ifndef BVH_TRAV_WARPS_PER_SM_RAYS
+#define BVH_TRAV_WARPS_PER_SM_RAYS 24
 #endif
 struct RayQuery {
   static constexpr bool kHasKey = true;                    // D11: candidates are ranked by where the ray enters them
   static constexpr int kWords = 8;
-  static constexpr int kCtasPerSm = BVH_TRAV_CTAS_RAYS;   // the ray state does not fit the 64 registers of 8 CTAs per SM
+  static constexpr int kCtasPerSm = BVH_TRAV_WARPS_PER_SM_RAYS * 32 / kTravThreads;   // the ray state does not fit 64 registers
   float o[3], inv[3], tmin, tmax;
   uint32_t par;        // bit a: d[a] == 0
   __device__ __forceinline__ void load(const float* __restrict__ q, int64_t j) {
@@ -287,9 +291,6 @@ struct TraverseArgs {
   int32_t* out;              // fill: indices; collect: rows
   int64_t cap;               // collect: entries per row.  fill with only_over: only rows with counts[j] > cap are filled
   int only_over;
-  int64_t num_chunks;
-  int ctas_per_sm;
-  int num_sms;
 };
 
 // Row output of the fill / collect passes.  The hits of a row arrive a few at a time (one scan step of 32 leaves gives
@@ -367,18 +368,19 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
   const uint32_t lt_mask = (1u << lane) - 1u;
   int* const buf = s_buf + (STORE ? (threadIdx.x >> 5) * kRangeBufInts : 0);
   const int cap = (MODE == kModeCollect) ? (int)A.cap : 0x7fffffff;   // row positions >= cap are not stored
-  const int64_t sm_slot = blockIdx.x % A.num_sms;
-  const int64_t r = blockIdx.x / A.num_sms;
   float contain_extent = 0.0f;
   if (kContainment) {
     const NodesHeader* h = reinterpret_cast<const NodesHeader*>(nodes);
     const float e = fmaxf(fmaxf(h->scene_hi[0] - h->scene_lo[0], h->scene_hi[1] - h->scene_lo[1]), h->scene_hi[2] - h->scene_lo[2]);
     contain_extent = e * cbrtf((float)kContainMinLeaves / (float)n);   // side of a cube holding that share of a uniform scene
   }
-  for (int64_t k = 0;; ++k) {
-    const int64_t chunk = (k * A.num_sms + sm_slot) * A.ctas_per_sm + r;
-    if (chunk >= A.num_chunks) break;
-    const int64_t t = chunk * kTravThreads + threadIdx.x;
+  {
+    // One block per chunk of kTravThreads consecutive positions of the (Morton-ordered) query list.  The hardware's block
+    // scheduler hands the chunks out in order as blocks retire, which balances queries of very different cost (C3: 100
+    // to 2800 hits) and keeps the chunks that run at the same time neighbours on the curve.  Round 1 ran a persistent
+    // grid with a static, SM-local assignment of chunks instead: 26-35 % slower on C3 (4.26 / 6.42 ms count / fill
+    // against 3.3 / 4.4), because blocks whose chunks were expensive finished long after the others.
+    const int64_t t = (int64_t)blockIdx.x * kTravThreads + threadIdx.x;
     bool have = t < A.q;
     const int64_t j = have ? (order ? (int64_t)order[t] : t) : 0;
     if (MODE == kModeFill && A.only_over) have = have && (int64_t)A.counts[j] > A.cap;
@@ -642,14 +644,9 @@ __global__ void __launch_bounds__(kTravThreads, Query::kCtasPerSm) traverse_kern
 
 template <typename Query>
 static cudaError_t launch_traverse_kind(TraverseArgs A, int mode, cudaStream_t stream) {
-  A.num_chunks = (A.q + kTravThreads - 1) / kTravThreads;
-  A.num_sms = sm_count();
-  // persistent grid: up to SMs x Query::kCtasPerSm CTAs; fewer CTAs per SM when there is not enough work to fill them
-  int ctas_per_sm = (int)((A.num_chunks + A.num_sms - 1) / A.num_sms);
-  if (ctas_per_sm > Query::kCtasPerSm) ctas_per_sm = Query::kCtasPerSm;
-  if (ctas_per_sm < 1) ctas_per_sm = 1;
-  A.ctas_per_sm = ctas_per_sm;
-  const unsigned g = (unsigned)(A.num_sms * ctas_per_sm);
+  const int64_t chunks = (A.q + kTravThreads - 1) / kTravThreads;
+  if (chunks > 0x7fffffff) return cudaErrorInvalidValue;
+  const unsigned g = (unsigned)chunks;
   if (mode == kModeCount)
     traverse_kernel<Query, kModeCount><<<g, kTravThreads, 0, stream>>>(A);
   else if (mode == kModeFill)
