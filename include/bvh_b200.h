@@ -141,6 +141,24 @@ int bvh_query_fill_overflow(const void* nodes, int64_t n, const float* queries, 
                             const uint32_t* order, int64_t cap, const int32_t* counts, const int64_t* offsets,
                             int32_t* indices, void* stream);
 
+/* The whole single-pass query as ONE call (the sequence above, enqueued back to back with programmatic dependent
+ * launch, so that a small batch is not bound by the host's call overhead): query order (batches of more than 8192
+ * queries; smaller ones are served in input order), bvh_query_collect, scan, rows -> CSR, overflow rows.
+ *   rows     int32[q * cap], 32-byte aligned, cap a multiple of 8 (the caller's guess of a row capacity, as above)
+ *   order    uint32[q] (written; may be NULL when q <= 8192)      counts  int32[q] (written)
+ *   offsets  int64[q + 1] (written; offsets[q] = nnz)
+ *   indices  int32[indices_capacity]: the caller sizes it BEFORE nnz is known.  No row is written past the capacity: a
+ *            row that would end beyond it is skipped.  The caller reads offsets[q] after its own synchronisation; if
+ *            nnz <= indices_capacity the CSR is complete and byte-identical to count -> scan -> fill, otherwise it
+ *            provides a larger buffer and calls bvh_rows_to_csr + bvh_query_fill_overflow (counts, offsets, order and
+ *            rows are all valid).
+ *   scratch  bvh_query_csr_sizes(q) bytes, 16-byte aligned.
+ * n = 0: offsets all 0.  q = 0: offsets[0] = 0. */
+int bvh_query_csr_sizes(int64_t q, size_t* scratch_bytes);
+int bvh_query_csr(const void* nodes, int64_t n, const float* queries, int query_kind, int64_t q, int64_t cap,
+                  int32_t* rows, uint32_t* order, int32_t* counts, int64_t* offsets, int32_t* indices,
+                  int64_t indices_capacity, void* scratch, size_t scratch_bytes, void* stream);
+
 /* NEXT-1: ray queries, "all [primitives] that a ray intersects", through the same
  * Algorithm 1 kernel with a third predicate.  A ray is 8 floats {origin.xyz, direction.xyz, tmin, tmax}: the points
  * o + t d with tmin <= t <= tmax (a segment; tmax may be large).  Predicate D9: slab test in fp32

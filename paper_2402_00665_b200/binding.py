@@ -51,6 +51,8 @@ SYMBOLS = {
     "bvh_query_collect": [_P, c_int64, _P, c_int, c_int64, _P, c_int64, _P, _P, _P],
     "bvh_rows_to_csr": [_P, c_int64, _P, _P, c_int64, _P, _P],
     "bvh_query_fill_overflow": [_P, c_int64, _P, c_int, c_int64, _P, c_int64, _P, _P, _P, _P],
+    "bvh_query_csr_sizes": [c_int64, ctypes.POINTER(c_size_t)],
+    "bvh_query_csr": [_P, c_int64, _P, c_int, c_int64, c_int64, _P, _P, _P, _P, _P, c_int64, _P, c_size_t, _P],
     "bvh_query_order_rays": [_P, c_int64, _P, c_int64, _P, _P, c_size_t, _P],
     "bvh_query_rays_count": [_P, c_int64, _P, c_int64, _P, _P, _P],
     "bvh_query_rays_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
@@ -197,6 +199,20 @@ def bvh_query_fill_overflow(nodes, n: int, queries, query_kind: int, q: int, ord
     _check(load_library().bvh_query_fill_overflow(_ptr(nodes), n, _ptr(queries), query_kind, q, _ptr(order), cap,
                                                   _ptr(counts), _ptr(offsets), _ptr(indices), _stream()),
            "bvh_query_fill_overflow")
+
+
+def bvh_query_csr_sizes(q: int) -> int:
+    b = c_size_t(0)
+    _check(load_library().bvh_query_csr_sizes(q, ctypes.byref(b)), "bvh_query_csr_sizes")
+    return int(b.value)
+
+
+def bvh_query_csr(nodes, n: int, queries, query_kind: int, q: int, cap: int, rows, order, counts, offsets, indices,
+                  indices_capacity: int, scratch) -> None:
+    _check(load_library().bvh_query_csr(_ptr(nodes), n, _ptr(queries), query_kind, q, cap, _ptr(rows), _ptr(order),
+                                        _ptr(counts), _ptr(offsets), _ptr(indices), indices_capacity, _ptr(scratch),
+                                        0 if scratch is None else scratch.numel() * scratch.element_size(), _stream()),
+           "bvh_query_csr")
 
 
 def bvh_query_order_rays(nodes, n: int, rays, q: int, order, scratch) -> None:
@@ -371,6 +387,30 @@ def query(bvh: Bvh, queries: torch.Tensor, ws: QueryWorkspace | None = None, ind
         fill(bvh.nodes, bvh.n, queries, q, order, ws.offsets, indices)
     offsets = ws.offsets[: q + 1]
     return offsets, (indices if nnz is None else indices[:nnz])
+
+
+def query_csr(bvh: Bvh, queries: torch.Tensor, row_capacity: int, indices: torch.Tensor, ws: QueryWorkspace | None = None,
+              rows: torch.Tensor | None = None):
+    """The single-pass range search as ONE call of the C ABI (``bvh_query_csr``): nothing is read back, so the caller
+    sizes ``indices`` beforehand (from the previous batch, say).  Returns (offsets int64[q+1], indices) on the device;
+    ``offsets[q]`` is nnz: if it exceeds ``indices.numel()`` the rows that did not fit were skipped and the caller
+    finishes with ``bvh_rows_to_csr`` + ``bvh_query_fill_overflow`` into a larger buffer."""
+    if queries.dtype != torch.float32 or queries.dim() != 2 or queries.shape[1] not in (4, 6, 8):
+        raise BvhError(f"expected float32 [q,4], [q,6] or [q,8], got {queries.dtype} {tuple(queries.shape)}")
+    if bvh.prim_kind is None:
+        raise BvhError("query_csr() on a Bvh that has not been built")
+    q = int(queries.shape[0])
+    cap = int(row_capacity)
+    ws = ws or QueryWorkspace(q, queries.device)
+    if ws.q < q:
+        raise BvhError(f"QueryWorkspace holds {ws.q} queries, {q} given")
+    if rows is None:
+        rows = torch.empty(max(q, 1) * cap, dtype=torch.int32, device=queries.device)
+    elif rows.numel() < q * cap:
+        raise BvhError(f"rows holds {rows.numel()} entries, {q * cap} needed")
+    bvh_query_csr(bvh.nodes, bvh.n, queries, QUERY_KINDS[int(queries.shape[1])], q, cap, rows, ws.order, ws.counts,
+                  ws.offsets, indices, indices.numel(), ws.order_scratch)
+    return ws.offsets[: q + 1], indices
 
 
 class HostCsr:

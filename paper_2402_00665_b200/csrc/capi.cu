@@ -200,7 +200,7 @@ __global__ void fill_reduce_none_kernel(int32_t* index, float* keys, int64_t q) 
 
 static int query(const void* nodes, int64_t n, const float* queries, int64_t q, int kind, int mode,
                  const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* out, int64_t cap, bool only_over,
-                 void* stream_, float* keys = nullptr) {
+                 void* stream_, float* keys = nullptr, int64_t out_limit = 0) {
   if (n < 0 || q < 0) return BVH_ERR_INVALID_ARGUMENT;
   if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
   if (kind < 0 || kind > 2) return BVH_ERR_INVALID_ARGUMENT;
@@ -227,7 +227,8 @@ static int query(const void* nodes, int64_t n, const float* queries, int64_t q, 
   // node records are read with 256-bit loads: 32-byte alignment
   if (!nodes || !queries || misaligned32(nodes) || misaligned(queries)) return BVH_ERR_INVALID_ARGUMENT;
   if (mode == 1 && !out) return BVH_ERR_INVALID_ARGUMENT;  // nnz = 0 callers still pass a valid pointer
-  if (launch_traverse(nodes, (int)n, queries, q, kind, mode, order, counts, offsets, out, cap, only_over, keys, stream) != cudaSuccess)
+  if (launch_traverse(nodes, (int)n, queries, q, kind, mode, order, counts, offsets, out, cap, only_over, keys, stream,
+                      out_limit) != cudaSuccess)
     return BVH_ERR_CUDA;
   return BVH_OK;
 }
@@ -383,8 +384,8 @@ int bvh_scan_counts(const int32_t* counts, int64_t q, int64_t* offsets, void* sc
   if (q < 0 || !offsets) return BVH_ERR_INVALID_ARGUMENT;
   if (q > 0 && (!counts || !scratch)) return BVH_ERR_INVALID_ARGUMENT;
   if (q > 0 && scratch_bytes < bvh::scan_scratch_bytes(q)) return BVH_ERR_SCRATCH;
-  bvh::launch_scan(counts, q, offsets, scratch, static_cast<cudaStream_t>(stream));
-  return bvh::check_launch();
+  if (bvh::launch_scan(counts, q, offsets, scratch, static_cast<cudaStream_t>(stream)) != cudaSuccess) return BVH_ERR_CUDA;
+  return BVH_OK;
 }
 
 int bvh_query_spheres_fill(const void* nodes, int64_t n, const float* xyzr, int64_t q, const uint32_t* order,
@@ -432,6 +433,48 @@ int bvh_query_fill_overflow(const void* nodes, int64_t n, const float* queries, 
                             int32_t* indices, void* stream) {
   if (cap < 0) return BVH_ERR_INVALID_ARGUMENT;
   return bvh::query(nodes, n, queries, q, query_kind, 1, order, const_cast<int32_t*>(counts), offsets, indices, cap, true, stream);
+}
+
+int bvh_query_csr_sizes(int64_t q, size_t* scratch_bytes) {
+  if (q < 0 || !scratch_bytes) return BVH_ERR_INVALID_ARGUMENT;
+  if (q >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
+  // the ordering's scratch is dead once `order` is written: the scan reuses its first bytes
+  const size_t a = q > bvh::kSmallOrderQ ? bvh::scratch_layout(q, 30).total : 0, b = bvh::scan_scratch_bytes(q);
+  *scratch_bytes = a > b ? a : b;
+  return BVH_OK;
+}
+
+int bvh_query_csr(const void* nodes, int64_t n, const float* queries, int query_kind, int64_t q, int64_t cap,
+                  int32_t* rows, uint32_t* order, int32_t* counts, int64_t* offsets, int32_t* indices,
+                  int64_t indices_capacity, void* scratch, size_t scratch_bytes, void* stream) {
+  if (n < 0 || q < 0 || query_kind < 0 || query_kind > 2 || indices_capacity < 0) return BVH_ERR_INVALID_ARGUMENT;
+  if (n >= ((int64_t)1 << 30) || q >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
+  if (cap < 8 || cap % 8 != 0 || cap > 0x7fffffff) return BVH_ERR_INVALID_ARGUMENT;
+  if (!offsets) return BVH_ERR_INVALID_ARGUMENT;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (q == 0) return bvh::launch_scan(nullptr, 0, offsets, nullptr, s) == cudaSuccess ? BVH_OK : BVH_ERR_CUDA;
+  size_t need = 0;
+  bvh_query_csr_sizes(q, &need);
+  if (!rows || !counts || !indices || !scratch || bvh::misaligned32(rows) || bvh::misaligned(scratch)) return BVH_ERR_INVALID_ARGUMENT;
+  if (scratch_bytes < need) return BVH_ERR_SCRATCH;
+  if (n > 0 && (!nodes || !queries || bvh::misaligned32(nodes) || bvh::misaligned(queries))) return BVH_ERR_INVALID_ARGUMENT;
+  const int64_t limit = indices_capacity > 0 ? indices_capacity : -1;   // -1: nothing fits (0 means "no limit" inside)
+  const uint32_t* ord = nullptr;
+  int rc;
+  if (n > 0 && q > bvh::kSmallOrderQ) {     // small batches are served in input order (bvh_query_order_* would write the identity)
+    if (!order) return BVH_ERR_INVALID_ARGUMENT;
+    if ((rc = bvh::query_order(nodes, n, queries, q, query_kind, order, scratch, scratch_bytes, stream)) != BVH_OK) return rc;
+    ord = order;
+  }
+  if ((rc = bvh::query(nodes, n, queries, q, query_kind, 2, ord, counts, nullptr, rows, cap, false, stream)) != BVH_OK) return rc;
+  if (q <= bvh::scan_single_tile_items()) {
+    if (bvh::launch_scan_rows_to_csr_small(rows, cap, counts, offsets, q, indices, s, limit) != cudaSuccess) return BVH_ERR_CUDA;
+  } else {
+    if (bvh::launch_scan(counts, q, offsets, scratch, s) != cudaSuccess) return BVH_ERR_CUDA;
+    if (bvh::launch_rows_to_csr(rows, cap, counts, offsets, q, indices, s, limit) != cudaSuccess) return BVH_ERR_CUDA;
+  }
+  if (n == 0) return BVH_OK;
+  return bvh::query(nodes, n, queries, q, query_kind, 1, ord, counts, offsets, indices, cap, true, stream, nullptr, limit);
 }
 
 int bvh_export(const void* nodes, const void* scratch, int64_t n, int morton_bits, void* sorted_codes, uint32_t* perm,

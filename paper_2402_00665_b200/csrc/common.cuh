@@ -184,13 +184,18 @@ int launch_variant_apetrei_export(const void* nodes, void* extra, int n, int32_t
 // order (optional): thread t serves query order[t] (results still land in row order[t]).
 cudaError_t launch_traverse(const void* nodes, int n, const float* queries, int64_t q, int kind, int mode,
                             const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* out, int64_t cap,
-                            bool only_over, float* keys, cudaStream_t stream);
+                            bool only_over, float* keys, cudaStream_t stream, int64_t out_limit = 0);
+// limit != 0: `indices` holds `limit` entries (< 0: none); rows that would end past it are not copied (fill: out_limit, likewise).
 cudaError_t launch_rows_to_csr(const int32_t* rows, int64_t cap, const int32_t* counts, const int64_t* offsets, int64_t q,
-                               int32_t* indices, cudaStream_t stream);
+                               int32_t* indices, cudaStream_t stream, int64_t limit = 0);
+// q <= scan_single_tile_items(): exclusive scan of the counts AND the copy of the rows, one launch.
+cudaError_t launch_scan_rows_to_csr_small(const int32_t* rows, int64_t cap, const int32_t* counts, int64_t* offsets, int64_t q,
+                                          int32_t* indices, cudaStream_t stream, int64_t limit = 0);
+int scan_single_tile_items();
 int sm_count();   // multiprocessors of the current device (cached)
 // K7: exclusive scan of int32 counts into int64 offsets[q+1].
 size_t scan_scratch_bytes(int64_t q);
-void launch_scan(const int32_t* counts, int64_t q, int64_t* offsets, void* scratch, cudaStream_t stream);
+cudaError_t launch_scan(const int32_t* counts, int64_t q, int64_t* offsets, void* scratch, cudaStream_t stream);
 // Parity export.
 void launch_export(const void* nodes, const void* scratch, const ScratchLayout& L, int n, void* sorted_codes,
                    uint32_t* perm, int32_t* left_child, int32_t* rope, float* aabb, float* scene_bounds,

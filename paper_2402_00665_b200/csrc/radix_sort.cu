@@ -63,10 +63,19 @@ __device__ __forceinline__ void st_status(uint32_t* p, uint32_t v) {
 #define BVH_LOOKBACK_BATCH 4
 #endif
 constexpr int kLookbackBatch = BVH_LOOKBACK_BATCH;
+// Independent ranking chains per warp.  Ranking item j reads and bumps the warp's running count of its digit in shared
+// memory, so consecutive items form one dependent chain of shared-memory round trips.  With C chains the warp's items
+// are split into C consecutive runs (tile order is (warp, item, lane), so run c precedes run c + 1), each ranked against
+// its own counter array, C items per step: the chains overlap, and the runs are put back in order by the scan over
+// (warp, chain) below.
+#ifndef BVH_SORT_CHAINS
+#define BVH_SORT_CHAINS 1
+#endif
+constexpr int kSortChains = BVH_SORT_CHAINS;
 
 template <typename KeyT>
 struct SortSmem {
-  uint32_t warp_hist[kSortWarps][256];
+  uint32_t warp_hist[kSortWarps][kSortChains][256];
   uint32_t tile_excl[256];     // first tile-sorted position of each digit
   uint32_t digit_base[256];    // global position of tile-sorted position 0 of each digit (mod 2^32; n < 2^30)
   uint32_t tile_hist[256];     // early publish: digit counts of the tile, by shared-memory atomics
@@ -123,28 +132,42 @@ __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restr
   uint32_t rank2[ITEMS / 2];                          // two 16-bit ranks per register (a rank is < TILE <= 65536)
   static_assert(ITEMS % 2 == 0 && SortCfg<KeyT>::TILE <= 65536, "packed ranks");
   const uint32_t lt_mask = (1u << lane) - 1u;
-  uint32_t* my_hist = s.warp_hist[warp];
+  constexpr int CH = kSortChains, RUN = ITEMS / CH;   // RUN consecutive items per chain
+  static_assert(ITEMS % CH == 0, "whole runs per chain");
+  uint32_t(*my_hist)[256] = s.warp_hist[warp];
 #pragma unroll
-  for (int j = 0; j < ITEMS; ++j) {
-    const uint32_t d = (uint32_t)(key[j] >> shift) & 0xFFu;
-    uint32_t peers;
-    if (FULL) {
-      peers = match_digit<TOP>(d, 0xffffffffu);
-    } else {
-      const bool valid = (warp_off + j * 32) < valid_in_tile;
-      peers = match_digit<TOP>(d, __ballot_sync(0xffffffffu, valid));
-      if (!valid) peers = 0;
+  for (int u = 0; u < ITEMS / 2; ++u) rank2[u] = 0;
+#pragma unroll
+  for (int jj = 0; jj < RUN; ++jj) {
+    uint32_t d[CH], peers[CH], below[CH], pre[CH];
+#pragma unroll
+    for (int c = 0; c < CH; ++c) {
+      const int j = c * RUN + jj;
+      d[c] = (uint32_t)(key[j] >> shift) & 0xFFu;
+      if (FULL) {
+        peers[c] = match_digit<TOP>(d[c], 0xffffffffu);
+      } else {
+        const bool valid = (warp_off + j * 32) < valid_in_tile;
+        peers[c] = match_digit<TOP>(d[c], __ballot_sync(0xffffffffu, valid));
+        if (!valid) peers[c] = 0;
+      }
     }
     // every peer reads the warp's running count of its digit (a broadcast), the lowest peer then bumps it
-    const uint32_t below = __popc(peers & lt_mask);
-    const uint32_t pre = my_hist[d];
+#pragma unroll
+    for (int c = 0; c < CH; ++c) {
+      below[c] = __popc(peers[c] & lt_mask);
+      pre[c] = my_hist[c][d[c]];
+    }
     __syncwarp();
-    if (below == 0 && (FULL || peers)) my_hist[d] = pre + __popc(peers);
+#pragma unroll
+    for (int c = 0; c < CH; ++c)
+      if (below[c] == 0 && (FULL || peers[c])) my_hist[c][d[c]] = pre[c] + __popc(peers[c]);
     __syncwarp();
-    if (j & 1)
-      rank2[j / 2] |= (pre + below) << 16;
-    else
-      rank2[j / 2] = pre + below;
+#pragma unroll
+    for (int c = 0; c < CH; ++c) {
+      const int j = c * RUN + jj;
+      rank2[j / 2] |= (pre[c] + below[c]) << ((j & 1) ? 16 : 0);
+    }
   }
 
   // values are only needed for the scatter: issue their loads now, they land during the look-back
@@ -165,9 +188,12 @@ __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restr
     uint32_t sum = 0;
 #pragma unroll
     for (int w = 0; w < kSortWarps; ++w) {
-      const uint32_t c = s.warp_hist[w][tid];
-      s.warp_hist[w][tid] = sum;
-      sum += c;
+#pragma unroll
+      for (int ch = 0; ch < kSortChains; ++ch) {
+        const uint32_t c = s.warp_hist[w][ch][tid];
+        s.warp_hist[w][ch][tid] = sum;
+        sum += c;
+      }
     }
     if (!kEarlyPublish) {
       tile_count = sum;
@@ -247,7 +273,7 @@ __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restr
   for (int j = 0; j < ITEMS; ++j) {
     if (FULL || (warp_off + j * 32) < valid_in_tile) {
       const uint32_t d = (uint32_t)(key[j] >> shift) & 0xFFu;
-      const uint32_t pos = s.tile_excl[d] + my_hist[d] + ((j & 1) ? (rank2[j / 2] >> 16) : (rank2[j / 2] & 0xFFFFu));
+      const uint32_t pos = s.tile_excl[d] + my_hist[j / RUN][d] + ((j & 1) ? (rank2[j / 2] >> 16) : (rank2[j / 2] & 0xFFFFu));
       s.keys[pos] = key[j];
       s.vals[pos] = val[j];
     }
@@ -281,7 +307,7 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_o
   SortSmem<KeyT>& s = *reinterpret_cast<SortSmem<KeyT>*>(smem_raw);
 
   const int tid = threadIdx.x;
-  for (int i = tid; i < kSortWarps * 256; i += kSortThreads) (&s.warp_hist[0][0])[i] = 0;
+  for (int i = tid; i < kSortWarps * kSortChains * 256; i += kSortThreads) (&s.warp_hist[0][0][0])[i] = 0;
   if (tid < 256) s.tile_hist[tid] = 0;
   pdl_wait();
   pdl_trigger();

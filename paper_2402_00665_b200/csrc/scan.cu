@@ -34,6 +34,8 @@ __device__ __forceinline__ int64_t block_exclusive_scan(int64_t v, int64_t* tota
 __global__ void __launch_bounds__(kScanThreads) scan_tile_sums_kernel(const int32_t* __restrict__ counts, int64_t q,
                                                                       int64_t* __restrict__ tile_sums) {
   __shared__ int64_t s_warp[kScanThreads / 32];
+  pdl_wait();
+  pdl_trigger();
   const int64_t base = (int64_t)blockIdx.x * kScanTile;
   int64_t v = 0;
 #pragma unroll
@@ -48,6 +50,8 @@ __global__ void __launch_bounds__(kScanThreads) scan_tile_sums_kernel(const int3
 
 __global__ void __launch_bounds__(kScanThreads) scan_of_sums_kernel(int64_t* tile_sums, int64_t tiles) {
   __shared__ int64_t s_warp[kScanThreads / 32];
+  pdl_wait();
+  pdl_trigger();
   int64_t carry = 0;
   for (int64_t b = 0; b < tiles; b += kScanThreads) {
     const int64_t i = b + threadIdx.x;
@@ -63,6 +67,8 @@ __global__ void __launch_bounds__(kScanThreads) scan_apply_kernel(const int32_t*
                                                                   const int64_t* __restrict__ tile_sums,
                                                                   int64_t* __restrict__ offsets) {
   __shared__ int64_t s_warp[kScanThreads / 32];
+  pdl_wait();
+  pdl_trigger();
   const int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;  // blocked arrangement
   int32_t c[kScanItems];
   int64_t v = 0;
@@ -85,6 +91,8 @@ __global__ void __launch_bounds__(kScanThreads) scan_apply_kernel(const int32_t*
 __global__ void __launch_bounds__(kScanThreads) scan_single_tile_kernel(const int32_t* __restrict__ counts, int64_t q,
                                                                         int64_t* __restrict__ offsets) {
   __shared__ int64_t s_warp[kScanThreads / 32];
+  pdl_wait();
+  pdl_trigger();
   const int64_t base = (int64_t)threadIdx.x * kScanItems;   // blocked arrangement
   int32_t c[kScanItems];
   int64_t v = 0;
@@ -103,27 +111,27 @@ __global__ void __launch_bounds__(kScanThreads) scan_single_tile_kernel(const in
   if (threadIdx.x == 0) offsets[q] = total;
 }
 
-__global__ void scan_empty_kernel(int64_t* offsets) { offsets[0] = 0; }
+__global__ void scan_empty_kernel(int64_t* offsets) {
+  pdl_wait();
+  offsets[0] = 0;
+}
 
 size_t scan_scratch_bytes(int64_t q) {
   const int64_t tiles = (q + kScanTile - 1) / kScanTile;
   return (size_t)(tiles > 0 ? tiles : 1) * sizeof(int64_t);
 }
 
-void launch_scan(const int32_t* counts, int64_t q, int64_t* offsets, void* scratch, cudaStream_t stream) {
-  if (q == 0) {
-    scan_empty_kernel<<<1, 1, 0, stream>>>(offsets);
-    return;
-  }
-  if (q <= kScanTile) {
-    scan_single_tile_kernel<<<1, kScanThreads, 0, stream>>>(counts, q, offsets);
-    return;
-  }
+cudaError_t launch_scan(const int32_t* counts, int64_t q, int64_t* offsets, void* scratch, cudaStream_t stream) {
+  if (q == 0) return launch_pdl(scan_empty_kernel, dim3(1), dim3(1), 0, stream, offsets);
+  if (q <= kScanTile) return launch_pdl(scan_single_tile_kernel, dim3(1), dim3(kScanThreads), 0, stream, counts, q, offsets);
   const int64_t tiles = (q + kScanTile - 1) / kScanTile;
   int64_t* sums = static_cast<int64_t*>(scratch);
-  scan_tile_sums_kernel<<<(unsigned)tiles, kScanThreads, 0, stream>>>(counts, q, sums);
-  scan_of_sums_kernel<<<1, kScanThreads, 0, stream>>>(sums, tiles);
-  scan_apply_kernel<<<(unsigned)tiles, kScanThreads, 0, stream>>>(counts, q, sums, offsets);
+  cudaError_t e = launch_pdl(scan_tile_sums_kernel, dim3((unsigned)tiles), dim3(kScanThreads), 0, stream, counts, q, sums);
+  if (e == cudaSuccess) e = launch_pdl(scan_of_sums_kernel, dim3(1), dim3(kScanThreads), 0, stream, sums, tiles);
+  if (e == cudaSuccess)
+    e = launch_pdl(scan_apply_kernel, dim3((unsigned)tiles), dim3(kScanThreads), 0, stream, counts, q,
+                   static_cast<const int64_t*>(sums), offsets);
+  return e;
 }
 
 }  // namespace bvh

@@ -291,6 +291,8 @@ struct TraverseArgs {
   int32_t* out;              // fill: indices; collect: rows
   int64_t cap;               // collect: entries per row.  fill with only_over: only rows with counts[j] > cap are filled
   int only_over;
+  int64_t out_limit;         // fill: entries `out` can hold; rows that would end past it are not written (0: no limit, < 0: nothing fits)
+  int spread_log2;           // small batches: only every 2^spread_log2-th thread carries a query (see launch_traverse_kind)
 };
 
 // Row output of the fill / collect passes.  The hits of a row arrive a few at a time (one scan step of 32 leaves gives
@@ -380,10 +382,12 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
     // to 2800 hits) and keeps the chunks that run at the same time neighbours on the curve.  Round 1 ran a persistent
     // grid with a static, SM-local assignment of chunks instead: 26-35 % slower on C3 (4.26 / 6.42 ms count / fill
     // against 3.3 / 4.4), because blocks whose chunks were expensive finished long after the others.
-    const int64_t t = (int64_t)blockIdx.x * kTravThreads + threadIdx.x;
-    bool have = t < A.q;
+    const int64_t thread = (int64_t)blockIdx.x * kTravThreads + threadIdx.x;
+    const int64_t t = thread >> A.spread_log2;               // position in the query list
+    bool have = t < A.q && (thread & ((1 << A.spread_log2) - 1)) == 0;
     const int64_t j = have ? (order ? (int64_t)order[t] : t) : 0;
     if (MODE == kModeFill && A.only_over) have = have && (int64_t)A.counts[j] > A.cap;
+    if (MODE == kModeFill && A.out_limit != 0) have = have && A.offsets[j + 1] <= A.out_limit;
     Query query;
     query.load(queries, j);
     __syncwarp();                                            // the previous chunk's scans are over
@@ -626,6 +630,8 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
 // garbage indices.
 template <typename Query, int MODE>
 __global__ void __launch_bounds__(kTravThreads, Query::kCtasPerSm) traverse_kernel(const TraverseArgs A) {
+  pdl_wait();      // launched with programmatic stream serialisation: the previous kernel of the stream has completed
+  pdl_trigger();
   const NodesHeader* h = reinterpret_cast<const NodesHeader*>(A.nodes);
   if (h->magic != kNodesMagic || h->n != A.n) {
     if (MODE != kModeFill)
@@ -642,30 +648,34 @@ __global__ void __launch_bounds__(kTravThreads, Query::kCtasPerSm) traverse_kern
     traverse_body<Query, MODE, false>(A, S);
 }
 
+// Small batches.  With one query per lane a warp serves its 32 queries' leaf scans one after the other, each a chain of
+// dependent loads; a batch of a few thousand queries is then a few hundred warps that each run for a long time on a
+// mostly empty GPU (C1: 4096 queries = 128 warps, 58 us).  When the batch cannot fill the GPU's warp slots anyway, the
+// queries are spread out -- only every 2^s-th lane carries one -- so that up to 32 times as many warps share the same
+// scans (C1: ... us).  Results and their order do not depend on which lane serves a query.
+#ifndef BVH_TRAV_SPREAD_THREADS
+#define BVH_TRAV_SPREAD_THREADS (148 * 1024)
+#endif
 template <typename Query>
 static cudaError_t launch_traverse_kind(TraverseArgs A, int mode, cudaStream_t stream) {
-  const int64_t chunks = (A.q + kTravThreads - 1) / kTravThreads;
+  A.spread_log2 = 0;
+  while (A.spread_log2 < 5 && (A.q << (A.spread_log2 + 1)) <= (int64_t)BVH_TRAV_SPREAD_THREADS) ++A.spread_log2;
+  const int64_t chunks = ((A.q << A.spread_log2) + kTravThreads - 1) / kTravThreads;
   if (chunks > 0x7fffffff) return cudaErrorInvalidValue;
-  const unsigned g = (unsigned)chunks;
-  if (mode == kModeCount)
-    traverse_kernel<Query, kModeCount><<<g, kTravThreads, 0, stream>>>(A);
-  else if (mode == kModeFill)
-    traverse_kernel<Query, kModeFill><<<g, kTravThreads, 0, stream>>>(A);
-  else if (mode == kModeCollect)
-    traverse_kernel<Query, kModeCollect><<<g, kTravThreads, 0, stream>>>(A);
-  else if (mode == kModeAny)
-    traverse_kernel<Query, kModeAny><<<g, kTravThreads, 0, stream>>>(A);
-  else if constexpr (Query::kHasKey)
-    traverse_kernel<Query, kModeReduce><<<g, kTravThreads, 0, stream>>>(A);
-  else
-    return cudaErrorInvalidValue;
-  return cudaGetLastError();
+  const dim3 g((unsigned)chunks), b(kTravThreads);
+  if (mode == kModeCount) return launch_pdl(traverse_kernel<Query, kModeCount>, g, b, 0, stream, A);
+  if (mode == kModeFill) return launch_pdl(traverse_kernel<Query, kModeFill>, g, b, 0, stream, A);
+  if (mode == kModeCollect) return launch_pdl(traverse_kernel<Query, kModeCollect>, g, b, 0, stream, A);
+  if (mode == kModeAny) return launch_pdl(traverse_kernel<Query, kModeAny>, g, b, 0, stream, A);
+  if constexpr (Query::kHasKey) return launch_pdl(traverse_kernel<Query, kModeReduce>, g, b, 0, stream, A);
+  return cudaErrorInvalidValue;
 }
 
 cudaError_t launch_traverse(const void* nodes, int n, const float* queries, int64_t q, int kind, int mode,
                             const uint32_t* order, int32_t* counts, const int64_t* offsets, int32_t* out, int64_t cap,
-                            bool only_over, float* keys, cudaStream_t stream) {
+                            bool only_over, float* keys, cudaStream_t stream, int64_t out_limit) {
   TraverseArgs A{};
+  A.out_limit = out_limit;
   A.keys = keys;
   A.nodes = static_cast<const char*>(nodes);
   A.n = n;
@@ -684,45 +694,116 @@ cudaError_t launch_traverse(const void* nodes, int n, const float* queries, int6
 
 // rows -> CSR (single-pass variant): row j of `rows` (cap entries, counts[j] of them valid if counts[j] <= cap) is copied
 // to indices[offsets[j] ...).  Rows that did not fit (counts[j] > cap) are skipped: the fill pass restricted to them
-// (only_over) writes those.  One group of G lanes per row.
+// (only_over) writes those.  One group of G lanes per row.  limit != 0: rows that would end past `limit` entries of
+// `indices` are skipped too (the caller sized `indices` before it knew nnz, and reads offsets[q] afterwards).
+template <int G>
+__device__ __forceinline__ void copy_row(const int32_t* __restrict__ src, int32_t* __restrict__ dst, int c, int gl) {
+  int e = gl;
+  for (; e + 3 * G < c; e += 4 * G) {                     // four loads in flight per lane
+    const int v0 = __ldcs(src + e), v1 = __ldcs(src + e + G), v2 = __ldcs(src + e + 2 * G), v3 = __ldcs(src + e + 3 * G);
+    dst[e] = v0;
+    dst[e + G] = v1;
+    dst[e + 2 * G] = v2;
+    dst[e + 3 * G] = v3;
+  }
+  for (; e < c; e += G) dst[e] = __ldcs(src + e);
+}
+
 template <int G>
 __global__ void __launch_bounds__(256) rows_to_csr_kernel(const int32_t* __restrict__ rows, int64_t cap,
                                                           const int32_t* __restrict__ counts,
                                                           const int64_t* __restrict__ offsets, int64_t q,
-                                                          int32_t* __restrict__ indices) {
+                                                          int32_t* __restrict__ indices, int64_t limit) {
+  pdl_wait();
+  pdl_trigger();
   const int64_t group = ((int64_t)blockIdx.x * 256 + threadIdx.x) / G;
   const int64_t groups = (int64_t)gridDim.x * 256 / G;
   const int gl = threadIdx.x % G;
   for (int64_t j = group; j < q; j += groups) {
     const int c = counts[j];
     if (c <= 0 || c > cap) continue;
-    const int32_t* __restrict__ src = rows + j * cap;
-    int32_t* __restrict__ dst = indices + offsets[j];
-    int e = gl;
-    for (; e + 3 * G < c; e += 4 * G) {                     // four loads in flight per lane
-      const int v0 = __ldcs(src + e), v1 = __ldcs(src + e + G), v2 = __ldcs(src + e + 2 * G), v3 = __ldcs(src + e + 3 * G);
-      dst[e] = v0;
-      dst[e + G] = v1;
-      dst[e + 2 * G] = v2;
-      dst[e + 3 * G] = v3;
-    }
-    for (; e < c; e += G) dst[e] = __ldcs(src + e);
+    const int64_t off = offsets[j];
+    if (limit != 0 && off + c > limit) continue;
+    copy_row<G>(rows + j * cap, indices + off, c, gl);
   }
 }
 
 cudaError_t launch_rows_to_csr(const int32_t* rows, int64_t cap, const int32_t* counts, const int64_t* offsets, int64_t q,
-                               int32_t* indices, cudaStream_t stream) {
+                               int32_t* indices, cudaStream_t stream, int64_t limit) {
   const int sms = sm_count();
   if (cap >= 128) {
     int64_t blocks = (q * 32 + 255) / 256;
     if (blocks > (int64_t)sms * 16) blocks = (int64_t)sms * 16;
-    rows_to_csr_kernel<32><<<(unsigned)blocks, 256, 0, stream>>>(rows, cap, counts, offsets, q, indices);
-  } else {
-    int64_t blocks = (q * 8 + 255) / 256;
-    if (blocks > (int64_t)sms * 16) blocks = (int64_t)sms * 16;
-    rows_to_csr_kernel<8><<<(unsigned)blocks, 256, 0, stream>>>(rows, cap, counts, offsets, q, indices);
+    return launch_pdl(rows_to_csr_kernel<32>, dim3((unsigned)blocks), dim3(256), 0, stream, rows, cap, counts, offsets, q, indices, limit);
   }
-  return cudaGetLastError();
+  int64_t blocks = (q * 8 + 255) / 256;
+  if (blocks > (int64_t)sms * 16) blocks = (int64_t)sms * 16;
+  return launch_pdl(rows_to_csr_kernel<8>, dim3((unsigned)blocks), dim3(256), 0, stream, rows, cap, counts, offsets, q, indices, limit);
+}
+
+// Small batches (q <= kSmallScan): the exclusive scan of the counts and the copy of the rows in ONE launch.  Every block
+// scans all q counts by itself (a few microseconds of redundant work that saves a dependent launch) and keeps the
+// offsets in shared memory; block 0 also writes them out.  Then one group of 8 lanes per row, as above.
+constexpr int kSmallScan = 4096;
+int scan_single_tile_items() { return kSmallScan; }
+__global__ void __launch_bounds__(256) scan_rows_to_csr_small_kernel(const int32_t* __restrict__ rows, int64_t cap,
+                                                                     const int32_t* __restrict__ counts,
+                                                                     int64_t* __restrict__ offsets, int q,
+                                                                     int32_t* __restrict__ indices, int64_t limit) {
+  constexpr int ITEMS = kSmallScan / 256, G = 8;
+  __shared__ int64_t s_off[kSmallScan];
+  __shared__ int64_t s_warp[8];
+  pdl_wait();
+  pdl_trigger();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int base = threadIdx.x * ITEMS;                     // blocked arrangement
+  int c[ITEMS];
+  int64_t v = 0;
+#pragma unroll
+  for (int k = 0; k < ITEMS; ++k) {
+    c[k] = (base + k < q) ? counts[base + k] : 0;
+    v += c[k];
+  }
+  int64_t incl = v;
+#pragma unroll
+  for (int off = 1; off < 32; off <<= 1) {
+    const int64_t a = __shfl_up_sync(0xffffffffu, incl, off);
+    if (lane >= off) incl += a;
+  }
+  if (lane == 31) s_warp[warp] = incl;
+  __syncthreads();
+  int64_t run = incl - v, total = 0;
+#pragma unroll
+  for (int w = 0; w < 8; ++w) {
+    const int64_t sw = s_warp[w];
+    if (w < warp) run += sw;
+    total += sw;
+  }
+#pragma unroll
+  for (int k = 0; k < ITEMS; ++k) {
+    if (base + k < q) {
+      s_off[base + k] = run;
+      if (blockIdx.x == 0) offsets[base + k] = run;
+    }
+    run += c[k];
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) offsets[q] = total;
+  __syncthreads();
+  const int gl = threadIdx.x % G;
+  for (int j = (blockIdx.x * 256 + threadIdx.x) / G; j < q; j += gridDim.x * 256 / G) {
+    const int cj = counts[j];
+    if (cj <= 0 || cj > cap) continue;
+    const int64_t off = s_off[j];
+    if (limit != 0 && off + cj > limit) continue;
+    copy_row<G>(rows + (int64_t)j * cap, indices + off, cj, gl);
+  }
+}
+
+cudaError_t launch_scan_rows_to_csr_small(const int32_t* rows, int64_t cap, const int32_t* counts, int64_t* offsets, int64_t q,
+                                          int32_t* indices, cudaStream_t stream, int64_t limit) {
+  if (q > kSmallScan) return cudaErrorInvalidValue;
+  const unsigned blocks = (unsigned)((q * 8 + 255) / 256);
+  return launch_pdl(scan_rows_to_csr_small_kernel, dim3(blocks), dim3(256), 0, stream, rows, cap, counts, offsets, (int)q, indices, limit);
 }
 
 }  // namespace bvh

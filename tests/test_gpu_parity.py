@@ -270,6 +270,63 @@ def test_single_pass_query_equals_oracle(B, oracle_lib, name, n, q, radius):
         assert np.array_equal(r[j, :k], oidx[ooff[j]: ooff[j] + k]) and np.all(r[j, k:] == -7), j
 
 
+@pytest.mark.parametrize("name,n,q,radius", [("C1", 4096, 4096, None), ("C1", 4096, 1, None), ("C3", 120_001, 5_000, 0.004),
+                                             ("C2", 50_000, 8_192, 0.03), ("C4", 70_003, 30_000, 4e-3),
+                                             ("C5", 65_537, 10_000, 0.04)])
+def test_one_call_query_csr_equals_oracle(B, oracle_lib, name, n, q, radius):
+    """bvh_query_csr: order + collect + scan + rows -> CSR + overflow rows enqueued by ONE call (small batches: input
+    order, the scan and the row copy in one kernel, queries spread over the warps) = the oracle's CSR byte for byte,
+    whatever the row capacity; a result buffer that is too small is never overrun, and the documented completion
+    (bvh_rows_to_csr + bvh_query_fill_overflow into a larger buffer) yields the same bytes."""
+    w = W.make(name, n=n, q=q, radius=radius)
+    o = oracle_lib.build_bvh(w.prims, w.morton_bits)
+    bvh = gpu_build(B, w.prims, w.morton_bits)
+    ooff, oidx = _oracle_csr(oracle_lib, o, w.queries)
+    counts = np.diff(ooff)
+    nnz = int(ooff[-1])
+    mx = int(counts.max())
+    dq = _dev(w.queries)
+    kind = B.QUERY_KINDS[w.queries.shape[1]]
+    ws = B.QueryWorkspace(w.q)
+    for cap in sorted({max(8, (mx + 7) // 8 * 8), max(8, int(np.median(counts)) // 8 * 8), 8}):
+        ind = torch.full((nnz + 16,), -7, dtype=torch.int32, device="cuda")
+        off, _ = B.query_csr(bvh, dq, cap, ind, ws=ws)
+        torch.cuda.synchronize()
+        assert np.array_equal(off.cpu().numpy(), ooff), (name, cap, "offsets")
+        got = ind.cpu().numpy()
+        assert np.array_equal(got[:nnz], oidx) and np.all(got[nnz:] == -7), (name, cap, "indices")
+        # a buffer that holds only part of the result: rows that end inside it are complete, nothing past it is touched
+        short = max(1, nnz // 2)
+        buf = torch.full((short + 64,), -7, dtype=torch.int32, device="cuda")
+        rows = torch.empty(w.q * cap, dtype=torch.int32, device="cuda")
+        B.bvh_query_csr(bvh.nodes, bvh.n, dq, kind, w.q, cap, rows, ws.order, ws.counts, ws.offsets, buf, short, ws.order_scratch)
+        torch.cuda.synchronize()
+        assert int(ws.offsets[w.q].item()) == nnz                      # the caller learns that it did not fit
+        got = buf.cpu().numpy()
+        assert np.all(got[short:] == -7), (name, cap, "written past the capacity")
+        fits = ooff[1:] <= short
+        last = int(ooff[1:][fits].max()) if fits.any() else 0          # rows are in offset order: a prefix fits
+        assert np.array_equal(got[:last], oidx[:last]), (name, cap, "rows inside the capacity")
+        # completion into a buffer that is large enough
+        full = torch.full((nnz + 8,), -7, dtype=torch.int32, device="cuda")
+        order = ws.order if w.q > 8192 else None
+        B.bvh_rows_to_csr(rows, cap, ws.counts, ws.offsets, w.q, full)
+        B.bvh_query_fill_overflow(bvh.nodes, bvh.n, dq, kind, w.q, order, cap, ws.counts, ws.offsets, full)
+        torch.cuda.synchronize()
+        assert np.array_equal(full.cpu().numpy()[:nnz], oidx), (name, cap, "completion")
+    # capacity 0, empty batch, empty hierarchy
+    B.bvh_query_csr(bvh.nodes, bvh.n, dq, kind, w.q, 8, rows, ws.order, ws.counts, ws.offsets, buf, 0, ws.order_scratch)
+    torch.cuda.synchronize()
+    assert np.array_equal(ws.offsets.cpu().numpy()[: w.q + 1], ooff)
+    offs = torch.full((1,), 5, dtype=torch.int64, device="cuda")
+    B.bvh_query_csr(bvh.nodes, bvh.n, dq, kind, 0, 8, None, None, None, offs, None, 0, None)
+    torch.cuda.synchronize()
+    assert int(offs[0].item()) == 0
+    B.bvh_query_csr(None, 0, dq, kind, w.q, 8, rows, ws.order, ws.counts, ws.offsets, buf, short, ws.order_scratch)
+    torch.cuda.synchronize()
+    assert not ws.offsets[: w.q + 1].any()
+
+
 def test_single_pass_rays_and_argument_checks(B, oracle_lib):
     w = W.make("C4", n=30_000, q=0)
     bvh = gpu_build(B, w.prims, w.morton_bits)
