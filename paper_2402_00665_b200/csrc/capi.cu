@@ -155,14 +155,24 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
     if (events && events[k]) cudaEventRecord(static_cast<cudaEvent_t>(events[k]), stream);
   };
   mark(0);
-  if (cudaMemsetAsync(base, 0, L.zero_bytes, stream) != cudaSuccess) return BVH_ERR_CUDA;
-  mark(1);
-  if (launch_scene_bounds(prim, (int)n, is_box, header, stream) != cudaSuccess) return BVH_ERR_CUDA;
-  mark(2);
-  if (launch_morton(prim, (int)n, is_box, morton_bits, header, base + L.keys[0], hist, stream) != cudaSuccess) return BVH_ERR_CUDA;
-  mark(3);
-  if (launch_sort(sort_buffers(scratch, L), L.key_bytes, L.passes, (int)n, stream, events ? events + 4 : nullptr) != cudaSuccess)
-    return BVH_ERR_CUDA;
+  // A small build: bounds, codes and sort in one launch by one block (small_build.cu); nothing of the scratch needs
+  // zeroing then (no histograms, no tile status, and with at most kMergeFan level-1 windows no arrival counter).
+  if (variant == 0 && n <= kSmallBuildMax && hierarchy_total_segments((int)n) <= hierarchy_fan() + 1) {
+    mark(1);
+    if (launch_small_front(prim, (int)n, is_box, morton_bits, header, base + L.keys[0],
+                           reinterpret_cast<uint32_t*>(base + L.vals[0]), stream) != cudaSuccess)
+      return BVH_ERR_CUDA;
+    for (int k = 2; k < 4 + L.passes; ++k) mark(k);
+  } else {
+    if (cudaMemsetAsync(base, 0, L.zero_bytes, stream) != cudaSuccess) return BVH_ERR_CUDA;
+    mark(1);
+    if (launch_scene_bounds(prim, (int)n, is_box, header, stream) != cudaSuccess) return BVH_ERR_CUDA;
+    mark(2);
+    if (launch_morton(prim, (int)n, is_box, morton_bits, header, base + L.keys[0], hist, stream) != cudaSuccess) return BVH_ERR_CUDA;
+    mark(3);
+    if (launch_sort(sort_buffers(scratch, L), L.key_bytes, L.passes, (int)n, stream, events ? events + 4 : nullptr) != cudaSuccess)
+      return BVH_ERR_CUDA;
+  }
   if (variant == 1) {
     if (launch_variant_karras(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
                               nodes, (int)n, header, base + L.total, stream) != 0)

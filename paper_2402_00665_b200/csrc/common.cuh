@@ -142,6 +142,16 @@ cudaError_t launch_scene_bounds(const float* prim, int n, bool is_box, Header* h
 // K2: Morton codes + the digit histograms of every sort pass.
 cudaError_t launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
                    uint32_t* hist, cudaStream_t stream);
+// K1 + K2 + K3 of a small build (n <= kSmallBuildMax) in one launch by one thread-block cluster (small_build.cu): writes the scene
+// bounds into `header`, the sorted codes and the permutation where the one-sweep sort would leave them.  Needs no
+// zero-initialised scratch.
+#ifndef BVH_SMALL_BUILD_MAX
+#define BVH_SMALL_BUILD_MAX 16384
+#endif
+constexpr int kSmallBuildMax = BVH_SMALL_BUILD_MAX;   // <= 16384: a cluster of 8 blocks x 256 threads x 8 pairs
+static_assert(kSmallBuildMax <= 16384, "the pairs of a small build live in one cluster's registers and shared memory");
+cudaError_t launch_small_front(const float* prim, int n, bool is_box, int morton_bits, Header* header, void* codes,
+                               uint32_t* perm, cudaStream_t stream);
 // K3: one-sweep LSD radix sort of (key, index) pairs, `passes` 8-bit digits from the least significant.
 // Pass p reads keys[p&1]/vals[p&1] and writes the other buffer; with an even pass count the result is in
 // keys[0]/vals[0].  final_vals (optional) receives the last pass's values instead of vals[...].
@@ -168,6 +178,7 @@ cudaError_t launch_hierarchy(const float* prim, bool is_box, const void* sorted_
 int hierarchy_levels(int n, int segs[kMaxHierLevels]);   // windows per level, level 1 first; returns the level count
 int hierarchy_total_segments(int n);
 int hierarchy_seg_capacity();
+int hierarchy_fan();          // level-1 windows per level-2 window
 // NEXT-2 measurement variant (variants.cu): Karras' top-down hierarchy + Algorithm 2 + a separate box pass.
 size_t variant_extra_bytes(int64_t n);
 int launch_variant_karras(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,

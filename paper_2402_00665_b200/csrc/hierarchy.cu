@@ -714,5 +714,6 @@ cudaError_t launch_hierarchy(const float* prim, bool is_box, const void* sorted_
 }
 
 int hierarchy_seg_capacity() { return kSegCap; }
+int hierarchy_fan() { return kMergeFan; }
 
 }  // namespace bvh

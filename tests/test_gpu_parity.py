@@ -106,15 +106,35 @@ def test_c1_brute_force(B, oracle_lib):
     assert np.array_equal(csr_rows_sorted(goff, gidx[: goff[-1]]), bidx)
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 7, 31, 32, 33, 255, 256, 257, 4095, 4096, 4097])
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 7, 31, 32, 33, 255, 256, 257, 511, 513, 1024, 1025, 2047, 2048, 2049, 4095,
+                               4096, 4097, 8191, 8192, 8193, 16383, 16384, 16385])
 @pytest.mark.parametrize("bits", [30, 63])
 def test_tiny_and_boundary_sizes(B, oracle_lib, n, bits):
+    """Sizes around every switch of the build: one leaf, one group of 32, one level-1 window of 256, and the cluster sizes
+    and pairs per thread of the one-launch front of a small build (small_build.cu: 256 x {1, 2, 4, 8} pairs x {1 .. 8}
+    blocks, up to 16384; above that the one-sweep pipeline)."""
     pts = W.uniform_cube(n, seed=100 + n)
     o = oracle_lib.build_bvh(pts, bits)
     bvh = gpu_build(B, pts, bits)
     assert_build_equal(export_np(bvh), o, f"n={n}")
     qs = W.spheres_at(W.uniform_cube(64, seed=7), 0.3)
     assert_query_equal(B, bvh, o, oracle_lib, qs, f"n={n}")
+
+
+@pytest.mark.parametrize("bits", [30, 63])
+@pytest.mark.parametrize("n", [700, 3000, 6000, 12_000])
+def test_small_build_boxes_and_ties(B, oracle_lib, n, bits):
+    """The one-launch front of a small build on box primitives and on inputs with many equal codes (a coarse lattice:
+    the stable order of equal codes is the original index, G5/G6), bit for bit against the oracle."""
+    w = W.make("C4", n=n, q=0)
+    o = oracle_lib.build_bvh(w.prims, bits)
+    assert_build_equal(export_np(gpu_build(B, w.prims, bits)), o, f"boxes n={n}")
+    rng = np.random.default_rng(n)
+    pts = (rng.integers(0, 5, size=(n, 3)).astype(np.float32) * np.float32(0.25)) + np.float32(0.0)
+    o = oracle_lib.build_bvh(pts, bits)
+    e = export_np(gpu_build(B, pts, bits))
+    assert_build_equal(e, o, f"lattice n={n}")
+    assert len(np.unique(o.sorted_codes)) <= 125
 
 
 @pytest.mark.parametrize("bits", [30, 63])
