@@ -5,7 +5,8 @@ A "step" is one pass of the whole hot path over one batch of synthetic input: li
 bounds, Morton codes, one-sweep radix sort, modified-Apetrei bottom-up pass with ropes and boxes) followed
 by stackless sphere range search to CSR.  The query part of the step is the single-pass form of
 count-then-fill (order, collect = one traversal that counts and stores rows, scan, rows -> CSR, overflow
-rows); the two-traversal form (count, scan, fill) is timed beside it as `query_two_pass`.  Workload at N=1: BASELINE.json configs[2]
+rows) as ONE call of the C ABI (bvh_query_csr); the same stages as separate calls give the per-kernel breakdown, and
+the two-traversal form (count, scan, fill) is timed beside it as `query_two_pass`.  Workload at N=1: BASELINE.json configs[2]
 ("C3": 10,000,000 Gaussian-mixture points, 30-bit Morton, 1,000,000 sphere queries of radius 0.002), the
 config `north_star` quotes its target on.
 
@@ -251,10 +252,17 @@ def run_ours(args) -> dict | None:
     build_fn = binding.bvh_build_boxes if is_box else binding.bvh_build_points
 
     def step():
-        """One pass of the hot path through the public entry points: the build as ONE call (no events inside it),
-        then the single-pass query with an event after each stage."""
+        """One pass of the hot path through the public entry points: the build as ONE call and the single-pass query
+        as ONE call (bvh_query_csr), no events inside either."""
         e_b0.record()
         build_fn(d_prims, n, bits, bvh.nodes, bvh.scratch)
+        e_b1.record()
+        binding.bvh_query_csr(bvh.nodes, n, d_queries, kind, q, cap, d_rows, ws.order, ws.counts, ws.offsets, d_indices,
+                              d_indices.numel(), ws.order_scratch)
+        e_over.record()
+
+    def staged_query():
+        """The same query through its separate entry points, an event after each stage (per-kernel breakdown)."""
         e_b1.record()
         order_fn(bvh.nodes, n, d_queries, q, ws.order, ws.order_scratch)
         e_order.record()
@@ -280,15 +288,23 @@ def run_ours(args) -> dict | None:
     build_names = ["init", "bounds", "morton"] + [f"sort_pass{p}" for p in range(P)] + ["hierarchy"]
     query_names = ["order", "collect", "scan", "rows_to_csr", "overflow"]
     names = build_names + query_names
-    launches_per_step = {"init": 0, "bounds": 1, "morton": 1, **{f"sort_pass{p}": 1 for p in range(P)},
-                         "hierarchy": 2 if n > 256 else 1, "order": 5, "collect": 1, "scan": 3, "rows_to_csr": 1,
-                         "overflow": 1}
+    # kernels of this library per stage when the stages are called one by one (the staged legs) ...
+    small_build = n <= 16384          # bounds + Morton + sort in one launch (csrc/small_build.cu), no memset
+    launches_per_step = {"init": 0, "bounds": 1, "morton": 0 if small_build else 1,
+                         **{f"sort_pass{p}": 0 if small_build else 1 for p in range(P)},
+                         "hierarchy": 2 if n > 256 else 1, "order": 5 if q > 8192 else 1, "collect": 1,
+                         "scan": 3 if q > 4096 else 1, "rows_to_csr": 1, "overflow": 1}
+    # ... and in the timed step, where the query is one call: no identity order for q <= 8192, scan + row copy fused for q <= 4096
+    step_launches = (sum(launches_per_step[k] for k in ["bounds", "morton", "hierarchy"] + [f"sort_pass{p}" for p in range(P)])
+                     + (5 if q > 8192 else 0) + 1 + (4 if q > 4096 else 1) + 1)
 
     def read_times() -> dict:
-        return {"_build": e_b0.elapsed_time(e_b1), "order": e_b1.elapsed_time(e_order),
-                "collect": e_order.elapsed_time(e_collect), "scan": e_collect.elapsed_time(e_scan),
-                "rows_to_csr": e_scan.elapsed_time(e_rows), "overflow": e_rows.elapsed_time(e_over),
-                "_query": e_b1.elapsed_time(e_over), "_step": e_b0.elapsed_time(e_over)}
+        return {"_build": e_b0.elapsed_time(e_b1), "_query": e_b1.elapsed_time(e_over), "_step": e_b0.elapsed_time(e_over)}
+
+    def read_query_stage_times() -> dict:
+        return {"order": e_b1.elapsed_time(e_order), "collect": e_order.elapsed_time(e_collect),
+                "scan": e_collect.elapsed_time(e_scan), "rows_to_csr": e_scan.elapsed_time(e_rows),
+                "overflow": e_rows.elapsed_time(e_over), "_query_staged": e_b1.elapsed_time(e_over)}
 
     def read_stage_times() -> dict:
         t = {"init": stage[0].elapsed_time(stage[1]), "bounds": stage[1].elapsed_time(stage[2]),
@@ -324,6 +340,14 @@ def run_ours(args) -> dict | None:
     torch.cuda.synchronize()
     dist_barrier(world, device)
     clocks = sampler.stop() if rank == 0 else None
+
+    # ---- per-stage breakdown of the single-pass query: the same stages as separate calls, an event after each ----------
+    for _ in range(args.steps):
+        flush.fill_(1)
+        staged_query()
+        torch.cuda.synchronize()
+        for k, v in read_query_stage_times().items():
+            acc[k] = acc.get(k, 0.0) + v
 
     # ---- the two-traversal query, same inputs, same hierarchy (not part of `value` / `ms_per_step`) ------------------
     for _ in range(args.steps):
@@ -481,7 +505,8 @@ def run_ours(args) -> dict | None:
         "query": {"ms": round(ms["_query"], 4), "mqueries_per_s": round(q_all / (ms["_query"] * 1e-3) / 1e6, 3),
                   "alg_bytes": int(model["query_total"]), "gbs": round(query_gbs, 1),
                   "frac_of_measured_peak": round(query_gbs / peak, 4), "frac_of_8TBs": round(query_gbs / NOMINAL_HBM_GBS, 4),
-                  "path": "single pass: order + collect + scan + rows_to_csr + fill_overflow (byte-identical CSR)",
+                  "path": "bvh_query_csr, one call: order + collect + scan + rows_to_csr + fill_overflow (byte-identical CSR)",
+                  "staged_ms": round(ms["_query_staged"], 4),
                   "excluded": "nnz read-back and indices allocation (included in e2e)"},
         "query_two_pass": {"ms": round(tp_ms, 4), "mqueries_per_s": round(q_all / (tp_ms * 1e-3) / 1e6, 3),
                            "count_ms": round(ms["tp_count"], 4), "scan_ms": round(ms["tp_scan"], 4),
@@ -491,7 +516,7 @@ def run_ours(args) -> dict | None:
                      "alg_bytes_per_launch": dk["alg_bytes"], "ms_per_launch": dk["ms"]},
         "kernels": kernels,
         "build_staged_ms": round(ms["_build_staged"], 4),
-        "gpu_launches": K * sum(launches_per_step.values()),
+        "gpu_launches": K * step_launches,
         "e2e": {"value": round(n_all / (e2e_b / e2e_steps) / 1e6, 2), "unit": UNIT,
                 "h2d_bytes_per_step": int(h_prims.numel() * 4 + h_queries.numel() * 4),
                 "d2h_bytes_per_step": int(32 + (q + 1) * 8 + nnz * 4), "steps": e2e_steps,
