@@ -46,9 +46,10 @@ NOMINAL_HBM_GBS = 8000.0   # the denominator BASELINE.json north_star names
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of a kernel from the `ncu --set full` captures
 # summarised in profiles/, keyed by (workload, n, q): `roofline.traffic` is null for any other workload or size.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r02_ncu.md rows 13 (collect), 17 (rows_to_csr), 19 (count), 23 (fill), 6 (hierarchy, level 1): DRAM rd + wr
-    ("C3", 10_000_000, 1_000_000): {"collect": 4_324_314_000, "rows_to_csr": 5_007_352_000, "count": 390_046_000,
-                                    "fill": 4_343_356_000, "hierarchy": 1_330_786_000},
+    # profiles/r02b_ncu.md: one step, rows 2 (collect), 6 (rows_to_csr), 14 (hierarchy, level 1); two-pass leg, rows 0 (count),
+    # 1 (fill): DRAM read + write
+    ("C3", 10_000_000, 1_000_000): {"collect": 3_143_800_000, "rows_to_csr": 4_996_000_000, "count": 233_777_000,
+                                    "fill": 3_204_300_000, "hierarchy": 1_330_800_000},
 }
 
 
@@ -71,6 +72,7 @@ def byte_model(n: int, q: int, nnz: int, prim_floats: int, query_floats: int, bi
         "rows_to_csr": (4 + 8) * q + 8 * nnz,            # counts, offsets, every hit read and written once
         "overflow": 4 * q,                               # counts (no row overflows when the capacity holds the largest row)
     }
+    per_kernel["front"] = sum(v for k, v in per_kernel.items() if k in ("init", "bounds", "morton") or k.startswith("sort_pass"))
     build_total = (3 * S + 4 * K + (2 * P - 1) * (K + 4) + 100) * n      # SURVEY.md B_build
     query_total = (2 * Sq + 24) * q + 4 * nnz                            # SURVEY.md B_query
     return {"per_kernel": per_kernel, "build_total": build_total, "query_total": query_total}
@@ -285,17 +287,18 @@ def run_ours(args) -> dict | None:
         fill_fn(bvh.nodes, n, d_queries, q, ws.order, ws.offsets, d_indices)
         t_c3.record()
 
-    build_names = ["init", "bounds", "morton"] + [f"sort_pass{p}" for p in range(P)] + ["hierarchy"]
+    small_build = n <= 16384          # bounds + Morton + sort in one launch (csrc/small_build.cu), no memset
+    build_names = ["front", "hierarchy"] if small_build else \
+        ["init", "bounds", "morton"] + [f"sort_pass{p}" for p in range(P)] + ["hierarchy"]
     query_names = ["order", "collect", "scan", "rows_to_csr", "overflow"]
     names = build_names + query_names
     # kernels of this library per stage when the stages are called one by one (the staged legs) ...
-    small_build = n <= 16384          # bounds + Morton + sort in one launch (csrc/small_build.cu), no memset
-    launches_per_step = {"init": 0, "bounds": 1, "morton": 0 if small_build else 1,
-                         **{f"sort_pass{p}": 0 if small_build else 1 for p in range(P)},
+    launches_per_step = {**({"front": 1} if small_build else
+                            {"init": 0, "bounds": 1, "morton": 1, **{f"sort_pass{p}": 1 for p in range(P)}}),
                          "hierarchy": 2 if n > 256 else 1, "order": 5 if q > 8192 else 1, "collect": 1,
                          "scan": 3 if q > 4096 else 1, "rows_to_csr": 1, "overflow": 1}
     # ... and in the timed step, where the query is one call: no identity order for q <= 8192, scan + row copy fused for q <= 4096
-    step_launches = (sum(launches_per_step[k] for k in ["bounds", "morton", "hierarchy"] + [f"sort_pass{p}" for p in range(P)])
+    step_launches = (sum(launches_per_step[k] for k in build_names)
                      + (5 if q > 8192 else 0) + 1 + (4 if q > 4096 else 1) + 1)
 
     def read_times() -> dict:
@@ -307,6 +310,9 @@ def run_ours(args) -> dict | None:
                 "overflow": e_rows.elapsed_time(e_over), "_query_staged": e_b1.elapsed_time(e_over)}
 
     def read_stage_times() -> dict:
+        if small_build:   # bounds + Morton + sort are one launch (and there is no memset): one stage, "front"
+            return {"front": stage[0].elapsed_time(stage[3 + P]), "hierarchy": stage[3 + P].elapsed_time(stage[12]),
+                    "_build_staged": stage[0].elapsed_time(stage[12])}
         t = {"init": stage[0].elapsed_time(stage[1]), "bounds": stage[1].elapsed_time(stage[2]),
              "morton": stage[2].elapsed_time(stage[3])}
         prev = stage[3]

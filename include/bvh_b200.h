@@ -74,6 +74,8 @@ int bvh_build_boxes(const float* minmax, int64_t n, int morton_bits, void* nodes
  * asynchronous, nothing is created or synchronised.  NULL entries are skipped.  Stages:
  *   [0] start  [1] scratch initialised  [2] scene bounds  [3] Morton codes + digit histograms
  *   [4+p] sort pass p (p < 4 for 30-bit, p < 8 for 63-bit)  [12] bottom-up pass (Algorithm 4)
+ * A small build (n <= 16384) runs bounds, Morton codes and the whole sort as ONE launch and initialises no scratch: only
+ * [0], the event of the last sort pass ([7] or [11]) and [12] are recorded then.
  * stage_events must hold BVH_NUM_STAGE_EVENTS entries.  prim_is_box: 0 = xyz points, 1 = minmax boxes. */
 #define BVH_NUM_STAGE_EVENTS 13
 int bvh_build_staged(const float* prim, int prim_is_box, int64_t n, int morton_bits, void* nodes, void* scratch,

@@ -158,11 +158,10 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   // A small build: bounds, codes and sort in one launch by one block (small_build.cu); nothing of the scratch needs
   // zeroing then (no histograms, no tile status, and with at most kMergeFan level-1 windows no arrival counter).
   if (variant == 0 && n <= kSmallBuildMax && hierarchy_total_segments((int)n) <= hierarchy_fan() + 1) {
-    mark(1);
     if (launch_small_front(prim, (int)n, is_box, morton_bits, header, base + L.keys[0],
                            reinterpret_cast<uint32_t*>(base + L.vals[0]), stream) != cudaSuccess)
       return BVH_ERR_CUDA;
-    for (int k = 2; k < 4 + L.passes; ++k) mark(k);
+    mark(3 + L.passes);    // one launch: only the end of the front is marked (an event per stage would cost more than the stage)
   } else {
     if (cudaMemsetAsync(base, 0, L.zero_bytes, stream) != cudaSuccess) return BVH_ERR_CUDA;
     mark(1);
