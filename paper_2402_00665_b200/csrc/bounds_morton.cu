@@ -149,11 +149,15 @@ template <typename KeyT, int PASSES, int PRIM_FLOATS, bool FROM_ROOT>
 __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __restrict__ prim, int n,
                                                                 const Header* __restrict__ header,
                                                                 const NodesHeader* __restrict__ root,
-                                                                KeyT* __restrict__ codes, uint32_t* __restrict__ hist) {
+                                                                KeyT* __restrict__ codes, uint32_t* __restrict__ hist,
+                                                                int shift0, const uint32_t* __restrict__ run_if) {
+  // shift0: the histograms are those of the PASSES 8-bit digits from bit shift0 up.  run_if (optional): the kernel is
+  // part of the conditional second sort of a 63-bit build (tie_fixup.cu) and does nothing unless *run_if != 0.
   __shared__ uint32_t s_hist[PASSES * 256];
   for (int i = threadIdx.x; i < PASSES * 256; i += kMortonThreads) s_hist[i] = 0;
   pdl_wait();
   pdl_trigger();
+  if (run_if && *run_if == 0) return;
   float scene[6];
   if (FROM_ROOT) {
 #pragma unroll
@@ -181,7 +185,7 @@ __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __r
     }
     const KeyT code = morton_code<KeyT>(cell);
 #pragma unroll
-    for (int p = 0; p < PASSES; ++p) atomicAdd(&s_hist[p * 256 + (int)((code >> (8 * p)) & 0xFF)], 1u);
+    for (int p = 0; p < PASSES; ++p) atomicAdd(&s_hist[p * 256 + (int)((code >> (shift0 + 8 * p)) & 0xFF)], 1u);
     return code;
   };
   const int64_t tid0 = (int64_t)blockIdx.x * kMortonThreads + threadIdx.x, stride = (int64_t)gridDim.x * kMortonThreads;
@@ -253,30 +257,31 @@ static unsigned morton_grid(int n, int per_thread = 1) {
 }
 
 cudaError_t launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
-                   uint32_t* hist, cudaStream_t stream) {
+                          uint32_t* hist, cudaStream_t stream, int passes, int shift0, const uint32_t* run_if) {
   const unsigned g = morton_grid(n, is_box ? 2 : 4);
+  const dim3 G(g), T(kMortonThreads);
+  const NodesHeader* none = nullptr;
   if (morton_bits == 30) {
-    if (is_box)
-      return launch_pdl(morton_kernel<uint32_t, 4, 6, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint32_t*)codes, hist);
-    else
-      return launch_pdl(morton_kernel<uint32_t, 4, 3, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint32_t*)codes, hist);
-  } else {
-    if (is_box)
-      return launch_pdl(morton_kernel<uint64_t, 8, 6, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint64_t*)codes, hist);
-    else
-      return launch_pdl(morton_kernel<uint64_t, 8, 3, false>, dim3(g), dim3(kMortonThreads), 0, stream, prim, n, header, nullptr, (uint64_t*)codes, hist);
+    if (is_box) return launch_pdl(morton_kernel<uint32_t, 4, 6, false>, G, T, 0, stream, prim, n, header, none, (uint32_t*)codes, hist, shift0, run_if);
+    return launch_pdl(morton_kernel<uint32_t, 4, 3, false>, G, T, 0, stream, prim, n, header, none, (uint32_t*)codes, hist, shift0, run_if);
   }
+  if (passes == 4) {   // 63-bit codes sorted by their upper 32 bits first (tie_fixup.cu)
+    if (is_box) return launch_pdl(morton_kernel<uint64_t, 4, 6, false>, G, T, 0, stream, prim, n, header, none, (uint64_t*)codes, hist, shift0, run_if);
+    return launch_pdl(morton_kernel<uint64_t, 4, 3, false>, G, T, 0, stream, prim, n, header, none, (uint64_t*)codes, hist, shift0, run_if);
+  }
+  if (is_box) return launch_pdl(morton_kernel<uint64_t, 8, 6, false>, G, T, 0, stream, prim, n, header, none, (uint64_t*)codes, hist, shift0, run_if);
+  return launch_pdl(morton_kernel<uint64_t, 8, 3, false>, G, T, 0, stream, prim, n, header, none, (uint64_t*)codes, hist, shift0, run_if);
 }
 
 cudaError_t launch_query_morton(const float* queries, int q, int kind, const NodesHeader* root, uint32_t* codes, uint32_t* hist,
                          cudaStream_t stream) {
   const unsigned g = morton_grid(q);
   if (kind == 0)
-    return launch_pdl(morton_kernel<uint32_t, 4, 4, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist);
+    return launch_pdl(morton_kernel<uint32_t, 4, 4, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, 0, nullptr);
   else if (kind == 2)
-    return launch_pdl(morton_kernel<uint32_t, 4, 8, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist);
+    return launch_pdl(morton_kernel<uint32_t, 4, 8, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, 0, nullptr);
   else
-    return launch_pdl(morton_kernel<uint32_t, 4, 6, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist);
+    return launch_pdl(morton_kernel<uint32_t, 4, 6, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, 0, nullptr);
 }
 
 }  // namespace bvh

@@ -21,6 +21,7 @@ ScratchLayout scratch_layout(int64_t n, int morton_bits) {
   ScratchLayout L{};
   L.key_bytes = (morton_bits == 30) ? 4 : 8;
   L.passes = (morton_bits == 30) ? 4 : 8;
+  L.slots = (morton_bits == 30) ? 4 : 12;
   const int tile = sort_tile_items(L.key_bytes);
   L.tiles = (int)((n + tile - 1) / tile);
   if (L.tiles < 1) L.tiles = 1;
@@ -28,13 +29,15 @@ ScratchLayout scratch_layout(int64_t n, int morton_bits) {
   L.header = off;
   off += sizeof(Header);
   L.hist = off;
-  off += align_up((size_t)L.passes * 256 * sizeof(uint32_t), 256);
+  off += align_up((size_t)L.slots * 256 * sizeof(uint32_t), 256);
   L.status = off;
-  off += align_up((size_t)L.passes * L.tiles * 256 * sizeof(uint32_t), 256);
+  off += align_up((size_t)L.slots * L.tiles * 256 * sizeof(uint32_t), 256);
   const size_t nn = (size_t)(n > 0 ? n : 1);
   L.segments = hierarchy_total_segments((int)nn);
   L.arrivals = off;
   off += align_up((size_t)L.segments * sizeof(uint32_t), 256);
+  L.fix_flag = off;
+  if (morton_bits == 63) off += align_up((size_t)tie_fixup_tiles((int64_t)nn) * sizeof(uint32_t), 256);
   L.zero_bytes = off;
   for (int b = 0; b < 2; ++b) {
     L.keys[b] = off;
@@ -48,6 +51,8 @@ ScratchLayout scratch_layout(int64_t n, int morton_bits) {
   off += align_up((size_t)L.segments * hierarchy_seg_capacity() * sizeof(int2), 256);
   L.seg_count = off;
   off += align_up((size_t)L.segments * sizeof(int32_t), 256);
+  L.fix_list = off;
+  if (morton_bits == 63) off += align_up((size_t)tie_fixup_tiles((int64_t)nn) * sizeof(uint32_t), 256);
   L.total = off;
   return L;
 }
@@ -134,6 +139,11 @@ static inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_
 
 static int check_launch() { return cudaGetLastError() == cudaSuccess ? BVH_OK : BVH_ERR_CUDA; }
 
+#ifndef BVH_TWO_STAGE_SORT
+#define BVH_TWO_STAGE_SORT 1
+#endif
+constexpr bool kTwoStageSort = BVH_TWO_STAGE_SORT != 0;
+
 static int build(const float* prim, bool is_box, int64_t n, int morton_bits, void* nodes, void* scratch,
                  size_t scratch_bytes, void* stream_, void* const* events = nullptr, int variant = 0) {
   if (n < 0) return BVH_ERR_INVALID_ARGUMENT;
@@ -167,10 +177,33 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
     mark(1);
     if (launch_scene_bounds(prim, (int)n, is_box, header, stream) != cudaSuccess) return BVH_ERR_CUDA;
     mark(2);
-    if (launch_morton(prim, (int)n, is_box, morton_bits, header, base + L.keys[0], hist, stream) != cudaSuccess) return BVH_ERR_CUDA;
-    mark(3);
-    if (launch_sort(sort_buffers(scratch, L), L.key_bytes, L.passes, (int)n, stream, events ? events + 4 : nullptr) != cudaSuccess)
-      return BVH_ERR_CUDA;
+    if (morton_bits == 30 || !kTwoStageSort) {
+      if (launch_morton(prim, (int)n, is_box, morton_bits, header, base + L.keys[0], hist, stream, L.passes) != cudaSuccess) return BVH_ERR_CUDA;
+      mark(3);
+      if (launch_sort(sort_buffers(scratch, L), L.key_bytes, L.passes, (int)n, stream, events ? events + 4 : nullptr) != cudaSuccess)
+        return BVH_ERR_CUDA;
+    } else {
+      // 63-bit codes (tie_fixup.cu): four passes over the upper 32 bits, then every run of equal upper bits ordered by the
+      // lower 31 in shared memory.  Should a run not fit a block, the fix-up raises header->sort_fallback and the plain
+      // eight-pass sort below redoes the order from fresh codes; its nine kernels are enqueued in any case (nothing here
+      // may read the flag back) and return at once while the flag is clear.
+      const SortBuffers B = sort_buffers(scratch, L);
+      if (launch_morton(prim, (int)n, is_box, morton_bits, header, base + L.keys[0], hist, stream, 4, 31) != cudaSuccess) return BVH_ERR_CUDA;
+      mark(3);
+      if (launch_sort(B, L.key_bytes, 4, (int)n, stream, events ? events + 4 : nullptr, 31, 0) != cudaSuccess) return BVH_ERR_CUDA;
+      if (launch_tie_fixup(base + L.keys[0], B.vals[0], (int)n, reinterpret_cast<uint32_t*>(base + L.fix_flag),
+                           reinterpret_cast<uint32_t*>(base + L.fix_list), &header->fix_count, &header->sort_fallback,
+                           stream) != cudaSuccess)
+        return BVH_ERR_CUDA;
+      mark(8);
+      if (launch_morton(prim, (int)n, is_box, morton_bits, header, base + L.keys[0], hist + 4 * 256, stream, 8, 0,
+                        &header->sort_fallback) != cudaSuccess)
+        return BVH_ERR_CUDA;
+      if (launch_sort(B, L.key_bytes, 8, (int)n, stream, nullptr, 0, 4, &header->sort_fallback) != cudaSuccess) return BVH_ERR_CUDA;
+      mark(9);
+      mark(10);
+      mark(11);
+    }
   }
   if (variant == 1) {
     if (launch_variant_karras(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),

@@ -52,22 +52,27 @@ struct ScratchLayout {
   size_t hist;          // uint32 [passes][256]   global digit histograms
   size_t status;        // uint32 [passes][tiles][256]  onesweep tile status words
   size_t arrivals;      // uint32 [segments]  children arrived at each window of the bottom-up pass (hierarchy.cu)
+  size_t fix_flag;      // uint32 [tie_fixup_tiles]  63-bit codes: tile is on the work list of long runs (tie_fixup.cu)
   size_t zero_bytes;    // header + hist + status + arrivals are contiguous from 0 and zero-initialised per build
   size_t keys[2];       // KeyT [n]   ping-pong; sorted codes end in keys[0]
   size_t vals[2];       // uint32 [n] ping-pong; permutation ends in vals[0]
   size_t seg_items;     // int2 [segments][192]  subtrees handed from one window of the bottom-up pass to its parent
   size_t seg_count;     // int32 [segments]      how many each window handed over
+  size_t fix_list;      // uint32 [tie_fixup_tiles]  the work list
   size_t total;
   int segments;         // windows of all levels of the bottom-up pass (hierarchy.cu)
-  int passes;
+  int passes;           // 8-bit digits of a code: 4 (30-bit) or 8 (63-bit)
+  int slots;            // histogram / status / ticket slots: passes, or 4 + 8 for the two-stage sort of 63-bit codes
   int tiles;
   int key_bytes;
 };
 
 struct Header {
   uint32_t bounds_enc[8];    // [0..2] = ~ord(min.xyz), [3..5] = ord(max.xyz), maximised with atomicMax
-  uint32_t tile_counter[8];  // one dynamic tile counter per sort pass
-  uint32_t pad[48];
+  uint32_t tile_counter[16]; // one dynamic tile counter per sort pass (63-bit builds: 4 passes + 8 of the conditional second sort)
+  uint32_t sort_fallback;    // raised by tie_long_kernel: a run of equal upper bits did not fit a block; run the second sort
+  uint32_t fix_count;        // tiles on the work list of tie_long_kernel
+  uint32_t pad[38];
 };
 static_assert(sizeof(Header) == 256, "header is one 256-byte block");
 
@@ -140,8 +145,9 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
 // K1: scene bounds.  is_box: prim is n*6 floats, else n*3.
 cudaError_t launch_scene_bounds(const float* prim, int n, bool is_box, Header* header, cudaStream_t stream);
 // K2: Morton codes + the digit histograms of every sort pass.
+// passes / shift0: histograms of `passes` 8-bit digits from bit shift0 up.  run_if: see tie_fixup.cu.
 cudaError_t launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
-                   uint32_t* hist, cudaStream_t stream);
+                          uint32_t* hist, cudaStream_t stream, int passes, int shift0 = 0, const uint32_t* run_if = nullptr);
 // K1 + K2 + K3 of a small build (n <= kSmallBuildMax) in one launch by one thread-block cluster (small_build.cu): writes the scene
 // bounds into `header`, the sorted codes and the permutation where the one-sweep sort would leave them.  Needs no
 // zero-initialised scratch.
@@ -166,7 +172,14 @@ struct SortBuffers {
   uint32_t* final_vals;
 };
 SortBuffers sort_buffers(void* scratch, const ScratchLayout& L);
-cudaError_t launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStream_t stream, void* const* pass_events);
+// shift0: first bit of pass 0's digit.  slot0: pass p uses histogram, status block and ticket slot0 + p.  run_if: see tie_fixup.cu.
+cudaError_t launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStream_t stream, void* const* pass_events,
+                        int shift0 = 0, int slot0 = 0, const uint32_t* run_if = nullptr);
+// 63-bit codes sorted by their upper 32 bits: orders every run of equal upper bits by the lower 31 (tie_fixup.cu).
+// tile_flag [tie_fixup_tiles(n)] zeroed, tile_list [tie_fixup_tiles(n)], list_count zeroed: the work list of long runs.
+cudaError_t launch_tie_fixup(void* keys, uint32_t* vals, int n, uint32_t* tile_flag, uint32_t* tile_list, uint32_t* list_count,
+                             uint32_t* fallback, cudaStream_t stream);
+int tie_fixup_tiles(int64_t n);
 // Morton codes (30-bit) of query centres in the frame of the root box + digit histograms: orders queries.
 cudaError_t launch_query_morton(const float* queries, int q, int kind, const NodesHeader* frame, uint32_t* codes, uint32_t* hist,
                          cudaStream_t stream);

@@ -80,7 +80,11 @@ __device__ __forceinline__ void load_box_cg(const char* nodes, int n, int leaf_k
 #endif
 constexpr int kSegCap = 192;                       // >= 186 = 2 x 93 bits of augmented key
 constexpr int kMergeFan = BVH_MERGE_FAN;           // windows of the level below per merge window
-constexpr int kMergeFanMax = 128;                  // what the prefix / search code of merge_window is written for
+#ifndef BVH_MERGE_FAN_MAX
+#define BVH_MERGE_FAN_MAX (BVH_MERGE_FAN <= 128 ? 128 : (BVH_MERGE_FAN <= 256 ? 256 : 512))
+#endif
+constexpr int kMergeFanMax = BVH_MERGE_FAN_MAX;    // a power of two >= kMergeFan: the prefix / search code of merge_window
+static_assert((kMergeFanMax & (kMergeFanMax - 1)) == 0 && kMergeFanMax % 32 == 0, "segment prefix: whole lanes, binary search");
 static_assert(kMergeFan >= 2 && kMergeFan <= kMergeFanMax, "merge_window handles up to kMergeFanMax child windows");
 constexpr int kMergeMaxItems = BVH_MERGE_MAX_ITEMS;  // items a merge window holds in shared memory at once
 static_assert(kMergeMaxItems >= 2 * kSegCap, "a pass over windows of kMergeMaxItems items must shrink the list");

@@ -301,7 +301,7 @@ template <typename KeyT, bool IOTA, bool TOP>
 __global__ void __launch_bounds__(kSortThreads, BVH_SORT_MINBLOCKS)
 onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_out, const uint32_t* __restrict__ vals_in,
                      uint32_t* __restrict__ vals_out, const uint32_t* __restrict__ hist, uint32_t* status,
-                     uint32_t* tile_counter, int n, int shift) {
+                     uint32_t* tile_counter, int n, int shift, const uint32_t* __restrict__ run_if) {
   constexpr int TILE = SortCfg<KeyT>::TILE;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SortSmem<KeyT>& s = *reinterpret_cast<SortSmem<KeyT>*>(smem_raw);
@@ -311,20 +311,34 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_o
   if (tid < 256) s.tile_hist[tid] = 0;
   pdl_wait();
   pdl_trigger();
-  if (tid == 0) s.tile = atomicAdd(tile_counter, 1u);
-  __syncthreads();
-  const uint32_t tile = s.tile;
-  const uint32_t tile_base = tile * (uint32_t)TILE;
-  const int valid_in_tile = min(TILE, n - (int)tile_base);
-  if (valid_in_tile == TILE)
-    sort_tile<KeyT, IOTA, true, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, TILE, shift);
-  else
-    sort_tile<KeyT, IOTA, false, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, valid_in_tile,
-                                 shift);
+  // A pass of the conditional second sort of a 63-bit build (tie_fixup.cu): nothing to do unless the flag is up.  Such a
+  // pass is launched with a small grid whose blocks keep taking tiles (tickets) until none is left, so that the usual
+  // case -- flag clear -- costs a launch of a few hundred blocks whatever n is.
+  if (run_if && *run_if == 0) return;
+  const uint32_t tiles = (uint32_t)((n + TILE - 1) / TILE);
+  while (true) {
+    if (tid == 0) s.tile = atomicAdd(tile_counter, 1u);
+    __syncthreads();
+    const uint32_t tile = s.tile;
+    if (tile >= tiles) return;
+    const uint32_t tile_base = tile * (uint32_t)TILE;
+    const int valid_in_tile = min(TILE, n - (int)tile_base);
+    if (valid_in_tile == TILE)
+      sort_tile<KeyT, IOTA, true, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, TILE, shift);
+    else
+      sort_tile<KeyT, IOTA, false, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, valid_in_tile,
+                                        shift);
+    if (!run_if) return;                // the ordinary pass: one tile per block
+    __syncthreads();
+    for (int i = tid; i < kSortWarps * kSortChains * 256; i += kSortThreads) (&s.warp_hist[0][0][0])[i] = 0;
+    if (tid < 256) s.tile_hist[tid] = 0;
+    __syncthreads();
+  }
 }
 
 template <typename KeyT>
-static cudaError_t sort_all(const SortBuffers& B, int n, int passes, cudaStream_t stream, void* const* pass_events) {
+static cudaError_t sort_all(const SortBuffers& B, int n, int passes, cudaStream_t stream, void* const* pass_events, int shift0,
+                            int slot0, const uint32_t* run_if) {
   const int tiles = (n + SortCfg<KeyT>::TILE - 1) / SortCfg<KeyT>::TILE;
   KeyT* keys[2] = {static_cast<KeyT*>(B.keys[0]), static_cast<KeyT*>(B.keys[1])};
   const size_t smem = sizeof(SortSmem<KeyT>);
@@ -337,19 +351,23 @@ static cudaError_t sort_all(const SortBuffers& B, int n, int passes, cudaStream_
   }();
   if (attr != cudaSuccess) return attr;
   for (int p = 0; p < passes; ++p) {
-    const int in = p & 1, out = in ^ 1;
-    uint32_t* st = B.status + (size_t)p * tiles * 256;
+    const int in = p & 1, out = in ^ 1, slot = slot0 + p;     // slot: which histogram / status block / ticket this pass uses
+    uint32_t* st = B.status + (size_t)slot * tiles * 256;
     uint32_t* vout = (p == passes - 1 && B.final_vals) ? B.final_vals : B.vals[out];
+    const int shift = shift0 + 8 * p;
+    const uint32_t* vin = B.vals[in];
+    const uint32_t* none = nullptr;
     cudaError_t e;
+    const int blocks = (run_if && tiles > 4 * sm_count()) ? 4 * sm_count() : tiles;   // conditional pass: persistent grid
     if (p == 0)
-      e = launch_pdl(onesweep_pass_kernel<KeyT, true, false>, dim3(tiles), dim3(kSortThreads), smem, stream,
-                 keys[in], keys[out], nullptr, vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
-    else if (p == passes - 1)
-      e = launch_pdl(onesweep_pass_kernel<KeyT, false, true>, dim3(tiles), dim3(kSortThreads), smem, stream,
-                 keys[in], keys[out], B.vals[in], vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
+      e = launch_pdl(onesweep_pass_kernel<KeyT, true, false>, dim3(blocks), dim3(kSortThreads), smem, stream,
+                 keys[in], keys[out], none, vout, B.hist + slot * 256, st, B.tile_counters + slot, n, shift, run_if);
+    else if (p == passes - 1 && sizeof(KeyT) == 4)   // (64-bit codes: the top digit of neighbouring keys is rarely shared; ballots)
+      e = launch_pdl(onesweep_pass_kernel<KeyT, false, true>, dim3(blocks), dim3(kSortThreads), smem, stream,
+                 keys[in], keys[out], vin, vout, B.hist + slot * 256, st, B.tile_counters + slot, n, shift, run_if);
     else
-      e = launch_pdl(onesweep_pass_kernel<KeyT, false, false>, dim3(tiles), dim3(kSortThreads), smem, stream,
-                 keys[in], keys[out], B.vals[in], vout, B.hist + p * 256, st, B.tile_counters + p, n, 8 * p);
+      e = launch_pdl(onesweep_pass_kernel<KeyT, false, false>, dim3(blocks), dim3(kSortThreads), smem, stream,
+                 keys[in], keys[out], vin, vout, B.hist + slot * 256, st, B.tile_counters + slot, n, shift, run_if);
     if (e != cudaSuccess) return e;
     if (pass_events && pass_events[p]) cudaEventRecord(static_cast<cudaEvent_t>(pass_events[p]), stream);
   }
@@ -370,9 +388,10 @@ SortBuffers sort_buffers(void* scratch, const ScratchLayout& L) {
   return B;
 }
 
-cudaError_t launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStream_t stream, void* const* pass_events) {
-  if (key_bytes == 4) return sort_all<uint32_t>(B, n, passes, stream, pass_events);
-  return sort_all<uint64_t>(B, n, passes, stream, pass_events);
+cudaError_t launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStream_t stream, void* const* pass_events,
+                        int shift0, int slot0, const uint32_t* run_if) {
+  if (key_bytes == 4) return sort_all<uint32_t>(B, n, passes, stream, pass_events, shift0, slot0, run_if);
+  return sort_all<uint64_t>(B, n, passes, stream, pass_events, shift0, slot0, run_if);
 }
 
 }  // namespace bvh

@@ -137,6 +137,49 @@ def test_small_build_boxes_and_ties(B, oracle_lib, n, bits):
     assert len(np.unique(o.sorted_codes)) <= 125
 
 
+@pytest.mark.parametrize("pattern", ["pairs", "short", "serial_limit", "medium", "tile_edge", "long", "mixed", "coincident_blocks"])
+def test_two_stage_sort_of_63bit_codes(B, oracle_lib, pattern):
+    """63-bit builds sort by the upper 32 bits of the code and then order every run of equal upper bits by the lower 31
+    (csrc/tie_fixup.cu).  Inputs whose primitives share 32-bit cells in runs of every size class: pairs, runs up to the
+    one-thread limit (32) and just past it, runs of hundreds (block path), runs that straddle the 2048-position tiles,
+    runs too long for a block (the conditional eight-pass sort takes over), exact duplicates inside runs (stability).
+    The hierarchy must be the oracle's bit for bit in every case."""
+    rng = np.random.default_rng(abs(hash(pattern)) % (1 << 31))
+    def cluster(m, side):                      # m points inside one tiny cube: same upper bits, different lower bits
+        c = rng.random(3) * 0.9 + 0.05
+        return (c + rng.random((m, 3)) * side).astype(np.float32)
+    bg = rng.random((40_000, 3)).astype(np.float32)
+    corners = np.array([[0, 0, 0], [1, 1, 1]], np.float32)
+    if pattern == "pairs":
+        parts = [cluster(2, 1e-6) for _ in range(3000)]
+    elif pattern == "short":
+        parts = [cluster(int(rng.integers(2, 20)), 1e-6) for _ in range(1500)]
+    elif pattern == "serial_limit":
+        parts = [cluster(m, 1e-6) for m in (31, 32, 33, 34, 32, 33) * 40]
+    elif pattern == "medium":
+        parts = [cluster(int(rng.integers(100, 900)), 2e-6) for _ in range(40)]
+    elif pattern == "tile_edge":
+        parts = [cluster(int(rng.integers(1500, 2040)), 2e-6) for _ in range(12)]
+    elif pattern == "long":
+        parts = [cluster(9000, 2e-6), cluster(300, 1e-6)]
+    elif pattern == "mixed":
+        parts = [cluster(int(m), 2e-6) for m in rng.integers(2, 400, 300)] + [cluster(5000, 2e-6)]
+    else:                                      # runs made of exact duplicates: the original index decides
+        parts = [np.repeat(cluster(7, 1e-6), 9, axis=0) for _ in range(200)]
+    pts = np.concatenate([corners, bg] + parts).astype(np.float32)
+    pts = pts[rng.permutation(len(pts))] + np.float32(0.0)
+    o = oracle_lib.build_bvh(pts, 63)
+    runs = np.diff(np.flatnonzero(np.diff(np.concatenate([[-1], (o.sorted_codes >> np.uint64(31)).astype(np.int64), [-2]])) != 0))
+    if pattern in ("long", "mixed"):
+        assert runs.max() > 4096               # the fix-up cannot hold it: the second sort must run
+    elif pattern in ("medium", "tile_edge"):
+        assert 33 < runs.max() <= 2048 + 64
+    bvh = gpu_build(B, pts, 63)
+    assert_build_equal(export_np(bvh), o, pattern)
+    bvh2 = gpu_build(B, pts, 63)               # a second build into fresh buffers: flags and work list start from zero again
+    assert_build_equal(export_np(bvh2), o, pattern + " again")
+
+
 @pytest.mark.parametrize("bits", [30, 63])
 @pytest.mark.parametrize("n", [1, 2, 5, 1000, 10_000])
 def test_all_points_coincident(B, oracle_lib, n, bits):
