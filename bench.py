@@ -72,6 +72,8 @@ def byte_model(n: int, q: int, nnz: int, prim_floats: int, query_floats: int, bi
         "rows_to_csr": (4 + 8) * q + 8 * nnz,            # counts, offsets, every hit read and written once
         "overflow": 4 * q,                               # counts (no row overflows when the capacity holds the largest row)
     }
+    per_kernel["tie_fixup"] = K * n                  # 63-bit two-stage sort: one read of the sorted codes
+    per_kernel["second_sort"] = 0                    # ... and nine kernels that return at once unless a run did not fit a block
     per_kernel["front"] = sum(v for k, v in per_kernel.items() if k in ("init", "bounds", "morton") or k.startswith("sort_pass"))
     build_total = (3 * S + 4 * K + (2 * P - 1) * (K + 4) + 100) * n      # SURVEY.md B_build
     query_total = (2 * Sq + 24) * q + 4 * nnz                            # SURVEY.md B_query
@@ -288,13 +290,16 @@ def run_ours(args) -> dict | None:
         t_c3.record()
 
     small_build = n <= 16384          # bounds + Morton + sort in one launch (csrc/small_build.cu), no memset
-    build_names = ["front", "hierarchy"] if small_build else \
-        ["init", "bounds", "morton"] + [f"sort_pass{p}" for p in range(P)] + ["hierarchy"]
+    two_stage = bits == 63 and not small_build   # 63-bit codes: 4 passes over the upper bits + tie fix-up (csrc/tie_fixup.cu)
+    sort_names = [f"sort_pass{p}" for p in range(4)] + ["tie_fixup", "second_sort"] if two_stage else \
+        [f"sort_pass{p}" for p in range(P)]
+    build_names = ["front", "hierarchy"] if small_build else ["init", "bounds", "morton"] + sort_names + ["hierarchy"]
     query_names = ["order", "collect", "scan", "rows_to_csr", "overflow"]
     names = build_names + query_names
     # kernels of this library per stage when the stages are called one by one (the staged legs) ...
     launches_per_step = {**({"front": 1} if small_build else
-                            {"init": 0, "bounds": 1, "morton": 1, **{f"sort_pass{p}": 1 for p in range(P)}}),
+                            {"init": 0, "bounds": 1, "morton": 1, **{k: 1 for k in sort_names},
+                             **({"tie_fixup": 2, "second_sort": 9} if two_stage else {})}),
                          "hierarchy": 2 if n > 256 else 1, "order": 5 if q > 8192 else 1, "collect": 1,
                          "scan": 3 if q > 4096 else 1, "rows_to_csr": 1, "overflow": 1}
     # ... and in the timed step, where the query is one call: no identity order for q <= 8192, scan + row copy fused for q <= 4096
@@ -316,9 +321,13 @@ def run_ours(args) -> dict | None:
         t = {"init": stage[0].elapsed_time(stage[1]), "bounds": stage[1].elapsed_time(stage[2]),
              "morton": stage[2].elapsed_time(stage[3])}
         prev = stage[3]
-        for p in range(P):
+        for p in range(4 if two_stage else P):
             t[f"sort_pass{p}"] = prev.elapsed_time(stage[4 + p])
             prev = stage[4 + p]
+        if two_stage:   # [8] after the fix-up, [11] after the (normally idle) kernels of the conditional second sort
+            t["tie_fixup"] = stage[7].elapsed_time(stage[8])
+            t["second_sort"] = stage[8].elapsed_time(stage[11])
+            prev = stage[11]
         t["hierarchy"] = prev.elapsed_time(stage[12])
         t["_build_staged"] = stage[0].elapsed_time(stage[12])
         return t

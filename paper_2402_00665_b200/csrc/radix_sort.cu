@@ -297,7 +297,11 @@ __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restr
 #ifndef BVH_SORT_MINBLOCKS
 #define BVH_SORT_MINBLOCKS 4
 #endif
-template <typename KeyT, bool IOTA, bool TOP>
+// COND: a pass of the conditional second sort of a 63-bit build (tie_fixup.cu) -- nothing to do unless *run_if != 0.
+// Such a pass is launched with a small grid whose blocks keep taking tiles (tickets) until none is left, so that the
+// usual case, flag clear, costs a launch of a few hundred blocks whatever n is.  The ordinary pass (COND = false) is
+// one tile per block.
+template <typename KeyT, bool IOTA, bool TOP, bool COND>
 __global__ void __launch_bounds__(kSortThreads, BVH_SORT_MINBLOCKS)
 onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_out, const uint32_t* __restrict__ vals_in,
                      uint32_t* __restrict__ vals_out, const uint32_t* __restrict__ hist, uint32_t* status,
@@ -311,16 +315,30 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_o
   if (tid < 256) s.tile_hist[tid] = 0;
   pdl_wait();
   pdl_trigger();
-  // A pass of the conditional second sort of a 63-bit build (tie_fixup.cu): nothing to do unless the flag is up.  Such a
-  // pass is launched with a small grid whose blocks keep taking tiles (tickets) until none is left, so that the usual
-  // case -- flag clear -- costs a launch of a few hundred blocks whatever n is.
-  if (run_if && *run_if == 0) return;
-  const uint32_t tiles = (uint32_t)((n + TILE - 1) / TILE);
-  while (true) {
+  if (COND) {
+    if (*run_if == 0) return;
+    const uint32_t tiles = (uint32_t)((n + TILE - 1) / TILE);
+    while (true) {
+      if (tid == 0) s.tile = atomicAdd(tile_counter, 1u);
+      __syncthreads();
+      const uint32_t tile = s.tile;
+      if (tile >= tiles) return;
+      const uint32_t tile_base = tile * (uint32_t)TILE;
+      const int valid_in_tile = min(TILE, n - (int)tile_base);
+      if (valid_in_tile == TILE)
+        sort_tile<KeyT, IOTA, true, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, TILE, shift);
+      else
+        sort_tile<KeyT, IOTA, false, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, valid_in_tile,
+                                          shift);
+      __syncthreads();
+      for (int i = tid; i < kSortWarps * kSortChains * 256; i += kSortThreads) (&s.warp_hist[0][0][0])[i] = 0;
+      if (tid < 256) s.tile_hist[tid] = 0;
+      __syncthreads();
+    }
+  } else {
     if (tid == 0) s.tile = atomicAdd(tile_counter, 1u);
     __syncthreads();
     const uint32_t tile = s.tile;
-    if (tile >= tiles) return;
     const uint32_t tile_base = tile * (uint32_t)TILE;
     const int valid_in_tile = min(TILE, n - (int)tile_base);
     if (valid_in_tile == TILE)
@@ -328,28 +346,24 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_o
     else
       sort_tile<KeyT, IOTA, false, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, valid_in_tile,
                                         shift);
-    if (!run_if) return;                // the ordinary pass: one tile per block
-    __syncthreads();
-    for (int i = tid; i < kSortWarps * kSortChains * 256; i += kSortThreads) (&s.warp_hist[0][0][0])[i] = 0;
-    if (tid < 256) s.tile_hist[tid] = 0;
-    __syncthreads();
   }
 }
 
-template <typename KeyT>
-static cudaError_t sort_all(const SortBuffers& B, int n, int passes, cudaStream_t stream, void* const* pass_events, int shift0,
-                            int slot0, const uint32_t* run_if) {
+template <typename KeyT, bool COND>
+static cudaError_t sort_passes(const SortBuffers& B, int n, int passes, cudaStream_t stream, void* const* pass_events, int shift0,
+                               int slot0, const uint32_t* run_if) {
   const int tiles = (n + SortCfg<KeyT>::TILE - 1) / SortCfg<KeyT>::TILE;
   KeyT* keys[2] = {static_cast<KeyT*>(B.keys[0]), static_cast<KeyT*>(B.keys[1])};
   const size_t smem = sizeof(SortSmem<KeyT>);
   // the opt-in to more than 48 KB of dynamic shared memory is a property of the function: set once per process
   static const cudaError_t attr = [&]() {
-    cudaError_t e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, true, false, COND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, false, COND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, true, COND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     return e;
   }();
   if (attr != cudaSuccess) return attr;
+  const int blocks = (COND && tiles > 4 * sm_count()) ? 4 * sm_count() : tiles;   // conditional pass: persistent grid
   for (int p = 0; p < passes; ++p) {
     const int in = p & 1, out = in ^ 1, slot = slot0 + p;     // slot: which histogram / status block / ticket this pass uses
     uint32_t* st = B.status + (size_t)slot * tiles * 256;
@@ -358,20 +372,26 @@ static cudaError_t sort_all(const SortBuffers& B, int n, int passes, cudaStream_
     const uint32_t* vin = B.vals[in];
     const uint32_t* none = nullptr;
     cudaError_t e;
-    const int blocks = (run_if && tiles > 4 * sm_count()) ? 4 * sm_count() : tiles;   // conditional pass: persistent grid
     if (p == 0)
-      e = launch_pdl(onesweep_pass_kernel<KeyT, true, false>, dim3(blocks), dim3(kSortThreads), smem, stream,
+      e = launch_pdl(onesweep_pass_kernel<KeyT, true, false, COND>, dim3(blocks), dim3(kSortThreads), smem, stream,
                  keys[in], keys[out], none, vout, B.hist + slot * 256, st, B.tile_counters + slot, n, shift, run_if);
     else if (p == passes - 1 && sizeof(KeyT) == 4)   // (64-bit codes: the top digit of neighbouring keys is rarely shared; ballots)
-      e = launch_pdl(onesweep_pass_kernel<KeyT, false, true>, dim3(blocks), dim3(kSortThreads), smem, stream,
+      e = launch_pdl(onesweep_pass_kernel<KeyT, false, true, COND>, dim3(blocks), dim3(kSortThreads), smem, stream,
                  keys[in], keys[out], vin, vout, B.hist + slot * 256, st, B.tile_counters + slot, n, shift, run_if);
     else
-      e = launch_pdl(onesweep_pass_kernel<KeyT, false, false>, dim3(blocks), dim3(kSortThreads), smem, stream,
+      e = launch_pdl(onesweep_pass_kernel<KeyT, false, false, COND>, dim3(blocks), dim3(kSortThreads), smem, stream,
                  keys[in], keys[out], vin, vout, B.hist + slot * 256, st, B.tile_counters + slot, n, shift, run_if);
     if (e != cudaSuccess) return e;
     if (pass_events && pass_events[p]) cudaEventRecord(static_cast<cudaEvent_t>(pass_events[p]), stream);
   }
   return cudaSuccess;
+}
+
+template <typename KeyT>
+static cudaError_t sort_all(const SortBuffers& B, int n, int passes, cudaStream_t stream, void* const* pass_events, int shift0,
+                            int slot0, const uint32_t* run_if) {
+  if (run_if) return sort_passes<KeyT, true>(B, n, passes, stream, pass_events, shift0, slot0, run_if);
+  return sort_passes<KeyT, false>(B, n, passes, stream, pass_events, shift0, slot0, run_if);
 }
 
 SortBuffers sort_buffers(void* scratch, const ScratchLayout& L) {
