@@ -17,10 +17,11 @@
 //    divergence, and in the fill pass the hits of the row leave as one contiguous run of stores
 //    (warp-cooperative CSR output; ballot + popc give each hit its slot).  Every leaf of the subtree is
 //    still tested, in ascending order, so the result and its order are those of Algorithm 1.
-//  * Scheduling.  The grid is persistent: 148 SMs x CTAs per SM, and CTA b works on query chunk
-//    ((k*148 + b%148) * R + b/148) at its step k, so that at any time the threads of an SM serve consecutive
-//    positions of the (Morton-ordered) query list: their node reads overlap and stay in that SM's L1
-//    (data divergence).  The block-to-SM mapping is only a locality assumption.
+//  * Scheduling.  One block per chunk of kTravThreads consecutive positions of the (Morton-ordered) query list; the
+//    hardware hands the chunks out in order as blocks retire, so the blocks that run at the same time serve
+//    neighbouring queries -- their node reads overlap in L1 / L2 (data divergence) -- and expensive
+//    chunks do not hold up a static share of the list.  A batch too small to fill the GPU is spread: one query per
+//    2^s lanes (launch_traverse_kind).
 //
 // Predicates (D8): sphere {c, r} -- squared distance from c to the box, fp32 round-to-nearest with
 // explicit intrinsics (no FMA contraction): d = max(max(lo - c, c - hi), 0) per axis,
