@@ -267,6 +267,9 @@ struct LeafRec<false> {
 #ifndef BVH_SCAN_UNROLL
 #define BVH_SCAN_UNROLL 4
 #endif
+#ifndef BVH_SCAN_SKIP_EMPTY
+#define BVH_SCAN_SKIP_EMPTY 0
+#endif
 
 // What a pass does with a leaf that satisfies the predicate (Alg. 1 L5, "Store the result or perform an operation"):
 //   kModeCount    count it (K6);
@@ -505,6 +508,9 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
             if (c + 32 * u < end) leaf[u].load(leaves, c + 32 * u);
 #pragma unroll
           for (int u = 0; u < U; ++u) {
+#if BVH_SCAN_SKIP_EMPTY
+            if (u > 0 && c - lane + 32 * u >= end) break;   // (warp-uniform) no leaf of the range is left for this step
+#endif
             const bool inside = c + 32 * u < end;
             const bool sat = leaf[u].hit(oq);              // evaluated on every lane (no branch); masked below
             const bool hit = inside & sat;                 // L3-5 on leaf c + 32u
