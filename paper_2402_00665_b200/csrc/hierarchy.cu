@@ -18,6 +18,10 @@ namespace bvh {
 #ifndef BVH_HIER_MINBLOCKS
 #define BVH_HIER_MINBLOCKS 12
 #endif
+#ifndef BVH_PHASE0_MAX_ROUNDS
+#define BVH_PHASE0_MAX_ROUNDS 3
+#endif
+constexpr int kPhase0MaxRounds = BVH_PHASE0_MAX_ROUNDS;   // lockstep rounds per group before the rest is left to phase 1 (>= 31: all)
 constexpr int kHierThreads = 128;               // threads of a level-1 block
 constexpr int kHierWindow = BVH_HIER_WINDOW;    // leaves of a level-1 window (one block); a multiple of kHierThreads
 static_assert(kHierWindow % kHierThreads == 0, "a level-1 window is a whole number of 32-leaf groups per warp");
@@ -528,7 +532,8 @@ hierarchy_local_kernel(const float* __restrict__ prim, const KeyT* __restrict__ 
 
     // ---- phase 0: rendezvous inside the group, in lockstep ----
     bool active = valid && n > 1;                             // G11: a single leaf has no parent
-    while (true) {
+#pragma unroll
+    for (int round = 0; round < kPhase0MaxRounds; ++round) {
       const bool is_left = delta_right < delta_left;          // L10
       const int partner = range_right + 1 - w0;               // lane of leaf r+1
       const bool look = active && is_left && partner < 32;
