@@ -18,6 +18,9 @@ namespace bvh {
 #ifndef BVH_HIER_MINBLOCKS
 #define BVH_HIER_MINBLOCKS 12
 #endif
+#ifndef BVH_HIER_UNROLL_GROUPS
+#define BVH_HIER_UNROLL_GROUPS 0
+#endif
 #ifndef BVH_PHASE0_MAX_ROUNDS
 #define BVH_PHASE0_MAX_ROUNDS 3
 #endif
@@ -123,7 +126,7 @@ struct ItemArrays {
   RT* l;         // first leaf of the item in this slot, minus `base` (level 1: offsets into the window, 16 bits)
   RT* r;         // last leaf, minus `base`
   int base;
-  float* box;    // box[c * stride + slot], c = 0..5 (min.xyz, max.xyz)
+  float2* box;   // box[c * stride + slot] = {min, max} of axis c = 0..2 (one 64-bit shared-memory access per axis)
   int stride;
   int* store;    // Algorithm 4's `store`, one entry per boundary (e | e+1), by item index: -1 empty, >= 0 first arrival, -2 both
 };
@@ -157,8 +160,9 @@ __device__ __forceinline__ ClimbEnd climb_from_item(int e, int M, const ItemArra
   float lo[3], hi[3];
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
-    lo[c] = A.box[c * A.stride + se];
-    hi[c] = A.box[(3 + c) * A.stride + se];
+    const float2 v = A.box[c * A.stride + se];
+    lo[c] = v.x;
+    hi[c] = v.y;
   }
   int fin = -1;
   while (true) {
@@ -188,8 +192,9 @@ __device__ __forceinline__ ClimbEnd climb_from_item(int e, int M, const ItemArra
     __threadfence_block();                                            // the sibling's box was written before its CAS
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      lo[c] = fminf(lo[c], A.box[c * A.stride + ssib]);
-      hi[c] = fmaxf(hi[c], A.box[(3 + c) * A.stride + ssib]);
+      const float2 v = A.box[c * A.stride + ssib];
+      lo[c] = fminf(lo[c], v.x);
+      hi[c] = fmaxf(hi[c], v.y);
     }
     const int q = (delta_right < delta_left) ? range_right : range_left;     // L20: Karras index
     const int left = (range_left == p) ? leaf_base + p : p;                  // L21 (reading G2)
@@ -202,8 +207,7 @@ __device__ __forceinline__ ClimbEnd climb_from_item(int e, int M, const ItemArra
     if (q == 0) return ClimbEnd{range_left, range_right, -2};                // L28: the root
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      A.box[c * A.stride + sa] = lo[c];
-      A.box[(3 + c) * A.stride + sa] = hi[c];
+      A.box[c * A.stride + sa] = make_float2(lo[c], hi[c]);
     }
     __threadfence_block();
   }
@@ -239,7 +243,7 @@ template <typename D>
 struct LocalSmem {
   D delta[kHierWindow + 2];      // delta[k] = delta*(c0 - 1 + k)
   int store[kHierWindow];
-  float box[6 * kHierWindow];
+  float2 box[3 * kHierWindow];
   uint16_t l[kHierWindow], r[kHierWindow];   // offsets from the window's first leaf
 };
 static_assert(kHierWindow <= 65536, "level-1 item ranges are kept as 16-bit offsets");
@@ -247,7 +251,7 @@ template <typename D>
 struct MergeSmem {
   D bd[kMergeMaxItems + 1], nd[kMergeMaxItems + 1];
   int l[kMergeMaxItems], r[kMergeMaxItems], store[kMergeMaxItems];
-  float box[6 * kMergeMaxItems];
+  float2 box[3 * kMergeMaxItems];
   int pref[kMergeFanMax + 1];
 };
 // Windows of every level (level 1 first) and where each level's hand-over segments and arrival counters start.
@@ -363,8 +367,7 @@ __device__ __forceinline__ void merge_window(MergeSmem<typename Delta<KeyT>::T>&
           load_box_cg(nodes_base, n, leaf_kind, carried, lo, hi);
 #pragma unroll
           for (int c = 0; c < 3; ++c) {
-            S.box[c * MAXI + e] = lo[c];
-            S.box[(3 + c) * MAXI + e] = hi[c];
+            S.box[c * MAXI + e] = make_float2(lo[c], hi[c]);
           }
         }
       }
@@ -431,7 +434,7 @@ hierarchy_local_kernel(const float* __restrict__ prim, const KeyT* __restrict__ 
   uint16_t* const s_l = smem.l;
   uint16_t* const s_r = smem.r;
   int* const s_store = smem.store;
-  float* const s_box = smem.box;
+  float2* const s_box = smem.box;
 
   Node* nodes = reinterpret_cast<Node*>(nodes_base + kNodesHeaderBytes);   // internal records, by Karras index
   char* leaves = nodes_base + leaf_offset_bytes(n);
@@ -495,7 +498,11 @@ hierarchy_local_kernel(const float* __restrict__ prim, const KeyT* __restrict__ 
 
   int wcount = 0;                                              // items this warp has staged (uniform in the warp)
   const uint32_t lt_mask = (1u << lane) - 1u;
+#if BVH_HIER_UNROLL_GROUPS
+#pragma unroll
+#else
 #pragma unroll 1
+#endif
   for (int g = 0; g < G; ++g) {
     const int w0 = wl0 + g * 32;                               // first leaf of the group
     const int i = w0 + lane;
@@ -582,8 +589,7 @@ hierarchy_local_kernel(const float* __restrict__ prim, const KeyT* __restrict__ 
       s_r[slot] = (uint16_t)(range_right - c0);
 #pragma unroll
       for (int a = 0; a < 3; ++a) {
-        s_box[a * W + slot] = lo[a];
-        s_box[(3 + a) * W + slot] = hi[a];
+        s_box[a * W + slot] = make_float2(lo[a], hi[a]);
       }
     }
     wcount += __popc(am);
