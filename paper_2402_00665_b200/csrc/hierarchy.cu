@@ -18,6 +18,13 @@ namespace bvh {
 #ifndef BVH_HIER_MINBLOCKS
 #define BVH_HIER_MINBLOCKS 12
 #endif
+#ifndef BVH_HIER_SLOT_TABLE
+#define BVH_HIER_SLOT_TABLE 0
+#endif
+template <bool SMALL>
+struct SlotType { using T = uint8_t; };
+template <>
+struct SlotType<false> { using T = uint16_t; };
 #ifndef BVH_HIER_UNROLL_GROUPS
 #define BVH_HIER_UNROLL_GROUPS 0
 #endif
@@ -140,6 +147,13 @@ struct StagedSlots {
   __device__ __forceinline__ int slot(int e) const {
     return e + (e >= b2 ? (e >= b3 ? o3 : o2) : (e >= b1 ? o1 : o0));
   }
+};
+// ... looked up in a table the block fills once (one shared-memory load instead of the compare chain, which the climb
+// needs up to three times per merge)
+template <typename ST>
+struct TableSlots {
+  const ST* table;
+  __device__ __forceinline__ int slot(int e) const { return (int)table[e]; }
 };
 // Where the subtree that started as one item stopped: its leaf range, and why: fin = -2 it became the root, -1 its
 // parent straddles the window, k >= 0 it arrived first at boundary k.
@@ -610,11 +624,24 @@ hierarchy_local_kernel(const float* __restrict__ prim, const KeyT* __restrict__ 
   const int M = map.b3 + s_wcount[3];
   const ItemArrays<uint16_t> A{s_l, s_r, c0, s_box, W, s_store};
   ClimbEnd end[G];
+#if BVH_HIER_SLOT_TABLE
+  using SlotT = typename SlotType<(W <= 256)>::T;
+  __shared__ SlotT s_slot[W];
+#pragma unroll
+  for (int j = 0; j < G; ++j) {
+    const int e = tid + j * T;
+    if (e < M) s_slot[e] = (SlotT)map.slot(e);
+  }
+  __syncthreads();
+  const TableSlots<SlotT> slots{s_slot};
+#else
+  const StagedSlots& slots = map;
+#endif
 #pragma unroll
   for (int j = 0; j < G; ++j) {
     end[j] = ClimbEnd{0, 0, -2};
     const int e = tid + j * T;
-    if (e < M) end[j] = climb_from_item<D>(e, M, A, DeltaByLeaf<D>{s_delta, c0}, map, nodes, n);
+    if (e < M) end[j] = climb_from_item<D>(e, M, A, DeltaByLeaf<D>{s_delta, c0}, slots, nodes, n);
   }
   __syncthreads();
 
