@@ -481,14 +481,16 @@ hierarchy_local_kernel(const float* __restrict__ prim, const KeyT* __restrict__ 
     const int i = wl0 + g * 32 + lane;
     orig[g] = (i < n) ? __ldcs(perm + i) : 0u;
   }
+  // delta* of the warp's own leaves, plus the one before and the one after them: everything phase 0 of this warp reads
+  // (the neighbouring warps write the same two values), so the warps need no block barrier before phase 0
 #pragma unroll
-  for (int j = 0; j < G; ++j) {
-    const int k = tid + j * T;                                 // window slot; coalesced
+  for (int g = 0; g < G; ++g) {
+    const int k = warp * PER_WARP + g * 32 + lane;             // window slot of this thread's leaf g
     s_delta[k + 1] = delta_star<KeyT>(codes, c0 + k, n);
-    s_store[k] = kInvalid;                                     // L1
+    s_store[k] = kInvalid;                                     // L1 (read in phase 1, after the barriers below)
   }
-  if (tid == 0) s_delta[0] = delta_star<KeyT>(codes, c0 - 1, n);
-  if (tid == 1) s_delta[W + 1] = delta_star<KeyT>(codes, c0 + W, n);
+  if (lane == 0) s_delta[warp * PER_WARP] = delta_star<KeyT>(codes, wl0 - 1, n);
+  if (lane == 1) s_delta[(warp + 1) * PER_WARP + 1] = delta_star<KeyT>(codes, wl0 + PER_WARP, n);
   float plo[G][3], phi[G][IS_BOX ? 3 : 1];
 #pragma unroll
   for (int g = 0; g < G; ++g) {
@@ -508,7 +510,7 @@ hierarchy_local_kernel(const float* __restrict__ prim, const KeyT* __restrict__ 
       }
     }
   }
-  __syncthreads();
+  __syncwarp();
 
   int wcount = 0;                                              // items this warp has staged (uniform in the warp)
   const uint32_t lt_mask = (1u << lane) - 1u;
