@@ -40,12 +40,23 @@ namespace bvh {
 #define BVH_TRAV_WARPS_PER_SM 32
 #endif
 #ifndef BVH_SCAN_LEAVES
-#define BVH_SCAN_LEAVES 128
+#define BVH_SCAN_LEAVES 96
+#endif
+#ifndef BVH_SCAN_LEAVES_SPARSE
+#define BVH_SCAN_LEAVES_SPARSE 64
 #endif
 constexpr int kTravThreads = BVH_TRAV_THREADS;         // queries of a block (one per thread)
 static_assert(kTravThreads % 32 == 0 && kTravThreads >= 32 && kTravThreads <= 1024, "whole warps");
 constexpr int kTravCtasPerSm = BVH_TRAV_WARPS_PER_SM * 32 / kTravThreads;   // resident blocks asked of the register allocator
+// Largest subtree (in leaves) whose leaves the warp scans instead of walking it; the scan loop is unrolled to take such
+// a range in ONE iteration (threshold / 32 loads in flight per lane).  Measured on B200 (profiles/r02_experiments.md):
+// 96 for batches with long rows (C3: 591 hits per query), 64 where rows are short (C2, C4, C5: 3 to 31 hits per
+// query: fewer leaves tested in vain per hit) -- which the single-pass call knows from its row capacity.
 constexpr int kScanLeaves = BVH_SCAN_LEAVES;
+constexpr int kScanLeavesSparse = BVH_SCAN_LEAVES_SPARSE;
+constexpr int kScanLeavesSpread = 128;                 // small batches, one query per warp: scanning is cheap, walking is latency
+constexpr int kSparseRowCap = 64;                      // collect with rows of at most this many entries: the sparse threshold
+static_assert(kScanLeaves % 32 == 0 && kScanLeavesSparse % 32 == 0 && kScanLeavesSparse <= kScanLeaves, "whole warp steps");
 
 struct NodeRec {
   float lox, loy, loz;
@@ -264,9 +275,6 @@ struct LeafRec<false> {
   __device__ __forceinline__ bool cand(const Query& q, float& key) const { return q.cand_box(r.lox, r.loy, r.loz, r.hix, r.hiy, r.hiz, key); }
 };
 
-#ifndef BVH_SCAN_UNROLL
-#define BVH_SCAN_UNROLL 4
-#endif
 #ifndef BVH_SCAN_SKIP_EMPTY
 #define BVH_SCAN_SKIP_EMPTY 0
 #endif
@@ -352,11 +360,11 @@ struct TravSmem {
 
 __host__ __device__ constexpr bool mode_stores(int mode) { return mode == kModeFill || mode == kModeCollect; }
 
-template <typename Query, int MODE, bool POINT_LEAF, bool SPREAD>
+template <typename Query, int MODE, bool POINT_LEAF, bool SPREAD, int SCAN>
 __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Query, mode_stores(MODE)>& S) {
   constexpr bool STORE = mode_stores(MODE);
   constexpr bool REDUCE = MODE == kModeReduce, ANY = MODE == kModeAny;
-  constexpr int U = POINT_LEAF ? BVH_SCAN_UNROLL : (BVH_SCAN_UNROLL > 2 ? 2 : BVH_SCAN_UNROLL);   // leaf loads in flight per lane
+  constexpr int U = POINT_LEAF ? SCAN / 32 : (SCAN / 32 > 2 ? 2 : SCAN / 32);   // leaf loads in flight per lane
   float* const s_query = S.query;
   int2* const s_range = S.range;
   int32_t** const s_row = S.row;
@@ -597,7 +605,7 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
           const int next_first = rope < 0 ? n : (rope >= leaf_base ? rope - leaf_base : rope);
           int next = rope;                                   // L10: N_skip
           if (query.hit_box(rec.lox, rec.loy, rec.loz, rec.hix, rec.hiy, rec.hiz)) {   // L3
-            if (next_first - first <= kScanLeaves) {         // small subtree: post its leaves, continue after it
+            if (next_first - first <= SCAN) {                // small subtree: post its leaves, continue after it
               s_range[threadIdx.x] = make_int2(first, next_first);
               post = true;
             } else if (try_contain && next_first - first > kContainMinLeaves &&
@@ -636,7 +644,7 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
 // header tells whether `nodes` holds a finished hierarchy over n primitives at all: if not (never built, built for
 // another n, overwritten), nothing is traversed -- counts come out as 0, nothing is stored -- instead of following
 // garbage indices.
-template <typename Query, int MODE, bool SPREAD>
+template <typename Query, int MODE, bool SPREAD, int SCAN = kScanLeaves>
 __global__ void __launch_bounds__(kTravThreads, Query::kCtasPerSm) traverse_kernel(const TraverseArgs A) {
   if (SPREAD) {      // small batches are launched with programmatic stream serialisation
     pdl_wait();      // the previous kernel of the stream has completed
@@ -653,9 +661,9 @@ __global__ void __launch_bounds__(kTravThreads, Query::kCtasPerSm) traverse_kern
   }
   __shared__ TravSmem<Query, mode_stores(MODE)> S;
   if (h->leaf_kind == kLeafPoints)
-    traverse_body<Query, MODE, true, SPREAD>(A, S);
+    traverse_body<Query, MODE, true, SPREAD, SCAN>(A, S);
   else
-    traverse_body<Query, MODE, false, SPREAD>(A, S);
+    traverse_body<Query, MODE, false, SPREAD, SCAN>(A, S);
 }
 
 // Small batches.  With one query per lane a warp serves its 32 queries' leaf scans one after the other, each a chain of
@@ -675,11 +683,11 @@ static cudaError_t launch_traverse_kind(TraverseArgs A, int mode, cudaStream_t s
   const dim3 g((unsigned)chunks), b(kTravThreads);
   if (A.spread_log2 > 0) {
     // small batch: bound by the latency of its dependent launches -> programmatic dependent launch
-    if (mode == kModeCount) return launch_pdl(traverse_kernel<Query, kModeCount, true>, g, b, 0, stream, A);
-    if (mode == kModeFill) return launch_pdl(traverse_kernel<Query, kModeFill, true>, g, b, 0, stream, A);
-    if (mode == kModeCollect) return launch_pdl(traverse_kernel<Query, kModeCollect, true>, g, b, 0, stream, A);
-    if (mode == kModeAny) return launch_pdl(traverse_kernel<Query, kModeAny, true>, g, b, 0, stream, A);
-    if constexpr (Query::kHasKey) return launch_pdl(traverse_kernel<Query, kModeReduce, true>, g, b, 0, stream, A);
+    if (mode == kModeCount) return launch_pdl(traverse_kernel<Query, kModeCount, true, kScanLeavesSpread>, g, b, 0, stream, A);
+    if (mode == kModeFill) return launch_pdl(traverse_kernel<Query, kModeFill, true, kScanLeavesSpread>, g, b, 0, stream, A);
+    if (mode == kModeCollect) return launch_pdl(traverse_kernel<Query, kModeCollect, true, kScanLeavesSpread>, g, b, 0, stream, A);
+    if (mode == kModeAny) return launch_pdl(traverse_kernel<Query, kModeAny, true, kScanLeavesSpread>, g, b, 0, stream, A);
+    if constexpr (Query::kHasKey) return launch_pdl(traverse_kernel<Query, kModeReduce, true, kScanLeavesSpread>, g, b, 0, stream, A);
     return cudaErrorInvalidValue;
   }
   // a batch that fills the GPU: plain stream order (measured on C3: with the attribute the one-call query is 1.5 % slower)
@@ -687,6 +695,8 @@ static cudaError_t launch_traverse_kind(TraverseArgs A, int mode, cudaStream_t s
     traverse_kernel<Query, kModeCount, false><<<g, b, 0, stream>>>(A);
   else if (mode == kModeFill)
     traverse_kernel<Query, kModeFill, false><<<g, b, 0, stream>>>(A);
+  else if (mode == kModeCollect && A.cap <= kSparseRowCap)
+    traverse_kernel<Query, kModeCollect, false, kScanLeavesSparse><<<g, b, 0, stream>>>(A);
   else if (mode == kModeCollect)
     traverse_kernel<Query, kModeCollect, false><<<g, b, 0, stream>>>(A);
   else if (mode == kModeAny)
