@@ -137,6 +137,36 @@ def test_small_build_boxes_and_ties(B, oracle_lib, n, bits):
     assert len(np.unique(o.sorted_codes)) <= 125
 
 
+@pytest.mark.parametrize("frame", ["unit", "odd", "tiny", "huge", "flat"])
+def test_30bit_cells_on_and_next_to_cell_boundaries(B, oracle_lib, frame):
+    """30-bit codes where D2's arithmetic is most fragile: coordinates exactly on cell boundaries, one and two ulps to
+    either side, and random ones, in frames whose extent is a power of two, an odd number, tiny, huge, or zero on one
+    axis: every code must be the oracle's.  (Written for a division-free quantisation that was measured and not kept:
+    profiles/r02_experiments.md; it pins the kernel's rounding all the same.)"""
+    rng = np.random.default_rng(abs(hash(frame)) % (1 << 31))
+    lo, hi = {"unit": (0.0, 1.0), "odd": (0.1, 0.7), "tiny": (1.0, 1.0 + 3e-5), "huge": (-3.0e7, 5.0e8),
+              "flat": (0.25, 0.8)}[frame]
+    lo32, hi32 = np.float32(lo), np.float32(hi)
+    e = np.float32(hi32 - lo32)
+    k = rng.integers(0, 1025, size=(30_000, 3))
+    on = (lo32 + (k.astype(np.float32) / np.float32(1024)) * e).astype(np.float32)       # on (or within an ulp of) a boundary
+    parts = [on]
+    for steps in (1, 2):
+        up, dn = on.copy(), on.copy()
+        for _ in range(steps):
+            up = np.nextafter(up, np.float32(np.inf)).astype(np.float32)
+            dn = np.nextafter(dn, np.float32(-np.inf)).astype(np.float32)
+        parts += [up, dn]
+    parts.append((lo32 + rng.random((60_000, 3)).astype(np.float32) * e).astype(np.float32))
+    pts = np.clip(np.concatenate(parts), lo32, hi32).astype(np.float32)
+    pts = np.concatenate([np.array([[lo32] * 3, [hi32] * 3], np.float32), pts]) + np.float32(0.0)
+    if frame == "flat":
+        pts[:, 1] = np.float32(0.5)                      # zero extent on y: t = 0 there (G7)
+    o = oracle_lib.build_bvh(pts, 30)
+    e_gpu = export_np(gpu_build(B, pts, 30))
+    assert_build_equal(e_gpu, o, frame)
+
+
 @pytest.mark.parametrize("pattern", ["pairs", "short", "serial_limit", "medium", "tile_edge", "long", "mixed", "coincident_blocks"])
 def test_two_stage_sort_of_63bit_codes(B, oracle_lib, pattern):
     """63-bit builds sort by the upper 32 bits of the code and then order every run of equal upper bits by the lower 31
