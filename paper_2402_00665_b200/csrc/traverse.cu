@@ -11,7 +11,7 @@
 //    leaf records [first, last], and the walk knows both bounds for free: the node a skip-connection leads to
 //    starts right after the subtree it skips (Algorithm 2: N_skip is node range_right + 1),
 //    and `first` is inherited on the way down (a left child starts where its parent starts).  When a node that
-//    satisfies the predicate covers at most kScanLeaves leaves, the lane does not walk that small subtree
+//    satisfies the predicate covers at most SCAN leaves (96; 64 / 128 in two cases: kScanLeaves below), the lane does not walk that small subtree
 //    node by node: it posts the range, and the warp tests those leaves together, lane l taking leaf
 //    first + l -- one coalesced load of consecutive leaf records instead of 32 scattered ones, no
 //    divergence, and in the fill pass the hits of the row leave as one contiguous run of stores
@@ -339,7 +339,8 @@ constexpr int kFillStage = BVH_FILL_STAGE;        // 0: store hits as they come;
 constexpr bool kContainment = BVH_CONTAINMENT != 0;
 constexpr int kContainMinLeaves = BVH_CONTAIN_MIN_LEAVES;
 constexpr int kStageInts = 8;                      // one sector
-constexpr int kRangeBufInts = kScanLeaves + kStageInts;
+constexpr int kScanLeavesMax = kScanLeaves > kScanLeavesSpread ? kScanLeaves : kScanLeavesSpread;
+constexpr int kRangeBufInts = kScanLeavesMax + kStageInts;
 
 __device__ __forceinline__ void store_sector(int32_t* p, const int* v) {   // 32-byte aligned: one full sector
   asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]),
