@@ -62,6 +62,11 @@ int bvh_sizes(int64_t n, int morton_bits, size_t* node_bytes, size_t* scratch_by
  *   4. one bottom-up pass from the leaves that merges ranges through ATOMICCAS on `store`, numbers
  *   each parent with its Karras index q, writes its left child and
  *   skip-connection (Alg. 4 L21-26, Algorithm 2) and the union of its children's boxes (G10).
+ * How step 3 is organised does not change its result (the stable order by (code, index) is unique): 30-bit codes take
+ * four one-sweep passes; 63-bit codes four passes over the upper 32 bits, then every run of equal upper bits is
+ * ordered by the lower 31 (a conditional eight-pass sort behind a device flag covers runs too long for a block); for
+ * n <= 16384 steps 1-3 are one launch of a thread-block cluster.  The sorted codes and the permutation are left in
+ * `scratch` for bvh_export.
  * xyz: n*3 floats (points; a point is the box min = max = point).  minmax: n*6 floats
  * {min.xyz, max.xyz}.  n = 0 is valid and enqueues nothing.  Output: `nodes` (node_bytes). */
 int bvh_build_points(const float* xyz, int64_t n, int morton_bits, void* nodes, void* scratch,
@@ -73,7 +78,8 @@ int bvh_build_boxes(const float* minmax, int64_t n, int morton_bits, void* nodes
  * stage_events[k] (a cudaEvent_t created by the caller, passed as void*) on `stream` -- recording is
  * asynchronous, nothing is created or synchronised.  NULL entries are skipped.  Stages:
  *   [0] start  [1] scratch initialised  [2] scene bounds  [3] Morton codes + digit histograms
- *   [4+p] sort pass p (p < 4 for 30-bit, p < 8 for 63-bit)  [12] bottom-up pass (Algorithm 4)
+ *   [4+p] sort pass p (30-bit: p < 4.  63-bit: [4..7] the four passes over the upper bits, [8] the tie fix-up,
+ *   [9..11] recorded together after the kernels of the conditional second sort)  [12] bottom-up pass (Algorithm 4)
  * A small build (n <= 16384) runs bounds, Morton codes and the whole sort as ONE launch and initialises no scratch: only
  * [0], the event of the last sort pass ([7] or [11]) and [12] are recorded then.
  * stage_events must hold BVH_NUM_STAGE_EVENTS entries.  prim_is_box: 0 = xyz points, 1 = minmax boxes. */
