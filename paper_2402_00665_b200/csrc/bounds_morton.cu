@@ -150,14 +150,13 @@ __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __r
                                                                 const Header* __restrict__ header,
                                                                 const NodesHeader* __restrict__ root,
                                                                 KeyT* __restrict__ codes, uint32_t* __restrict__ hist,
-                                                                int shift0, const uint32_t* __restrict__ run_if) {
-  // shift0: the histograms are those of the PASSES 8-bit digits from bit shift0 up.  run_if (optional): the kernel is
-  // part of the conditional second sort of a 63-bit build (tie_fixup.cu) and does nothing unless *run_if != 0.
+                                                                int shift0) {
+  // shift0: the histograms are those of the PASSES 8-bit digits from bit shift0 up (63-bit codes are sorted by their
+  // upper 32 bits first: tie_fixup.cu).
   __shared__ uint32_t s_hist[PASSES * 256];
   for (int i = threadIdx.x; i < PASSES * 256; i += kMortonThreads) s_hist[i] = 0;
   pdl_wait();
   pdl_trigger();
-  if (run_if && *run_if == 0) return;
   float scene[6];
   if (FROM_ROOT) {
 #pragma unroll
@@ -257,31 +256,31 @@ static unsigned morton_grid(int n, int per_thread = 1) {
 }
 
 cudaError_t launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
-                          uint32_t* hist, cudaStream_t stream, int passes, int shift0, const uint32_t* run_if) {
+                          uint32_t* hist, cudaStream_t stream, int passes, int shift0) {
   const unsigned g = morton_grid(n, is_box ? 2 : 4);
   const dim3 G(g), T(kMortonThreads);
   const NodesHeader* none = nullptr;
   if (morton_bits == 30) {
-    if (is_box) return launch_pdl(morton_kernel<uint32_t, 4, 6, false>, G, T, 0, stream, prim, n, header, none, (uint32_t*)codes, hist, shift0, run_if);
-    return launch_pdl(morton_kernel<uint32_t, 4, 3, false>, G, T, 0, stream, prim, n, header, none, (uint32_t*)codes, hist, shift0, run_if);
+    if (is_box) return launch_pdl(morton_kernel<uint32_t, 4, 6, false>, G, T, 0, stream, prim, n, header, none, (uint32_t*)codes, hist, shift0);
+    return launch_pdl(morton_kernel<uint32_t, 4, 3, false>, G, T, 0, stream, prim, n, header, none, (uint32_t*)codes, hist, shift0);
   }
   if (passes == 4) {   // 63-bit codes sorted by their upper 32 bits first (tie_fixup.cu)
-    if (is_box) return launch_pdl(morton_kernel<uint64_t, 4, 6, false>, G, T, 0, stream, prim, n, header, none, (uint64_t*)codes, hist, shift0, run_if);
-    return launch_pdl(morton_kernel<uint64_t, 4, 3, false>, G, T, 0, stream, prim, n, header, none, (uint64_t*)codes, hist, shift0, run_if);
+    if (is_box) return launch_pdl(morton_kernel<uint64_t, 4, 6, false>, G, T, 0, stream, prim, n, header, none, (uint64_t*)codes, hist, shift0);
+    return launch_pdl(morton_kernel<uint64_t, 4, 3, false>, G, T, 0, stream, prim, n, header, none, (uint64_t*)codes, hist, shift0);
   }
-  if (is_box) return launch_pdl(morton_kernel<uint64_t, 8, 6, false>, G, T, 0, stream, prim, n, header, none, (uint64_t*)codes, hist, shift0, run_if);
-  return launch_pdl(morton_kernel<uint64_t, 8, 3, false>, G, T, 0, stream, prim, n, header, none, (uint64_t*)codes, hist, shift0, run_if);
+  if (is_box) return launch_pdl(morton_kernel<uint64_t, 8, 6, false>, G, T, 0, stream, prim, n, header, none, (uint64_t*)codes, hist, shift0);
+  return launch_pdl(morton_kernel<uint64_t, 8, 3, false>, G, T, 0, stream, prim, n, header, none, (uint64_t*)codes, hist, shift0);
 }
 
 cudaError_t launch_query_morton(const float* queries, int q, int kind, const NodesHeader* root, uint32_t* codes, uint32_t* hist,
                          cudaStream_t stream) {
   const unsigned g = morton_grid(q);
   if (kind == 0)
-    return launch_pdl(morton_kernel<uint32_t, 4, 4, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, 0, nullptr);
+    return launch_pdl(morton_kernel<uint32_t, 4, 4, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, 0);
   else if (kind == 2)
-    return launch_pdl(morton_kernel<uint32_t, 4, 8, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, 0, nullptr);
+    return launch_pdl(morton_kernel<uint32_t, 4, 8, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, 0);
   else
-    return launch_pdl(morton_kernel<uint32_t, 4, 6, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, 0, nullptr);
+    return launch_pdl(morton_kernel<uint32_t, 4, 6, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, 0);
 }
 
 }  // namespace bvh

@@ -184,9 +184,9 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
         return BVH_ERR_CUDA;
     } else {
       // 63-bit codes (tie_fixup.cu): four passes over the upper 32 bits, then every run of equal upper bits ordered by the
-      // lower 31 in shared memory.  Should a run not fit a block, the fix-up raises header->sort_fallback and the plain
-      // eight-pass sort below redoes the order from fresh codes; its nine kernels are enqueued in any case (nothing here
-      // may read the flag back) and return at once while the flag is clear.
+      // lower 31 in shared memory.  Should a run not fit a block, the fix-up raises header->sort_fallback and eight more
+      // passes over all 63 bits redo the order; they are one cooperative launch, enqueued in any case (nothing here may
+      // read the flag back), that returns at once while the flag is clear.
       const SortBuffers B = sort_buffers(scratch, L);
       if (launch_morton(prim, (int)n, is_box, morton_bits, header, base + L.keys[0], hist, stream, 4, 31) != cudaSuccess) return BVH_ERR_CUDA;
       mark(3);
@@ -196,10 +196,7 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
                            stream) != cudaSuccess)
         return BVH_ERR_CUDA;
       mark(8);
-      if (launch_morton(prim, (int)n, is_box, morton_bits, header, base + L.keys[0], hist + 4 * 256, stream, 8, 0,
-                        &header->sort_fallback) != cudaSuccess)
-        return BVH_ERR_CUDA;
-      if (launch_sort(B, L.key_bytes, 8, (int)n, stream, nullptr, 0, 4, &header->sort_fallback) != cudaSuccess) return BVH_ERR_CUDA;
+      if (launch_second_sort(B, 8, (int)n, 4, &header->sort_fallback, stream) != cudaSuccess) return BVH_ERR_CUDA;
       mark(9);
       mark(10);
       mark(11);

@@ -145,9 +145,9 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
 // K1: scene bounds.  is_box: prim is n*6 floats, else n*3.
 cudaError_t launch_scene_bounds(const float* prim, int n, bool is_box, Header* header, cudaStream_t stream);
 // K2: Morton codes + the digit histograms of every sort pass.
-// passes / shift0: histograms of `passes` 8-bit digits from bit shift0 up.  run_if: see tie_fixup.cu.
+// passes / shift0: histograms of `passes` 8-bit digits from bit shift0 up.
 cudaError_t launch_morton(const float* prim, int n, bool is_box, int morton_bits, const Header* header, void* codes,
-                          uint32_t* hist, cudaStream_t stream, int passes, int shift0 = 0, const uint32_t* run_if = nullptr);
+                          uint32_t* hist, cudaStream_t stream, int passes, int shift0 = 0);
 // K1 + K2 + K3 of a small build (n <= kSmallBuildMax) in one launch by one thread-block cluster (small_build.cu): writes the scene
 // bounds into `header`, the sorted codes and the permutation where the one-sweep sort would leave them.  Needs no
 // zero-initialised scratch.
@@ -172,9 +172,11 @@ struct SortBuffers {
   uint32_t* final_vals;
 };
 SortBuffers sort_buffers(void* scratch, const ScratchLayout& L);
-// shift0: first bit of pass 0's digit.  slot0: pass p uses histogram, status block and ticket slot0 + p.  run_if: see tie_fixup.cu.
+// shift0: first bit of pass 0's digit.  slot0: pass p uses histogram, status block and ticket slot0 + p.
 cudaError_t launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStream_t stream, void* const* pass_events,
-                        int shift0 = 0, int slot0 = 0, const uint32_t* run_if = nullptr);
+                        int shift0 = 0, int slot0 = 0);
+// The conditional second sort of a 63-bit build as one cooperative launch (radix_sort.cu).
+cudaError_t launch_second_sort(const SortBuffers& B, int passes, int n, int slot0, const uint32_t* run_if, cudaStream_t stream);
 // 63-bit codes sorted by their upper 32 bits: orders every run of equal upper bits by the lower 31 (tie_fixup.cu).
 // tile_flag [tie_fixup_tiles(n)] zeroed, tile_list [tie_fixup_tiles(n)], list_count zeroed: the work list of long runs.
 cudaError_t launch_tie_fixup(void* keys, uint32_t* vals, int n, uint32_t* tile_flag, uint32_t* tile_list, uint32_t* list_count,

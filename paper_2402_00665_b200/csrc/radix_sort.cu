@@ -16,6 +16,8 @@
 // (profiles/): the code below is written to keep the per-pair instruction count down -- full tiles take
 // a path without bounds predicates, positions are 32-bit, values are loaded after the ranking so that
 // fewer registers are live (4 CTAs of 256 threads per SM).
+#include <cooperative_groups.h>
+
 #include "common.cuh"
 #include "device_helpers.cuh"
 
@@ -297,15 +299,11 @@ __device__ __forceinline__ void sort_tile(SortSmem<KeyT>& s, const KeyT* __restr
 #ifndef BVH_SORT_MINBLOCKS
 #define BVH_SORT_MINBLOCKS 4
 #endif
-// COND: a pass of the conditional second sort of a 63-bit build (tie_fixup.cu) -- nothing to do unless *run_if != 0.
-// Such a pass is launched with a small grid whose blocks keep taking tiles (tickets) until none is left, so that the
-// usual case, flag clear, costs a launch of a few hundred blocks whatever n is.  The ordinary pass (COND = false) is
-// one tile per block.
-template <typename KeyT, bool IOTA, bool TOP, bool COND>
+template <typename KeyT, bool IOTA, bool TOP>
 __global__ void __launch_bounds__(kSortThreads, BVH_SORT_MINBLOCKS)
 onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_out, const uint32_t* __restrict__ vals_in,
                      uint32_t* __restrict__ vals_out, const uint32_t* __restrict__ hist, uint32_t* status,
-                     uint32_t* tile_counter, int n, int shift, const uint32_t* __restrict__ run_if) {
+                     uint32_t* tile_counter, int n, int shift) {
   constexpr int TILE = SortCfg<KeyT>::TILE;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SortSmem<KeyT>& s = *reinterpret_cast<SortSmem<KeyT>*>(smem_raw);
@@ -315,55 +313,32 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, KeyT* __restrict__ keys_o
   if (tid < 256) s.tile_hist[tid] = 0;
   pdl_wait();
   pdl_trigger();
-  if (COND) {
-    if (*run_if == 0) return;
-    const uint32_t tiles = (uint32_t)((n + TILE - 1) / TILE);
-    while (true) {
-      if (tid == 0) s.tile = atomicAdd(tile_counter, 1u);
-      __syncthreads();
-      const uint32_t tile = s.tile;
-      if (tile >= tiles) return;
-      const uint32_t tile_base = tile * (uint32_t)TILE;
-      const int valid_in_tile = min(TILE, n - (int)tile_base);
-      if (valid_in_tile == TILE)
-        sort_tile<KeyT, IOTA, true, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, TILE, shift);
-      else
-        sort_tile<KeyT, IOTA, false, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, valid_in_tile,
-                                          shift);
-      __syncthreads();
-      for (int i = tid; i < kSortWarps * kSortChains * 256; i += kSortThreads) (&s.warp_hist[0][0][0])[i] = 0;
-      if (tid < 256) s.tile_hist[tid] = 0;
-      __syncthreads();
-    }
-  } else {
-    if (tid == 0) s.tile = atomicAdd(tile_counter, 1u);
-    __syncthreads();
-    const uint32_t tile = s.tile;
-    const uint32_t tile_base = tile * (uint32_t)TILE;
-    const int valid_in_tile = min(TILE, n - (int)tile_base);
-    if (valid_in_tile == TILE)
-      sort_tile<KeyT, IOTA, true, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, TILE, shift);
-    else
-      sort_tile<KeyT, IOTA, false, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, valid_in_tile,
-                                        shift);
-  }
+  if (tid == 0) s.tile = atomicAdd(tile_counter, 1u);
+  __syncthreads();
+  const uint32_t tile = s.tile;
+  const uint32_t tile_base = tile * (uint32_t)TILE;
+  const int valid_in_tile = min(TILE, n - (int)tile_base);
+  if (valid_in_tile == TILE)
+    sort_tile<KeyT, IOTA, true, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, TILE, shift);
+  else
+    sort_tile<KeyT, IOTA, false, TOP>(s, keys_in, keys_out, vals_in, vals_out, hist, status, tile, tile_base, valid_in_tile,
+                                      shift);
 }
 
-template <typename KeyT, bool COND>
-static cudaError_t sort_passes(const SortBuffers& B, int n, int passes, cudaStream_t stream, void* const* pass_events, int shift0,
-                               int slot0, const uint32_t* run_if) {
+template <typename KeyT>
+static cudaError_t sort_all(const SortBuffers& B, int n, int passes, cudaStream_t stream, void* const* pass_events, int shift0,
+                            int slot0) {
   const int tiles = (n + SortCfg<KeyT>::TILE - 1) / SortCfg<KeyT>::TILE;
   KeyT* keys[2] = {static_cast<KeyT*>(B.keys[0]), static_cast<KeyT*>(B.keys[1])};
   const size_t smem = sizeof(SortSmem<KeyT>);
   // the opt-in to more than 48 KB of dynamic shared memory is a property of the function: set once per process
   static const cudaError_t attr = [&]() {
-    cudaError_t e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, true, false, COND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, false, COND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, true, COND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     return e;
   }();
   if (attr != cudaSuccess) return attr;
-  const int blocks = (COND && tiles > 4 * sm_count()) ? 4 * sm_count() : tiles;   // conditional pass: persistent grid
   for (int p = 0; p < passes; ++p) {
     const int in = p & 1, out = in ^ 1, slot = slot0 + p;     // slot: which histogram / status block / ticket this pass uses
     uint32_t* st = B.status + (size_t)slot * tiles * 256;
@@ -373,25 +348,106 @@ static cudaError_t sort_passes(const SortBuffers& B, int n, int passes, cudaStre
     const uint32_t* none = nullptr;
     cudaError_t e;
     if (p == 0)
-      e = launch_pdl(onesweep_pass_kernel<KeyT, true, false, COND>, dim3(blocks), dim3(kSortThreads), smem, stream,
-                 keys[in], keys[out], none, vout, B.hist + slot * 256, st, B.tile_counters + slot, n, shift, run_if);
+      e = launch_pdl(onesweep_pass_kernel<KeyT, true, false>, dim3(tiles), dim3(kSortThreads), smem, stream,
+                 keys[in], keys[out], none, vout, B.hist + slot * 256, st, B.tile_counters + slot, n, shift);
     else if (p == passes - 1 && sizeof(KeyT) == 4)   // (64-bit codes: the top digit of neighbouring keys is rarely shared; ballots)
-      e = launch_pdl(onesweep_pass_kernel<KeyT, false, true, COND>, dim3(blocks), dim3(kSortThreads), smem, stream,
-                 keys[in], keys[out], vin, vout, B.hist + slot * 256, st, B.tile_counters + slot, n, shift, run_if);
+      e = launch_pdl(onesweep_pass_kernel<KeyT, false, true>, dim3(tiles), dim3(kSortThreads), smem, stream,
+                 keys[in], keys[out], vin, vout, B.hist + slot * 256, st, B.tile_counters + slot, n, shift);
     else
-      e = launch_pdl(onesweep_pass_kernel<KeyT, false, false, COND>, dim3(blocks), dim3(kSortThreads), smem, stream,
-                 keys[in], keys[out], vin, vout, B.hist + slot * 256, st, B.tile_counters + slot, n, shift, run_if);
+      e = launch_pdl(onesweep_pass_kernel<KeyT, false, false>, dim3(tiles), dim3(kSortThreads), smem, stream,
+                 keys[in], keys[out], vin, vout, B.hist + slot * 256, st, B.tile_counters + slot, n, shift);
     if (e != cudaSuccess) return e;
     if (pass_events && pass_events[p]) cudaEventRecord(static_cast<cudaEvent_t>(pass_events[p]), stream);
   }
   return cudaSuccess;
 }
 
+// The conditional second sort of a 63-bit build (tie_fixup.cu) as ONE cooperative launch: nothing unless *run_if != 0
+// (the usual case costs one launch instead of nine); else the digit histograms of the codes as they stand, then the
+// eight passes, a grid-wide barrier after each.  It starts from the codes and indices the four upper-bit passes left
+// in keys[0] / vals[0]: equal codes are in ascending original index there (those passes are stable), and eight more
+// stable passes over all 63 bits keep them so -- the order of the plain eight-pass sort.
 template <typename KeyT>
-static cudaError_t sort_all(const SortBuffers& B, int n, int passes, cudaStream_t stream, void* const* pass_events, int shift0,
-                            int slot0, const uint32_t* run_if) {
-  if (run_if) return sort_passes<KeyT, true>(B, n, passes, stream, pass_events, shift0, slot0, run_if);
-  return sort_passes<KeyT, false>(B, n, passes, stream, pass_events, shift0, slot0, run_if);
+__global__ void __launch_bounds__(kSortThreads, BVH_SORT_MINBLOCKS)
+second_sort_kernel(KeyT* keys0, KeyT* keys1, uint32_t* vals0, uint32_t* vals1, uint32_t* hist, uint32_t* status,
+                   uint32_t* tile_counters, int n, int passes, const uint32_t* __restrict__ run_if) {
+  constexpr int TILE = SortCfg<KeyT>::TILE;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  SortSmem<KeyT>& s = *reinterpret_cast<SortSmem<KeyT>*>(smem_raw);
+  pdl_wait();
+  if (*run_if == 0) return;
+  namespace cg = cooperative_groups;
+  cg::grid_group grid = cg::this_grid();
+  const int tid = threadIdx.x;
+  const uint32_t tiles = (uint32_t)((n + TILE - 1) / TILE);
+  // ---- digit histograms of all passes (shared-memory atomics, one global atomic per bin and block) ----
+  uint32_t* s_hist = reinterpret_cast<uint32_t*>(smem_raw);          // passes * 256 words <= 8 KB: aliases the sort's shared memory
+  for (int i = tid; i < passes * 256; i += kSortThreads) s_hist[i] = 0;
+  __syncthreads();
+  for (int64_t i = (int64_t)blockIdx.x * kSortThreads + tid; i < n; i += (int64_t)gridDim.x * kSortThreads) {
+    const KeyT k = keys0[i];
+    for (int p = 0; p < passes; ++p) atomicAdd(&s_hist[p * 256 + (int)((k >> (8 * p)) & 0xFF)], 1u);
+  }
+  __syncthreads();
+  for (int i = tid; i < passes * 256; i += kSortThreads)
+    if (s_hist[i]) atomicAdd(&hist[i], s_hist[i]);
+  grid.sync();
+  // ---- the passes ----
+  for (int p = 0; p < passes; ++p) {
+    const KeyT* kin = (p & 1) ? keys1 : keys0;
+    KeyT* kout = (p & 1) ? keys0 : keys1;
+    const uint32_t* vin = (p & 1) ? vals1 : vals0;
+    uint32_t* vout = (p & 1) ? vals0 : vals1;
+    uint32_t* st = status + (size_t)p * tiles * 256;
+    while (true) {
+      __syncthreads();
+      for (int i = tid; i < kSortWarps * kSortChains * 256; i += kSortThreads) (&s.warp_hist[0][0][0])[i] = 0;
+      if (tid < 256) s.tile_hist[tid] = 0;
+      if (tid == 0) s.tile = atomicAdd(tile_counters + p, 1u);
+      __syncthreads();
+      const uint32_t tile = s.tile;
+      if (tile >= tiles) break;
+      const uint32_t tile_base = tile * (uint32_t)TILE;
+      const int valid_in_tile = min(TILE, n - (int)tile_base);
+      if (valid_in_tile == TILE)
+        sort_tile<KeyT, false, true, false>(s, kin, kout, vin, vout, hist + p * 256, st, tile, tile_base, TILE, 8 * p);
+      else
+        sort_tile<KeyT, false, false, false>(s, kin, kout, vin, vout, hist + p * 256, st, tile, tile_base, valid_in_tile, 8 * p);
+    }
+    grid.sync();
+  }
+}
+
+// hist / status / tile_counters: those of slot `slot0` on (zeroed); passes must be even (the result returns to keys[0]).
+cudaError_t launch_second_sort(const SortBuffers& B, int passes, int n, int slot0, const uint32_t* run_if, cudaStream_t stream) {
+  using KeyT = uint64_t;
+  const size_t smem = sizeof(SortSmem<KeyT>);
+  static int blocks_per_sm = 0;
+  static const cudaError_t attr = [&]() {
+    cudaError_t e = cudaFuncSetAttribute(second_sort_kernel<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess)
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, second_sort_kernel<KeyT>, kSortThreads, smem);
+    return e;
+  }();
+  if (attr != cudaSuccess) return attr;
+  if (blocks_per_sm < 1 || (passes & 1)) return cudaErrorInvalidValue;
+  const int tiles = (n + SortCfg<KeyT>::TILE - 1) / SortCfg<KeyT>::TILE;
+  int blocks = blocks_per_sm * sm_count();                    // all co-resident: the grid-wide barrier needs that
+  if (blocks > tiles) blocks = tiles;
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(blocks);
+  cfg.blockDim = dim3(kSortThreads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeCooperative;
+  at[0].val.cooperative = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  const int tiles_all = tiles;
+  return cudaLaunchKernelEx(&cfg, second_sort_kernel<KeyT>, static_cast<KeyT*>(B.keys[0]), static_cast<KeyT*>(B.keys[1]), B.vals[0],
+                            B.vals[1], B.hist + slot0 * 256, B.status + (size_t)slot0 * tiles_all * 256, B.tile_counters + slot0, n,
+                            passes, run_if);
 }
 
 SortBuffers sort_buffers(void* scratch, const ScratchLayout& L) {
@@ -409,9 +465,9 @@ SortBuffers sort_buffers(void* scratch, const ScratchLayout& L) {
 }
 
 cudaError_t launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStream_t stream, void* const* pass_events,
-                        int shift0, int slot0, const uint32_t* run_if) {
-  if (key_bytes == 4) return sort_all<uint32_t>(B, n, passes, stream, pass_events, shift0, slot0, run_if);
-  return sort_all<uint64_t>(B, n, passes, stream, pass_events, shift0, slot0, run_if);
+                        int shift0, int slot0) {
+  if (key_bytes == 4) return sort_all<uint32_t>(B, n, passes, stream, pass_events, shift0, slot0);
+  return sort_all<uint64_t>(B, n, passes, stream, pass_events, shift0, slot0);
 }
 
 }  // namespace bvh

@@ -8,14 +8,15 @@
 // stably -- the order an LSD sort of all 63 bits gives (readings G5/G6).  Runs are short unless the input is
 // degenerate, so the fix-up is a streaming read of the codes plus a little work in shared memory.
 //
-// Two kernels.  tie_short_kernel streams over the codes, one thread per position: the thread at the start of a run of
-// 2 .. kFixSerial pairs orders it by a stable insertion sort (a handful of loads and stores through L1); a longer run
-// puts the tile of kFixTile positions it starts in on a work list.  tie_long_kernel takes the listed tiles: one block
+// Two kernels.  tie_short_kernel streams over the codes, a tile of kFixTile positions per block in shared memory: every
+// pair of a run of 2 .. kFixSerial pairs finds its rank in the run by (lower bits, position) and moves there; a longer
+// run puts the tile it starts in on a work list.  tie_long_kernel takes the listed tiles: one block
 // loads the runs that START in the tile (the last of them may reach into the next tile) into shared memory and
 // orders the long ones by a bitonic network over (lower bits, original index), the whole block per run.  A run that
-// reaches more than a tile past the tile it starts in does not fit: the block then raises `fallback`, and the build
-// runs the plain eight-pass sort after this kernel (its kernels are enqueued anyway and return at once when the flag
-// is clear) -- correct for every input, slower only for those with thousands of primitives inside one of 2^32 cells.
+// reaches more than a tile past the tile it starts in does not fit: the block then raises `fallback`, and eight more
+// stable passes over all 63 bits (second_sort_kernel in radix_sort.cu: ONE cooperative launch, enqueued in any case
+// because nothing may read the flag back, that returns at once while the flag is clear) redo the order -- correct for
+// every input, slower only for those with thousands of primitives inside one of 2^32 cells.
 #include "common.cuh"
 
 namespace bvh {
