@@ -48,8 +48,8 @@ NOMINAL_HBM_GBS = 8000.0   # the denominator BASELINE.json north_star names
 NCU_TRAFFIC_BYTES = {
     # profiles/r02b_ncu.md: one step, rows 2 (collect), 6 (rows_to_csr), 14 (hierarchy, level 1); two-pass leg, rows 0 (count),
     # 1 (fill): DRAM read + write
-    ("C3", 10_000_000, 1_000_000): {"collect": 3_143_800_000, "rows_to_csr": 4_996_000_000, "count": 233_777_000,
-                                    "fill": 3_204_300_000, "hierarchy": 1_330_800_000},
+    ("C3", 10_000_000, 1_000_000): {"collect": 3_180_800_000, "rows_to_csr": 4_995_000_000, "count": 241_363_000,
+                                    "fill": 3_220_800_000, "hierarchy": 1_335_100_000},
 }
 
 
