@@ -73,7 +73,7 @@ def byte_model(n: int, q: int, nnz: int, prim_floats: int, query_floats: int, bi
         "overflow": 4 * q,                               # counts (no row overflows when the capacity holds the largest row)
     }
     per_kernel["tie_fixup"] = K * n                  # 63-bit two-stage sort: one read of the sorted codes
-    per_kernel["second_sort"] = 0                    # ... and nine kernels that return at once unless a run did not fit a block
+    per_kernel["second_sort"] = 0                    # ... and one cooperative launch that returns at once unless a run did not fit a block
     per_kernel["front"] = sum(v for k, v in per_kernel.items() if k in ("init", "bounds", "morton") or k.startswith("sort_pass"))
     build_total = (3 * S + 4 * K + (2 * P - 1) * (K + 4) + 100) * n      # SURVEY.md B_build
     query_total = (2 * Sq + 24) * q + 4 * nnz                            # SURVEY.md B_query
@@ -299,7 +299,7 @@ def run_ours(args) -> dict | None:
     # kernels of this library per stage when the stages are called one by one (the staged legs) ...
     launches_per_step = {**({"front": 1} if small_build else
                             {"init": 0, "bounds": 1, "morton": 1, **{k: 1 for k in sort_names},
-                             **({"tie_fixup": 2, "second_sort": 9} if two_stage else {})}),
+                             **({"tie_fixup": 2, "second_sort": 1} if two_stage else {})}),
                          "hierarchy": 2 if n > 256 else 1, "order": 5 if q > 8192 else 1, "collect": 1,
                          "scan": 3 if q > 4096 else 1, "rows_to_csr": 1, "overflow": 1}
     # ... and in the timed step, where the query is one call: no identity order for q <= 8192, scan + row copy fused for q <= 4096
