@@ -527,7 +527,8 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
               const uint32_t m = __ballot_sync(0xffffffffu, hit);
               const int at = ocount + __popc(m & lt_mask);
               if (kFillStage == 0) {
-                if (hit && p0 + at < cap) orow[p0 + at] = (int)(leaf[u].payload() & kLeafPrimMask);
+                // (fill: the row is exactly as long as its hits; collect: positions past the capacity are dropped)
+                if (hit && (MODE == kModeFill || p0 + at < cap)) orow[p0 + at] = (int)(leaf[u].payload() & kLeafPrimMask);
               } else {
                 if (hit) buf[at] = (int)(leaf[u].payload() & kLeafPrimMask);
               }
