@@ -764,11 +764,13 @@ def test_ray_queries_point_leaves_and_brute_force(B, oracle_lib):
     assert np.array_equal(o2.cpu().numpy(), goff) and np.array_equal(i2.cpu().numpy(), gidx[: goff[-1]])
 
 
-def test_cuda_graph_capture_and_replay(B):
+@pytest.mark.parametrize("n", [65_536 + 77, 5_000])
+def test_cuda_graph_capture_and_replay(B, n):
     """The C ABI only enqueues work (no allocation, no synchronisation, no host read): a whole build + ordered
     count / scan / fill can be captured in a CUDA graph and replayed; the replay reproduces the eager result on the
-    captured inputs and follows the inputs when their contents change."""
-    w = W.make("C5", n=65_536 + 77, q=4096, radius=0.02)
+    captured inputs and follows the inputs when their contents change.  Both forms of the build: the pipeline (with its
+    cooperative launch of the conditional second sort) and the one-cluster front of a small build."""
+    w = W.make("C5", n=n, q=4096, radius=0.02)
     d, dq = _dev(w.prims), _dev(w.queries)
     bvh, ws = B.Bvh(w.n, w.morton_bits), B.QueryWorkspace(w.q)
     bvh.nodes.zero_()
