@@ -275,6 +275,9 @@ struct LeafRec<false> {
   __device__ __forceinline__ bool cand(const Query& q, float& key) const { return q.cand_box(r.lox, r.loy, r.loz, r.hix, r.hiy, r.hiz, key); }
 };
 
+#ifndef BVH_TRAV_LOAD_AFTER_SCAN
+#define BVH_TRAV_LOAD_AFTER_SCAN 0
+#endif
 #ifndef BVH_SCAN_SKIP_EMPTY
 #define BVH_SCAN_SKIP_EMPTY 0
 #endif
@@ -432,7 +435,11 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
       // the load is in flight ----
       const bool at_internal = walking && node < leaf_base;
       NodeRec rec;
+#if !BVH_TRAV_LOAD_AFTER_SCAN
       if (at_internal) rec = load_rec(internal + node);
+#else
+      if (at_internal) asm volatile("prefetch.global.L1 [%0];" ::"l"(internal + node));
+#endif
       // ---- SCAN: the warp tests every range posted in the previous round, 32 consecutive leaves per step ----------
       while (posted) {
         const int o = __ffs(posted) - 1;
@@ -561,6 +568,9 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
         }
       }
       // ---- WALK, second half: one step of Algorithm 1 per lane ---------------------------------------------------
+#if BVH_TRAV_LOAD_AFTER_SCAN
+      if (at_internal) rec = load_rec(internal + node);
+#endif
       if (walking && !(ANY && count != 0)) {               // (any hit: a lane whose scan just found one is done)
         if (!at_internal) {                                  // a single leaf (reached as a child or through a rope)
           const int i = node - leaf_base;
