@@ -273,14 +273,16 @@ cudaError_t launch_morton(const float* prim, int n, bool is_box, int morton_bits
 }
 
 cudaError_t launch_query_morton(const float* queries, int q, int kind, const NodesHeader* root, uint32_t* codes, uint32_t* hist,
-                         cudaStream_t stream) {
+                                cudaStream_t stream) {
+  // histograms of the kQueryOrderPasses digits from bit kQueryOrderShift up: the schedule only sorts by those
   const unsigned g = morton_grid(q);
+  constexpr int P = kQueryOrderPasses, S = kQueryOrderShift;
   if (kind == 0)
-    return launch_pdl(morton_kernel<uint32_t, 4, 4, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, 0);
+    return launch_pdl(morton_kernel<uint32_t, P, 4, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, S);
   else if (kind == 2)
-    return launch_pdl(morton_kernel<uint32_t, 4, 8, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, 0);
+    return launch_pdl(morton_kernel<uint32_t, P, 8, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, S);
   else
-    return launch_pdl(morton_kernel<uint32_t, 4, 6, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, 0);
+    return launch_pdl(morton_kernel<uint32_t, P, 6, true>, dim3(g), dim3(kMortonThreads), 0, stream, queries, q, nullptr, root, codes, hist, S);
 }
 
 }  // namespace bvh

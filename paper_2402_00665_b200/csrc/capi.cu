@@ -308,7 +308,7 @@ static int query_order(const void* nodes, int64_t n, const float* queries, int64
                           B.hist, stream) != cudaSuccess)
     return BVH_ERR_CUDA;
   B.final_vals = order;
-  if (launch_sort(B, 4, 4, (int)q, stream, nullptr) != cudaSuccess) return BVH_ERR_CUDA;
+  if (launch_sort(B, 4, kQueryOrderPasses, (int)q, stream, nullptr, kQueryOrderShift, 0) != cudaSuccess) return BVH_ERR_CUDA;
   return check_launch();
 }
 
