@@ -210,6 +210,21 @@ def test_two_stage_sort_of_63bit_codes(B, oracle_lib, pattern):
     assert_build_equal(export_np(bvh2), o, pattern + " again")
 
 
+def test_two_stage_sort_fallback_at_scale(B, oracle_lib):
+    """The conditional second sort with a persistent grid (more tiles than resident blocks) and grid-wide barriers: 2.5 M
+    points of which 200 000 sit inside ONE of the 2^32 cells, and a second dense cell of 30 000."""
+    rng = np.random.default_rng(77)
+    bg = rng.random((2_270_000, 3)).astype(np.float32)
+    c1 = (np.array([0.3, 0.6, 0.2]) + rng.random((200_000, 3)) * 5e-5).astype(np.float32)
+    c2 = (np.array([0.8, 0.1, 0.7]) + rng.random((30_000, 3)) * 5e-5).astype(np.float32)
+    pts = np.concatenate([np.array([[0, 0, 0], [1, 1, 1]], np.float32), bg, c1, c2]).astype(np.float32)
+    pts = pts[rng.permutation(len(pts))] + np.float32(0.0)
+    o = oracle_lib.build_bvh(pts, 63)
+    runs = np.diff(np.flatnonzero(np.diff(np.concatenate([[-1], (o.sorted_codes >> np.uint64(31)).astype(np.int64), [-2]])) != 0))
+    assert runs.max() > 20_000
+    assert_build_equal(export_np(gpu_build(B, pts, 63)), o, "fallback at scale")
+
+
 @pytest.mark.parametrize("bits", [30, 63])
 @pytest.mark.parametrize("n", [1, 2, 5, 1000, 10_000])
 def test_all_points_coincident(B, oracle_lib, n, bits):
