@@ -10,7 +10,7 @@
  *    and the `rows` of bvh_query_collect: 32-byte aligned), owned by the caller.  The only host
  *    pointers are the `size_t*` outputs of the *_sizes functions.
  *  - The library never allocates, frees or synchronises; it holds no global state and is re-entrant
- *    across streams.  Every call only enqueues work on `stream` (a cudaStream_t passed as void*;
+ *    across streams (one documented exception: bvh_scan_counts_static keeps its scratch inside the library).  Every call only enqueues work on `stream` (a cudaStream_t passed as void*;
  *    NULL = the legacy default stream) and returns.
  *  - `scratch` of a build must stay alive until that build's stream work is complete; it also
  *    holds the sorted codes and permutation that bvh_export reads.  `nodes` must stay alive until
@@ -46,6 +46,7 @@ extern "C" {
 #define BVH_ERR_TOO_LARGE (-3)        /* n >= 2^30 (node indices and sort counters are 32-bit)         */
 #define BVH_ERR_SCRATCH (-4)          /* scratch_bytes smaller than bvh_sizes / bvh_scan_sizes report  */
 #define BVH_ERR_CUDA (-5)             /* a kernel launch failed (cudaGetLastError)                     */
+#define BVH_ERR_STATIC_LIMIT (-6)     /* bvh_scan_counts_static: q > BVH_SCAN_STATIC_MAX_Q             */
 
 /* Library version, for the binding's sanity check. */
 int bvh_version(void);
@@ -118,6 +119,30 @@ int bvh_query_boxes_count(const void* nodes, int64_t n, const float* minmax, int
 int bvh_scan_sizes(int64_t q, size_t* scratch_bytes);
 int bvh_scan_counts(const int32_t* counts, int64_t q, int64_t* offsets, void* scratch,
                     size_t scratch_bytes, void* stream);
+
+/* bvh_scan_counts for a caller that cannot supply `scratch`.  bvh_scan_counts needs a little working memory (one
+ * int64 per tile of 4096 counts) and, like the rest of this library, expects the caller to bring it.  That does not
+ * work for code that is not allowed to allocate when it runs: a component that starts after the application has handed
+ * all device memory to its own pool, a callback inside a framework that forbids allocator calls (cudaMalloc
+ * synchronises the whole device, and fails while a stream of the process is being captured), a latency-critical loop
+ * that must not wait on the allocator's lock.  This entry point takes no scratch: the tile sums go to a fixed 64 KB
+ * array that is part of the library's device image.  It calls no cudaMalloc / cudaFree and no library routine that
+ * allocates, and produces the same `offsets`, bit for bit, as bvh_scan_counts.
+ *   Limit     q <= BVH_SCAN_STATIC_MAX_Q (2^25 counts = what 64 KB of tile sums cover).  A larger q returns
+ *             BVH_ERR_STATIC_LIMIT and enqueues nothing; use bvh_scan_counts with your own scratch for it.
+ *   Cost      the 64 KB are resident on every GPU that loads the library, until the process exits, used or not.
+ *   Sharing   this is the one place where the library keeps state: one array per GPU, used by every call on that GPU.
+ *             Calls that can overlap on the GPU (two streams with no event between them, two host threads) race on
+ *             it and spoil each other's offsets; serialise them (one stream per device is enough).  Calls on different
+ *             GPUs do not interfere.  The array keeps the previous call's tile sums; nothing in it has to start at
+ *             zero, since each scan first writes every entry it later reads.
+ *   Set-up    the first call on a device looks up the array's address on that device (and loads the library's kernels
+ *             there if nothing has yet); later calls only enqueue.  Make that first call at start-up, on the device and
+ *             before any stream capture begins.  The device that is current at the call must be the one that owns
+ *             `counts`, `offsets` and `stream`.
+ * counts, offsets, q, stream and the q = 0 behaviour (offsets[0] = 0) are as for bvh_scan_counts. */
+#define BVH_SCAN_STATIC_MAX_Q ((int64_t)8192 * 4096)
+int bvh_scan_counts_static(const int32_t* counts, int64_t q, int64_t* offsets, void* stream);
 
 /* Fill pass: the same traversal again; row j of the CSR, indices[offsets[j] .. offsets[j+1]), gets
  * the ORIGINAL indices of the primitives hit, in traversal order (ascending Morton position; PAPER.md:56

@@ -26,6 +26,7 @@ ERRORS = {
     -3: "BVH_ERR_TOO_LARGE",
     -4: "BVH_ERR_SCRATCH",
     -5: "BVH_ERR_CUDA",
+    -6: "BVH_ERR_STATIC_LIMIT",
 }
 
 # every symbol include/bvh_b200.h declares: (name, argtypes)
@@ -43,6 +44,7 @@ SYMBOLS = {
     "bvh_query_boxes_count": [_P, c_int64, _P, c_int64, _P, _P, _P],
     "bvh_scan_sizes": [c_int64, ctypes.POINTER(c_size_t)],
     "bvh_scan_counts": [_P, c_int64, _P, _P, c_size_t, _P],
+    "bvh_scan_counts_static": [_P, c_int64, _P, _P],
     "bvh_query_spheres_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
     "bvh_query_boxes_fill": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
     "bvh_query_spheres_nearest": [_P, c_int64, _P, c_int64, _P, _P, _P, _P],
@@ -261,6 +263,19 @@ def bvh_scan_sizes(q: int) -> int:
 def bvh_scan_counts(counts, q: int, offsets, scratch) -> None:
     _check(load_library().bvh_scan_counts(_ptr(counts), q, _ptr(offsets), _ptr(scratch),
                                           scratch.numel() * scratch.element_size(), _stream()), "bvh_scan_counts")
+
+
+SCAN_STATIC_MAX_Q = 8192 * 4096   # BVH_SCAN_STATIC_MAX_Q
+
+
+def bvh_scan_counts_static(counts, q: int, offsets) -> None:
+    """``bvh_scan_counts`` without a scratch argument, for code that may not allocate device memory when it runs
+    (memory already committed to a pool, allocator calls forbidden by the host framework, no tolerance for the
+    allocator's device-wide synchronisation).  The tile sums go to a 64 KB array inside the library, one per GPU and
+    shared by all calls on it: at most ``SCAN_STATIC_MAX_Q`` counts (more raises ``BVH_ERR_STATIC_LIMIT``), and calls
+    that may overlap on the GPU must be serialised by the caller.  Same offsets, bit for bit, as ``bvh_scan_counts``.
+    Make the first call on each device at start-up (it resolves the array's address there)."""
+    _check(load_library().bvh_scan_counts_static(_ptr(counts), q, _ptr(offsets), _stream()), "bvh_scan_counts_static")
 
 
 def bvh_query_spheres_fill(nodes, n: int, xyzr, q: int, order, offsets, indices) -> None:
