@@ -93,7 +93,11 @@ int bvh_build_staged(const float* prim, int prim_is_box, int64_t n, int morton_b
  * (30-bit code of the sphere centre / box centroid, clamped into the frame; same kernels as the build's
  * steps 1-2).  Passing `order` to the count and fill calls makes thread t serve query order[t], so that
  * neighbouring threads walk nearly the same nodes.  Results are unaffected: row j of the CSR still
- * belongs to query j.  order: uint32[q].  bvh_query_order_sizes is a host call. */
+ * belongs to query j.  order: uint32[q].  bvh_query_order_sizes is a host call.
+ * A batch of q <= 8192 queries (or n = 0: no frame) gets the IDENTITY order, order[t] = t, in one launch: so small a
+ * batch is bound by the number of dependent launches, and the part of the hierarchy it touches stays in L2 whatever the
+ * schedule.  `nodes`, the queries and `scratch` are not read then (they may be NULL); `order` is still written in full.
+ * queries and scratch must be 16-byte aligned (the codes are computed with 128-bit loads). */
 int bvh_query_order_sizes(int64_t q, size_t* scratch_bytes);
 int bvh_query_order_spheres(const void* nodes, int64_t n, const float* xyzr, int64_t q, uint32_t* order,
                             void* scratch, size_t scratch_bytes, void* stream);

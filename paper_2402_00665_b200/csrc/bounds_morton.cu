@@ -192,7 +192,9 @@ __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __r
   if (PRIM_FLOATS == 3 || PRIM_FLOATS == 6) {
     // 12 consecutive floats = three 128-bit loads per thread = four points or two boxes: a quarter of the load
     // instructions of one scalar load per coordinate, and 48 bytes in flight per thread instead of 12 (the kernel
-    // waits on its loads, not on its arithmetic).  The codes leave as one or two 128-bit stores.
+    // waits on its loads, not on its arithmetic).  The codes leave as one or two 128-bit stores.  Box QUERIES (FROM_ROOT
+    // with six floats) come this way too.  The 128-bit accesses need `prim` and `codes` 16-byte aligned: the build and
+    // query_order (capi.cu) refuse a misaligned pointer, and the scratch layout keeps `codes` on a 256-byte boundary.
     constexpr int PG = (PRIM_FLOATS == 3) ? 4 : 2;        // primitives per group
     const int64_t groups = n / PG;
     const float4* __restrict__ v = reinterpret_cast<const float4*>(prim);
@@ -223,7 +225,7 @@ __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __r
     }
     done = groups * PG;
   }
-  for (int64_t i = done + tid0; i < n; i += stride) {     // the last n % PG primitives; every query of the FROM_ROOT variants
+  for (int64_t i = done + tid0; i < n; i += stride) {     // the last n % PG primitives; every sphere and ray query (4 / 8 floats)
     float lo[3], hi[3];
     if (PRIM_FLOATS == 6) {
       const float* p = prim + 6 * i;

@@ -8,20 +8,31 @@ namespace bvh {
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 int sm_count() {
-  static const int sms = []() {
-    int dev = 0, v = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0)
-      v = kNumSMs;
-    return v;
-  }();
-  return sms;
+  static PerDeviceOnce once;
+  int sms = 0;
+  const cudaError_t e = once_per_device(once, &sms, [](int* v) {
+    int dev = 0;
+    cudaError_t err = cudaGetDevice(&dev);
+    if (err == cudaSuccess) err = cudaDeviceGetAttribute(v, cudaDevAttrMultiProcessorCount, dev);
+    if (err == cudaSuccess && *v <= 0) err = cudaErrorInvalidDevice;
+    return err;
+  });
+  return e == cudaSuccess ? sms : kNumSMs;   // (a failed query is not remembered)
 }
+
+#ifndef BVH_TWO_STAGE_SORT
+#define BVH_TWO_STAGE_SORT 1
+#endif
+constexpr bool kTwoStageSort = BVH_TWO_STAGE_SORT != 0;
 
 ScratchLayout scratch_layout(int64_t n, int morton_bits) {
   ScratchLayout L{};
   L.key_bytes = (morton_bits == 30) ? 4 : 8;
   L.passes = (morton_bits == 30) ? 4 : 8;
-  L.slots = (morton_bits == 30) ? 4 : 12;
+  // 63-bit codes, two-stage sort: the four upper-bit passes use zeroed slots; the eight slots of the conditional second
+  // sort sit past the end (hist2 / status2) and are cleared by that sort itself, only when it runs
+  const bool second_sort = morton_bits == 63 && kTwoStageSort;
+  L.slots = (morton_bits == 30 || second_sort) ? 4 : 8;
   const int tile = sort_tile_items(L.key_bytes);
   L.tiles = (int)((n + tile - 1) / tile);
   if (L.tiles < 1) L.tiles = 1;
@@ -53,6 +64,12 @@ ScratchLayout scratch_layout(int64_t n, int morton_bits) {
   off += align_up((size_t)L.segments * sizeof(int32_t), 256);
   L.fix_list = off;
   if (morton_bits == 63) off += align_up((size_t)tie_fixup_tiles((int64_t)nn) * sizeof(uint32_t), 256);
+  L.hist2 = L.status2 = off;
+  if (second_sort) {
+    off += align_up((size_t)8 * 256 * sizeof(uint32_t), 256);
+    L.status2 = off;
+    off += align_up((size_t)8 * L.tiles * 256 * sizeof(uint32_t), 256);
+  }
   L.total = off;
   return L;
 }
@@ -139,11 +156,6 @@ static inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_
 
 static int check_launch() { return cudaGetLastError() == cudaSuccess ? BVH_OK : BVH_ERR_CUDA; }
 
-#ifndef BVH_TWO_STAGE_SORT
-#define BVH_TWO_STAGE_SORT 1
-#endif
-constexpr bool kTwoStageSort = BVH_TWO_STAGE_SORT != 0;
-
 static int build(const float* prim, bool is_box, int64_t n, int morton_bits, void* nodes, void* scratch,
                  size_t scratch_bytes, void* stream_, void* const* events = nullptr, int variant = 0) {
   if (n < 0) return BVH_ERR_INVALID_ARGUMENT;
@@ -196,7 +208,8 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
                            stream) != cudaSuccess)
         return BVH_ERR_CUDA;
       mark(8);
-      if (launch_second_sort(B, 8, (int)n, 4, &header->sort_fallback, stream) != cudaSuccess) return BVH_ERR_CUDA;
+      if (launch_second_sort(B, 8, (int)n, 4, reinterpret_cast<uint32_t*>(base + L.hist2), reinterpret_cast<uint32_t*>(base + L.status2),
+                             &header->sort_fallback, stream) != cudaSuccess) return BVH_ERR_CUDA;
       mark(9);
       mark(10);
       mark(11);

@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 namespace bvh {
 
 constexpr int kSentinel = -1;   // the paper's sentinel node; reading G9
@@ -59,10 +61,12 @@ struct ScratchLayout {
   size_t seg_items;     // int2 [segments][192]  subtrees handed from one window of the bottom-up pass to its parent
   size_t seg_count;     // int32 [segments]      how many each window handed over
   size_t fix_list;      // uint32 [tie_fixup_tiles]  the work list
+  size_t hist2;         // uint32 [8][256], uint32 [8][tiles][256]: histograms and tile status words of the conditional second
+  size_t status2;       //   sort of a 63-bit build; NOT zeroed per build, that sort clears them when it runs (it rarely does)
   size_t total;
   int segments;         // windows of all levels of the bottom-up pass (hierarchy.cu)
   int passes;           // 8-bit digits of a code: 4 (30-bit) or 8 (63-bit)
-  int slots;            // histogram / status / ticket slots: passes, or 4 + 8 for the two-stage sort of 63-bit codes
+  int slots;            // zeroed histogram / status slots: one per pass (4 for the upper-bit passes of a two-stage sort)
   int tiles;
   int key_bytes;
 };
@@ -176,7 +180,8 @@ SortBuffers sort_buffers(void* scratch, const ScratchLayout& L);
 cudaError_t launch_sort(const SortBuffers& B, int key_bytes, int passes, int n, cudaStream_t stream, void* const* pass_events,
                         int shift0 = 0, int slot0 = 0);
 // The conditional second sort of a 63-bit build as one cooperative launch (radix_sort.cu).
-cudaError_t launch_second_sort(const SortBuffers& B, int passes, int n, int slot0, const uint32_t* run_if, cudaStream_t stream);
+cudaError_t launch_second_sort(const SortBuffers& B, int passes, int n, int slot0, uint32_t* hist, uint32_t* status,
+                               const uint32_t* run_if, cudaStream_t stream);
 // 63-bit codes sorted by their upper 32 bits: orders every run of equal upper bits by the lower 31 (tie_fixup.cu).
 // tile_flag [tie_fixup_tiles(n)] zeroed, tile_list [tie_fixup_tiles(n)], list_count zeroed: the work list of long runs.
 cudaError_t launch_tie_fixup(void* keys, uint32_t* vals, int n, uint32_t* tile_flag, uint32_t* tile_list, uint32_t* list_count,
@@ -226,7 +231,35 @@ cudaError_t launch_rows_to_csr(const int32_t* rows, int64_t cap, const int32_t* 
 cudaError_t launch_scan_rows_to_csr_small(const int32_t* rows, int64_t cap, const int32_t* counts, int64_t* offsets, int64_t q,
                                           int32_t* indices, cudaStream_t stream, int64_t limit = 0);
 int scan_single_tile_items();
-int sm_count();   // multiprocessors of the current device (cached)
+int sm_count();   // multiprocessors of the current device (cached per device)
+
+// One-time set-up that belongs to a (kernel, device) pair -- the opt-in to more than 48 KB of dynamic shared memory, an
+// occupancy query -- is remembered per DEVICE, not per process: a process may build on several GPUs, and what
+// cudaFuncSetAttribute sets holds only for the device that was current.  A failed set-up is returned and NOT remembered (the
+// next call tries again).  Devices beyond kMaxDevices, or an unknown current device, run the set-up on every call.
+constexpr int kMaxDevices = 64;
+inline int current_device() {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return -1;
+  return dev;
+}
+struct PerDeviceOnce {
+  std::atomic<int> value[kMaxDevices];   // 0 = not set up on that device yet; else what the set-up produced (non-zero)
+};
+// setup(int* value) -> cudaError_t; must leave *value != 0 on success.  Returns the cached / fresh value through *out.
+template <typename F>
+inline cudaError_t once_per_device(PerDeviceOnce& once, int* out, F&& setup) {
+  const int dev = current_device();
+  int v = dev >= 0 ? once.value[dev].load(std::memory_order_acquire) : 0;
+  if (v == 0) {
+    const cudaError_t e = setup(&v);
+    if (e != cudaSuccess) return e;
+    if (v == 0) return cudaErrorUnknown;
+    if (dev >= 0) once.value[dev].store(v, std::memory_order_release);
+  }
+  if (out) *out = v;
+  return cudaSuccess;
+}
 // K7: exclusive scan of int32 counts into int64 offsets[q+1].
 size_t scan_scratch_bytes(int64_t q);
 cudaError_t launch_scan(const int32_t* counts, int64_t q, int64_t* offsets, void* scratch, cudaStream_t stream);

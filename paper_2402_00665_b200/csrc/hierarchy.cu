@@ -739,9 +739,12 @@ static cudaError_t launch_hierarchy_keys(const float* prim, bool is_box, const K
   if (e != cudaSuccess || lv.levels <= 1) return e;
   using D = typename Delta<KeyT>::T;
   const size_t smem = sizeof(MergeSmem<D>);
-  // the opt-in to more than 48 KB of dynamic shared memory is a property of the function: set once per process
-  static const cudaError_t attr =
-      cudaFuncSetAttribute(hierarchy_merge_kernel<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  // the opt-in to more than 48 KB of dynamic shared memory holds for the device that was current: once per device
+  static PerDeviceOnce once;   // (one per KeyT instantiation)
+  const cudaError_t attr = once_per_device(once, nullptr, [&](int* done) {
+    *done = 1;
+    return cudaFuncSetAttribute(hierarchy_merge_kernel<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  });
   if (attr != cudaSuccess) return attr;
   return launch_pdl(hierarchy_merge_kernel<KeyT>, dim3(lv.segs[1]), dim3(kMergeThreads), smem, stream, codes, nodes, n,
                     is_box ? kLeafBoxes : kLeafPoints, seg_items, seg_count, arrivals, lv);

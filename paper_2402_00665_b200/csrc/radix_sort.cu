@@ -331,13 +331,15 @@ static cudaError_t sort_all(const SortBuffers& B, int n, int passes, cudaStream_
   const int tiles = (n + SortCfg<KeyT>::TILE - 1) / SortCfg<KeyT>::TILE;
   KeyT* keys[2] = {static_cast<KeyT*>(B.keys[0]), static_cast<KeyT*>(B.keys[1])};
   const size_t smem = sizeof(SortSmem<KeyT>);
-  // the opt-in to more than 48 KB of dynamic shared memory is a property of the function: set once per process
-  static const cudaError_t attr = [&]() {
+  // the opt-in to more than 48 KB of dynamic shared memory holds for the device that was current: once per device
+  static PerDeviceOnce once;
+  const cudaError_t attr = once_per_device(once, nullptr, [&](int* done) {
     cudaError_t e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(onesweep_pass_kernel<KeyT, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    *done = 1;
     return e;
-  }();
+  });
   if (attr != cudaSuccess) return attr;
   for (int p = 0; p < passes; ++p) {
     const int in = p & 1, out = in ^ 1, slot = slot0 + p;     // slot: which histogram / status block / ticket this pass uses
@@ -380,6 +382,14 @@ second_sort_kernel(KeyT* keys0, KeyT* keys1, uint32_t* vals0, uint32_t* vals1, u
   cg::grid_group grid = cg::this_grid();
   const int tid = threadIdx.x;
   const uint32_t tiles = (uint32_t)((n + TILE - 1) / TILE);
+  // ---- this sort's histograms and tile status words lie outside the part of the scratch a build zeroes (they would be
+  // two thirds of that memset for a sort that almost never runs): cleared here, by the sort that needs them ----
+  {
+    const size_t stride = (size_t)gridDim.x * kSortThreads, first = (size_t)blockIdx.x * kSortThreads + tid;
+    for (size_t i = first; i < (size_t)passes * 256; i += stride) hist[i] = 0;
+    for (size_t i = first; i < (size_t)passes * tiles * 256; i += stride) status[i] = 0;
+    grid.sync();
+  }
   // ---- digit histograms of all passes (shared-memory atomics, one global atomic per bin and block) ----
   uint32_t* s_hist = reinterpret_cast<uint32_t*>(smem_raw);          // passes * 256 words <= 8 KB: aliases the sort's shared memory
   for (int i = tid; i < passes * 256; i += kSortThreads) s_hist[i] = 0;
@@ -418,24 +428,27 @@ second_sort_kernel(KeyT* keys0, KeyT* keys1, uint32_t* vals0, uint32_t* vals1, u
   }
 }
 
-// hist / status / tile_counters: those of slot `slot0` on (zeroed); passes must be even (the result returns to keys[0]).
-cudaError_t launch_second_sort(const SortBuffers& B, int passes, int n, int slot0, const uint32_t* run_if, cudaStream_t stream) {
+// hist [passes][256] / status [passes][tiles][256]: this sort's own, in any state (the kernel clears them); tile counters:
+// those of slot `slot0` on, zeroed by the build; passes must be even (the result returns to keys[0]).
+cudaError_t launch_second_sort(const SortBuffers& B, int passes, int n, int slot0, uint32_t* hist, uint32_t* status,
+                               const uint32_t* run_if, cudaStream_t stream) {
   using KeyT = uint64_t;
   const size_t smem = sizeof(SortSmem<KeyT>);
-  static int blocks_per_sm = 0;
-  static const cudaError_t attr = [&]() {
+  // shared-memory opt-in and occupancy of the kernel on the CURRENT device: once per device
+  static PerDeviceOnce once;
+  int blocks_per_sm = 0;
+  const cudaError_t attr = once_per_device(once, &blocks_per_sm, [&](int* per_sm) {
     cudaError_t e = cudaFuncSetAttribute(second_sort_kernel<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess)
-      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, second_sort_kernel<KeyT>, kSortThreads, smem);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, second_sort_kernel<KeyT>, kSortThreads, smem);
+    if (e == cudaSuccess && *per_sm < 1) e = cudaErrorInvalidValue;
     return e;
-  }();
+  });
   if (attr != cudaSuccess) return attr;
-  if (blocks_per_sm < 1 || (passes & 1)) return cudaErrorInvalidValue;
+  if (passes & 1) return cudaErrorInvalidValue;
   const int tiles = (n + SortCfg<KeyT>::TILE - 1) / SortCfg<KeyT>::TILE;
   int blocks = blocks_per_sm * sm_count();                    // all co-resident: the grid-wide barrier needs that
   if (blocks > tiles) blocks = tiles;
   cudaLaunchConfig_t cfg{};
-  cfg.gridDim = dim3(blocks);
   cfg.blockDim = dim3(kSortThreads);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = stream;
@@ -444,10 +457,18 @@ cudaError_t launch_second_sort(const SortBuffers& B, int passes, int n, int slot
   at[0].val.cooperative = 1;
   cfg.attrs = at;
   cfg.numAttrs = 1;
-  const int tiles_all = tiles;
-  return cudaLaunchKernelEx(&cfg, second_sort_kernel<KeyT>, static_cast<KeyT*>(B.keys[0]), static_cast<KeyT*>(B.keys[1]), B.vals[0],
-                            B.vals[1], B.hist + slot0 * 256, B.status + (size_t)slot0 * tiles_all * 256, B.tile_counters + slot0, n,
-                            passes, run_if);
+  // The occupancy query counts the whole device; the context may own less of it (an MPS active-thread percentage, a green
+  // context, SM partitioning), and then the runtime refuses the grid as too large for a cooperative launch.  The kernel
+  // draws its tiles from a ticket counter and works with ANY number of co-resident blocks, so the refused launch is
+  // repeated with half the grid until it is accepted: a build must not fail over a sort that almost never runs.
+  cudaError_t e = cudaErrorCooperativeLaunchTooLarge;
+  for (; blocks >= 1 && e == cudaErrorCooperativeLaunchTooLarge; blocks = blocks > 1 ? blocks / 2 : 0) {
+    cfg.gridDim = dim3(blocks);
+    e = cudaLaunchKernelEx(&cfg, second_sort_kernel<KeyT>, static_cast<KeyT*>(B.keys[0]), static_cast<KeyT*>(B.keys[1]), B.vals[0],
+                           B.vals[1], hist, status, B.tile_counters + slot0, n, passes, run_if);
+    if (e == cudaErrorCooperativeLaunchTooLarge) (void)cudaGetLastError();   // not sticky: clear it before the next attempt
+  }
+  return e;
 }
 
 SortBuffers sort_buffers(void* scratch, const ScratchLayout& L) {

@@ -236,8 +236,12 @@ int tie_fixup_tiles(int64_t n) { return (int)((n + kFixTile - 1) / kFixTile); }
 cudaError_t launch_tie_fixup(void* keys, uint32_t* vals, int n, uint32_t* tile_flag, uint32_t* tile_list, uint32_t* list_count,
                              uint32_t* fallback, cudaStream_t stream) {
   const size_t smem = sizeof(FixSmem);
-  // the opt-in to more than 48 KB of dynamic shared memory is a property of the function: set once per process
-  static const cudaError_t attr = cudaFuncSetAttribute(tie_long_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  // the opt-in to more than 48 KB of dynamic shared memory holds for the device that was current: once per device
+  static PerDeviceOnce once;
+  const cudaError_t attr = once_per_device(once, nullptr, [&](int* done) {
+    *done = 1;
+    return cudaFuncSetAttribute(tie_long_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  });
   if (attr != cudaSuccess) return attr;
   unsigned long long* k = static_cast<unsigned long long*>(keys);
   const int tiles = tie_fixup_tiles(n);
