@@ -10,12 +10,22 @@ CSR is its local CSR shifted by the number of results of the ranks before it, an
 concatenation of the blocks.
 
 This module holds only that plumbing (block bounds, the all-gather, the offset shift, an optional gather to every
-rank); it is device-agnostic, which is how the N > 1 path is tested on CPU with ``gloo``.
+rank); it is device-agnostic, which is how the N > 1 path is tested on CPU with ``gloo``.  The tensors handed to a
+collective live where the group's backend can reach them: on the GPU under ``nccl``, on the host otherwise (``gloo``
+has no all-gather of CUDA tensors), so CUDA results can also be assembled by ranks that talk over ``gloo`` -- two
+processes sharing one GPU in the tests.
 """
 from __future__ import annotations
 
 import torch
 import torch.distributed as dist
+
+
+def _comm_device(t: torch.Tensor, group=None) -> torch.device:
+    """Where a tensor must live to go through a collective of ``group``: its own device under nccl, else the host."""
+    if dist.is_initialized() and "nccl" in str(dist.get_backend(group)):
+        return t.device
+    return torch.device("cpu")
 
 
 def block_bounds(q: int, rank: int, world: int) -> tuple[int, int]:
@@ -45,6 +55,7 @@ def assemble(local_offsets: torch.Tensor, local_indices: torch.Tensor, q: int, g
         raise ValueError(f"rank {rank}: expected offsets of {out.q_hi - out.q_lo + 1} entries, got {local_offsets.numel()}")
     nnz_local = local_offsets[-1].reshape(1).to(torch.int64)
     if world > 1:
+        nnz_local = nnz_local.to(_comm_device(nnz_local, group))
         sizes = [torch.zeros_like(nnz_local) for _ in range(world)]
         dist.all_gather(sizes, nnz_local, group=group)
         sizes = torch.cat(sizes).cpu()
@@ -71,10 +82,13 @@ def gather_global(csr: ShardedCsr, q: int, group=None) -> tuple[torch.Tensor, to
     off_pad[: csr.q_hi - csr.q_lo] = csr.offsets[:-1]
     idx_pad = torch.zeros(max(max_nnz, 1), dtype=torch.int32, device=dev)
     idx_pad[: csr.indices.numel()] = csr.indices
+    comm = _comm_device(off_pad, group)
+    off_pad, idx_pad = off_pad.to(comm), idx_pad.to(comm)
     offs = [torch.zeros_like(off_pad) for _ in range(world)]
     idxs = [torch.zeros_like(idx_pad) for _ in range(world)]
     dist.all_gather(offs, off_pad, group=group)
     dist.all_gather(idxs, idx_pad, group=group)
+    offs, idxs = [t.to(dev) for t in offs], [t.to(dev) for t in idxs]
     rows = [offs[r][: block_bounds(q, r, world)[1] - block_bounds(q, r, world)[0]] for r in range(world)]
     offsets = torch.cat(rows + [torch.tensor([csr.nnz_total], dtype=torch.int64, device=dev)])
     indices = torch.cat([idxs[r][: csr.nnz_per_rank[r]] for r in range(world)])
@@ -96,5 +110,8 @@ def sharded_query(local_query, queries: torch.Tensor, group=None) -> ShardedCsr:
     rank = dist.get_rank(group) if dist.is_initialized() else 0
     q = int(queries.shape[0])
     lo, hi = block_bounds(q, rank, world)
-    off, idx = local_query(queries[lo:hi])
+    block = queries[lo:hi]
+    if block.data_ptr() % 16 != 0:      # the C ABI wants 16-byte aligned queries: a block of 24-byte boxes may start off that
+        block = block.clone()
+    off, idx = local_query(block)
     return assemble(off, idx, q, group=group)

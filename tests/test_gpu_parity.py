@@ -6,6 +6,8 @@ position).  Sizes span several sort tiles (4096 / 3072 keys) plus a ragged tail.
 """
 from __future__ import annotations
 
+import os
+
 import numpy as np
 import pytest
 
@@ -208,6 +210,9 @@ def test_two_stage_sort_of_63bit_codes(B, oracle_lib, pattern):
     assert_build_equal(export_np(bvh), o, pattern)
     bvh2 = gpu_build(B, pts, 63)               # a second build into fresh buffers: flags and work list start from zero again
     assert_build_equal(export_np(bvh2), o, pattern + " again")
+    bvh2.build(_dev(pts))                      # and a third into USED buffers: the second sort finds its own histograms and
+    torch.cuda.synchronize()                   # status words as the last build left them and has to clear them itself
+    assert_build_equal(export_np(bvh2), o, pattern + " into used scratch")
 
 
 def test_two_stage_sort_fallback_at_scale(B, oracle_lib):
@@ -223,6 +228,24 @@ def test_two_stage_sort_fallback_at_scale(B, oracle_lib):
     runs = np.diff(np.flatnonzero(np.diff(np.concatenate([[-1], (o.sorted_codes >> np.uint64(31)).astype(np.int64), [-2]])) != 0))
     assert runs.max() > 20_000
     assert_build_equal(export_np(gpu_build(B, pts, 63)), o, "fallback at scale")
+
+
+def test_second_device_in_the_same_process(B, oracle_lib):
+    """What a kernel needs set once (the opt-in to more than 48 KB of dynamic shared memory, the occupancy of the
+    cooperative sort, the SM count) is remembered per device: after builds on cuda:0, the same builds on cuda:1 in the
+    same process must work and give the same bits.  63-bit codes with n > 16384 go through tie_long_kernel (83 KB of
+    shared memory) and the cooperative second sort; 30-bit through the one-sweep passes and the merge kernel."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    for name, n in (("C4", 70_003), ("C3", 120_001)):
+        w = W.make(name, n=n, q=16)
+        o = oracle_lib.build_bvh(w.prims, w.morton_bits)
+        for dev in ("cuda:0", "cuda:1", "cuda:0"):
+            with torch.cuda.device(dev):
+                bvh = B.Bvh(n, w.morton_bits, device=dev)
+                bvh.build(torch.from_numpy(w.prims).to(dev))
+                torch.cuda.synchronize(dev)
+                assert_build_equal(export_np(bvh), o, f"{name} on {dev}")
 
 
 @pytest.mark.parametrize("bits", [30, 63])
@@ -904,3 +927,75 @@ def test_variant_apetrei_algorithm3(B, oracle_lib, name, n):
         if tiny >= 2:
             assert int(gt["root"][0]) == ot.root and np.array_equal(gt["left"][: tiny - 1], ot.left)
             assert np.array_equal(gt["right"][: tiny - 1], ot.right)
+
+
+# ---- the paper's worked example and the equal-codes case, straight through the CUDA path ---------------------------
+# (tests/golden/*.txt are hand-derived from PAPER.md:120, :166, :101, :75; the oracle is not involved here)
+
+def _gold_rows(name):
+    with open(os.path.join(os.path.dirname(__file__), "golden", name)) as f:
+        return [ln.split("#")[0].strip() for ln in f if ln.split("#")[0].strip()]
+
+
+def _gold_arrays(name):
+    return {t[0]: [int(v) for v in t[1:]] for t in (ln.split() for ln in _gold_rows(name)) if t[0] not in ("keys", "internal")}
+
+
+def _p1_points():
+    """Eight points on the x axis whose 10-bit x cells are c = 0, 64, 128, 160, 608, 768, 800, 1023 (x = c / 1024 and x = 1
+    in the frame [0, 1]): c / 32 = 0, 2, 4, 5, 19, 24, 25, 31 has the same highest differing bit between neighbours
+    (1, 2, 0, 4, 3, 0, 2) as the golden's 5-bit keys, and interleaving with the zero bits of y and z keeps that order, so the
+    hierarchy is the one PAPER.md:120 describes.  Given in a shuffled order: the sort has to find the Morton order."""
+    c = np.array([0, 64, 128, 160, 608, 768, 800, 1024], np.float32) / np.float32(1024)
+    given = np.array([5, 2, 7, 0, 3, 6, 1, 4])
+    pts = np.zeros((8, 3), np.float32)
+    pts[:, 0] = c[given]
+    return pts, np.argsort(given)                      # perm[i] = where the i-th smallest x was given
+
+
+@pytest.mark.parametrize("bits", [30, 63])
+def test_paper_worked_example_p1_through_the_cuda_path(B, bits):
+    g = _gold_arrays("p1_worked_example.txt")
+    pts, perm = _p1_points()
+    bvh = gpu_build(B, pts, bits)
+    e = export_np(bvh)
+    assert e["perm"].tolist() == perm.tolist()
+    assert e["left_child"][:7].tolist() == g["left_child"]          # I_3 -> I_1, I_2;  I_4 -> L_4, I_5  (PAPER.md:120)
+    assert e["rope"].tolist() == g["rope"]                          # right-most path -> sentinel (PAPER.md:31, 75)
+    d = np.diff(e["sorted_codes"].astype(np.int64))
+    x = e["sorted_codes"][:-1] ^ e["sorted_codes"][1:]
+    assert (d > 0).all() and np.array_equal(np.argsort(x, kind="stable"), np.argsort(np.array(g["delta_star"]), kind="stable"))
+    # Algorithm 1 (PAPER.md:46-69) with an always-true predicate over the arrays the GPU built
+    node, walk = 0, []
+    while node != -1:
+        walk.append(node)
+        node = int(e["left_child"][node]) if node < 7 else int(e["rope"][node])
+        assert len(walk) <= 15
+    assert walk == g["walk"]
+    # and the GPU's own traversal: a sphere around everything reports every leaf, in leaf order
+    off, idx = gpu_query(B, bvh, np.array([[0.5, 0, 0, 2.0], [0.0625, 0, 0, 1.0 / 1024]], np.float32))
+    assert off.tolist() == [0, 8, 9] and idx[:8].tolist() == perm.tolist() and idx[8] == perm[1]
+
+
+def test_paper_worked_example_p1_apetrei_numbering_through_variant_2(B):
+    """Algorithm 3 unmodified: nodes named by their split, root stored; "the children of I_0 have a
+    gap of 3": root 3 with children 1 and 4."""
+    g = _gold_arrays("p1_apetrei_numbering.txt")
+    pts, _ = _p1_points()
+    _, v = _variant2(B, pts, 30)
+    assert int(v["root"][0]) == g["root"][0] == 3
+    assert v["left"][:7].tolist() == g["left"] and v["right"][:7].tolist() == g["right"]
+    assert (int(v["left"][3]), int(v["right"][3])) == (1, 4)
+    assert v["rope"].tolist() == g["rope"]
+
+
+@pytest.mark.parametrize("bits", [30, 63])
+def test_equal_codes_p4_goldens_through_the_cuda_path(B, bits):
+    """All codes equal: the augmented keys (code, i) decide; n = 1..5 against the hand-derived arrays."""
+    for line in _gold_rows("p4_equal_codes.txt"):
+        head, lc, rp = line.split("|")
+        n = int(head.split()[1])
+        e = export_np(gpu_build(B, np.full((n, 3), 0.25, np.float32), bits))
+        assert e["left_child"][: n - 1].tolist() == [int(t) for t in lc.split()], n
+        assert e["rope"].tolist() == [int(t) for t in rp.split()], n
+        assert e["perm"].tolist() == list(range(n))
