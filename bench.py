@@ -6,7 +6,10 @@ bounds, Morton codes, one-sweep radix sort, modified-Apetrei bottom-up pass with
 by stackless sphere range search to CSR.  The query part of the step is the single-pass form of
 count-then-fill (order, collect = one traversal that counts and stores rows, scan, rows -> CSR, overflow
 rows) as ONE call of the C ABI (bvh_query_csr); the same stages as separate calls give the per-kernel breakdown, and
-the two-traversal form (count, scan, fill) is timed beside it as `query_two_pass`.  Workload at N=1: BASELINE.json configs[2]
+the two-traversal form (count, scan, fill) is timed beside it as `query_two_pass`.  The row capacity of the single-pass
+query is learned from ANOTHER batch of the same workload (other seeds; an untimed count pass), never from the batch
+that is timed: rows that do not fit are traversed again inside the timed call (`query.overflow_rows`), and
+`query_small_capacity` times the same call with 1.25 x the other batch's mean row as capacity.  Workload at N=1: BASELINE.json configs[2]
 ("C3": 10,000,000 Gaussian-mixture points, 30-bit Morton, 1,000,000 sphere queries of radius 0.002), the
 config `north_star` quotes its target on.
 
@@ -232,14 +235,29 @@ def run_ours(args) -> dict | None:
     fill_fn = (binding.bvh_query_spheres_fill, binding.bvh_query_boxes_fill, binding.bvh_query_rays_fill)[kind]
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)
 
-    # one untimed pass to learn nnz and the largest row (same inputs every step -> same counts): sizes the result
-    # buffer and the row capacity of the single-pass query ("capacity from the previous batch")
+    # Row capacity of the single-pass query.  A caller cannot know the rows of the batch it is about to serve, so the
+    # capacity is NOT taken from this batch: it comes from an untimed count pass over ANOTHER batch of the same workload
+    # (other seeds: "the previous batch"), rounded up to 8.  Rows of the timed batch that are longer overflow and are
+    # traversed a second time inside the timed query; how many do is reported.  A second capacity, 1.25 x the previous
+    # batch's mean row, is timed beside it (less scratch, more overflow).
     bvh.build(d_prims)
+    cap, cap_small, prev_q = 8, 8, min(q, 1 << 20)
+    if prev_q > 0:
+        d_prev = torch.from_numpy(np.ascontiguousarray(
+            workloads.previous_queries(args.workload, prev_q, seed_offset=0 if shard else rank))).to(device)
+        count_fn(bvh.nodes, n, d_prev, prev_q, None, ws.counts)
+        prev_counts = ws.counts[:prev_q]
+        cap = max(8, (int(prev_counts.max().item()) + 7) // 8 * 8)
+        cap_small = max(8, (int(np.ceil(1.25 * float(prev_counts.double().mean().item()))) + 7) // 8 * 8)
+        del d_prev
+    # one untimed pass over the batch itself: nnz sizes the result buffer (same inputs every step -> same counts)
     order_fn(bvh.nodes, n, d_queries, q, ws.order, ws.order_scratch)
     count_fn(bvh.nodes, n, d_queries, q, ws.order, ws.counts)
     binding.bvh_scan_counts(ws.counts, q, ws.offsets, ws.scan_scratch)
     nnz = int(ws.offsets[q].item())
-    cap = max(8, (int(ws.counts[:q].max().item()) + 7) // 8 * 8) if q > 0 else 8
+    max_row = int(ws.counts[:q].max().item()) if q > 0 else 0
+    overflow_rows = int((ws.counts[:q] > cap).sum().item()) if q > 0 else 0
+    overflow_rows_small = int((ws.counts[:q] > cap_small).sum().item()) if q > 0 else 0
     d_indices = torch.empty(max(nnz, 1), dtype=torch.int32, device=device)
     d_rows = torch.empty(max(q, 1) * cap, dtype=torch.int32, device=device)
 
@@ -363,6 +381,20 @@ def run_ours(args) -> dict | None:
         torch.cuda.synchronize()
         for k, v in read_query_stage_times().items():
             acc[k] = acc.get(k, 0.0) + v
+
+    # ---- the one-call query again with the small capacity (1.25 x the previous batch's mean row): its own rows buffer ----
+    e_s0, e_s1 = ev(), ev()
+    d_rows_small = torch.empty(max(q, 1) * cap_small, dtype=torch.int32, device=device)
+    for it in range(args.steps + 1):
+        flush.fill_(1)
+        e_s0.record()
+        binding.bvh_query_csr(bvh.nodes, n, d_queries, kind, q, cap_small, d_rows_small, ws.order, ws.counts, ws.offsets,
+                              d_indices, d_indices.numel(), ws.order_scratch)
+        e_s1.record()
+        torch.cuda.synchronize()
+        if it > 0:   # the first one is a warm-up
+            acc["small_cap_query"] = acc.get("small_cap_query", 0.0) + e_s0.elapsed_time(e_s1)
+    del d_rows_small
 
     # ---- the two-traversal query, same inputs, same hierarchy (not part of `value` / `ms_per_step`) ------------------
     for _ in range(args.steps):
@@ -512,7 +544,10 @@ def run_ours(args) -> dict | None:
         "vs_baseline": None,
         "dtype": "u32 Morton codes / f32 boxes" if bits == 30 else "u64 Morton codes / f32 boxes", "data": "synthetic",
         "config": config_dict(args, w, world, {"hits_per_query": round(nnz_all / max(q_all, 1), 2), "nnz": int(nnz_all),
-                                               "row_capacity": cap, "multi": args.multi if world > 1 else "single"}),
+                                               "row_capacity": cap,
+                                               "row_capacity_source": f"largest row of another batch of the workload ({prev_q} "
+                                                                      "queries, other seeds), untimed count pass, rounded up to 8",
+                                               "multi": args.multi if world > 1 else "single"}),
         "build": {"ms": round(ms["_build"], 4), "mprims_per_s": round(value, 2), "alg_bytes": int(model["build_total"]),
                   "gbs": round(build_gbs, 1), "frac_of_measured_peak": round(build_gbs / peak, 4),
                   "frac_of_8TBs": round(build_gbs / NOMINAL_HBM_GBS, 4),
@@ -522,10 +557,18 @@ def run_ours(args) -> dict | None:
                   "frac_of_measured_peak": round(query_gbs / peak, 4), "frac_of_8TBs": round(query_gbs / NOMINAL_HBM_GBS, 4),
                   "path": "bvh_query_csr, one call: order + collect + scan + rows_to_csr + fill_overflow (byte-identical CSR)",
                   "staged_ms": round(ms["_query_staged"], 4),
+                  "row_capacity": cap, "rows_bytes": int(max(q, 1) * cap * 4), "largest_row": max_row,
+                  "overflow_rows": overflow_rows,
                   "excluded": "nnz read-back and indices allocation (included in e2e)"},
         "query_two_pass": {"ms": round(tp_ms, 4), "mqueries_per_s": round(q_all / (tp_ms * 1e-3) / 1e6, 3),
                            "count_ms": round(ms["tp_count"], 4), "scan_ms": round(ms["tp_scan"], 4),
                            "fill_ms": round(ms["tp_fill"], 4), "path": "order + count + scan + fill"},
+        "query_small_capacity": {"ms": round(ms["small_cap_query"], 4),
+                                 "mqueries_per_s": round(q_all / (ms["small_cap_query"] * 1e-3) / 1e6, 3),
+                                 "row_capacity": cap_small, "rows_bytes": int(max(q, 1) * cap_small * 4),
+                                 "overflow_rows": overflow_rows_small,
+                                 "path": "bvh_query_csr, one call, capacity = 1.25 x mean row of the other batch: the rows that "
+                                         "overflow are traversed again by the fill inside the call (byte-identical CSR)"},
         "roofline": {"bound": "hbm", "kernel": dominant, "achieved": dk["gbs"], "peak": peak, "unit": "GB/s",
                      "frac": dk["frac"], "traffic": traffic, "peak_source": peak_src,
                      "alg_bytes_per_launch": dk["alg_bytes"], "ms_per_launch": dk["ms"]},

@@ -218,3 +218,21 @@ def make(name: str, n: int | None = None, q: int | None = None, radius: float | 
         qs = spheres_at(hollow_shell(q, seed=1005 + so), r) if q else None
         return Workload(name, pts, "points", 63, qs, "spheres" if q else None, "hollow cube shell")
     raise KeyError(name)
+
+
+def previous_queries(name: str, q: int, radius: float | None = None, seed_offset: int = 0) -> np.ndarray:
+    """ANOTHER batch of ``q`` queries of config ``name``: same scene, same distribution and radius, other seeds (the
+    query seeds of :func:`make` + 500).  It stands for the batch a caller served before the one being measured -- what a
+    row capacity "taken from the previous batch" can honestly be derived from."""
+    so = 10000 * int(seed_offset)
+    if name == "C1":
+        return spheres_at(uniform_cube(q, seed=500 + so), 0.085 if radius is None else radius)
+    if name == "C2":
+        return spheres_at(uniform_cube(q, seed=1502 + so), 0.0157 if radius is None else radius)
+    if name == "C3":
+        return spheres_at(gaussian_mixture(q, seed=1503 + so, centre_seed=3 + so), 0.002 if radius is None else radius)
+    if name == "C4":
+        return boxes_around(sphere_surface(q, seed=1504 + so), 2.0 * (5e-4 if radius is None else radius))
+    if name == "C5":
+        return spheres_at(hollow_shell(q, seed=1505 + so), C5_RADIUS_FULL if radius is None else radius)
+    raise KeyError(name)
