@@ -126,7 +126,7 @@ cudaError_t launch_scene_bounds(const float* prim, int n, bool is_box, Header* h
   const int64_t nfloats = (int64_t)n * (is_box ? 6 : 3);
   const int64_t chunks = nfloats / (96 * 4);
   int64_t blocks = (chunks + (kBoundsThreads / 32) - 1) / (kBoundsThreads / 32);
-  const int64_t cap = (int64_t)kNumSMs * 8;
+  const int64_t cap = (int64_t)sm_count() * 8;
   if (blocks > cap) blocks = cap;
   if (blocks < 1) blocks = 1;
   return launch_pdl(scene_bounds_kernel, dim3((unsigned)blocks), dim3(kBoundsThreads), 0, stream, prim, nfloats, is_box, header);
@@ -251,7 +251,7 @@ __global__ void __launch_bounds__(kMortonThreads) morton_kernel(const float* __r
 static unsigned morton_grid(int n, int per_thread = 1) {
   const int64_t units = ((int64_t)n + per_thread - 1) / per_thread;
   int64_t blocks = (units + kMortonThreads - 1) / kMortonThreads;
-  const int64_t cap = (int64_t)kNumSMs * 8;
+  const int64_t cap = (int64_t)sm_count() * 8;
   if (blocks > cap) blocks = cap;
   if (blocks < 1) blocks = 1;
   return (unsigned)blocks;

@@ -11,7 +11,7 @@ namespace bvh {
 
 constexpr int kSentinel = -1;   // the paper's sentinel node; reading G9
 constexpr int kInvalid = -1;    // the paper's "invalid entry value (e.g., -1)" in `store`
-constexpr int kNumSMs = 148;    // B200: compile-time grid sizing of the streaming kernels (a performance choice, not a limit)
+constexpr int kNumSMs = 148;    // B200: what sm_count() falls back to when the device cannot be queried; grids are sized from sm_count()
 
 // 32-byte node record, read and written as two float4 (one 32-byte sector per node visit).
 //   lo = {min.x, min.y, min.z, bitcast(left_child)}   hi = {max.x, max.y, max.z, bitcast(rope)}

@@ -683,13 +683,14 @@ __global__ void __launch_bounds__(kTravThreads, Query::kCtasPerSm) traverse_kern
 // mostly empty GPU (C1: 4096 queries = 128 warps, 58 us).  When the batch cannot fill the GPU's warp slots anyway, the
 // queries are spread out -- only every 2^s-th lane carries one -- so that up to 32 times as many warps share the same
 // scans (C1: ... us).  Results and their order do not depend on which lane serves a query.
-#ifndef BVH_TRAV_SPREAD_THREADS
-#define BVH_TRAV_SPREAD_THREADS (148 * 1024)
+#ifndef BVH_TRAV_SPREAD_THREADS_PER_SM
+#define BVH_TRAV_SPREAD_THREADS_PER_SM 1024
 #endif
 template <typename Query>
 static cudaError_t launch_traverse_kind(TraverseArgs A, int mode, cudaStream_t stream) {
   A.spread_log2 = 0;
-  while (A.spread_log2 < 5 && (A.q << (A.spread_log2 + 1)) <= (int64_t)BVH_TRAV_SPREAD_THREADS) ++A.spread_log2;
+  const int64_t spread_threads = (int64_t)sm_count() * BVH_TRAV_SPREAD_THREADS_PER_SM;
+  while (A.spread_log2 < 5 && (A.q << (A.spread_log2 + 1)) <= spread_threads) ++A.spread_log2;
   const int64_t chunks = ((A.q << A.spread_log2) + kTravThreads - 1) / kTravThreads;
   if (chunks > 0x7fffffff) return cudaErrorInvalidValue;
   const dim3 g((unsigned)chunks), b(kTravThreads);
@@ -758,6 +759,56 @@ __device__ __forceinline__ void copy_row(const int32_t* __restrict__ src, int32_
   for (; e < c; e += G) dst[e] = __ldcs(src + e);
 }
 
+// The same copy by a whole warp with 128-bit accesses (rows of 128 entries and more: C3's rows_to_csr moves 4.7 GB, a fifth
+// of the query).  `src`, a row of `rows`, is 32-byte aligned; dst = indices + offsets[j] is aligned to 4 bytes only.  The
+// DESTINATION is cut at its 16-byte boundaries: with dst = D + a (D aligned, a in 0..3) the aligned vector m holds
+// D[4m .. 4m+3] = src[4m-a .. 4m-a+3], i.e. the last a entries of source vector m-1 and the first 4-a of source vector m.
+// Every lane loads source vector m (aligned), takes vector m-1 from the lane below it by shuffle, and stores one aligned
+// vector; the up to three entries before the first and after the last whole vector go as 4-byte copies.  Four vectors per
+// lane are in flight per round (2 KB per warp; the 4-byte version had 512 B).  Loads stay inside the row: for a whole
+// destination vector 4m <= c+a-4 < cap, and cap is a multiple of 8.  All loop bounds are warp-uniform (shuffles inside).
+__device__ __forceinline__ int4 shifted_vector(const int4& prev, const int4& cur, int a) {
+  if (a == 1) return make_int4(prev.w, cur.x, cur.y, cur.z);
+  if (a == 2) return make_int4(prev.z, prev.w, cur.x, cur.y);
+  if (a == 3) return make_int4(prev.y, prev.z, prev.w, cur.x);
+  return cur;
+}
+__device__ __forceinline__ void copy_row_wide(const int32_t* __restrict__ src, int32_t* __restrict__ dst, int c, int lane) {
+  constexpr int U = 4;
+  const int a = (int)((reinterpret_cast<uintptr_t>(dst) >> 2) & 3);
+  const int head = min(c, (4 - a) & 3);                    // src[0, head) lie before the first aligned vector
+  const int m0 = a ? 1 : 0, m_end = (c + a) >> 2;          // whole destination vectors: m0 <= m < m_end
+  if (lane < head) dst[lane] = __ldcs(src + lane);
+  const int4* __restrict__ s4 = reinterpret_cast<const int4*>(src);
+  int4* __restrict__ d4 = reinterpret_cast<int4*>(dst - a);
+  for (int mb = m0; mb < m_end; mb += 32 * U) {
+    int4 cur[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int m = mb + 32 * u + lane;
+      cur[u] = m < m_end ? __ldcs(s4 + m) : make_int4(0, 0, 0, 0);
+    }
+    int4 below = make_int4(0, 0, 0, 0);                    // lane 0 of the first vector: source vector mb - 1
+    if (a != 0 && lane == 0) below = __ldcs(s4 + mb - 1);
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      int4 prev;
+      prev.y = __shfl_up_sync(0xffffffffu, cur[u].y, 1);
+      prev.z = __shfl_up_sync(0xffffffffu, cur[u].z, 1);
+      prev.w = __shfl_up_sync(0xffffffffu, cur[u].w, 1);
+      prev.x = 0;
+      if (lane == 0) prev = below;
+      below.y = __shfl_sync(0xffffffffu, cur[u].y, 31);    // lane 0 of the next vector continues after lane 31 of this one
+      below.z = __shfl_sync(0xffffffffu, cur[u].z, 31);
+      below.w = __shfl_sync(0xffffffffu, cur[u].w, 31);
+      const int m = mb + 32 * u + lane;
+      if (m < m_end) d4[m] = shifted_vector(prev, cur[u], a);
+    }
+  }
+  const int t = max(head, 4 * m_end - a) + lane;           // fewer than four entries after the last whole vector
+  if (t < c) dst[t] = __ldcs(src + t);
+}
+
 template <int G>
 __global__ void __launch_bounds__(256) rows_to_csr_kernel(const int32_t* __restrict__ rows, int64_t cap,
                                                           const int32_t* __restrict__ counts,
@@ -773,7 +824,10 @@ __global__ void __launch_bounds__(256) rows_to_csr_kernel(const int32_t* __restr
     if (c <= 0 || c > cap) continue;
     const int64_t off = offsets[j];
     if (limit != 0 && off + c > limit) continue;
-    copy_row<G>(rows + j * cap, indices + off, c, gl);
+    if (G == 32)
+      copy_row_wide(rows + j * cap, indices + off, c, gl);
+    else
+      copy_row<G>(rows + j * cap, indices + off, c, gl);
   }
 }
 

@@ -189,16 +189,18 @@ __global__ void __launch_bounds__(256) karras_box_kernel(char* nodes_base, int n
 }
 
 template <typename KeyT>
-static void launch_variant_keys(const float* prim, bool is_box, const KeyT* codes, const uint32_t* perm, char* nodes, int n,
-                                const Header* header, VariantScratch v, cudaStream_t stream) {
+static cudaError_t launch_variant_keys(const float* prim, bool is_box, const KeyT* codes, const uint32_t* perm, char* nodes, int n,
+                                       const Header* header, VariantScratch v, cudaStream_t stream) {
   const unsigned gl = (unsigned)((n + 255) / 256);
+  cudaError_t e;
   if (is_box)
-    launch_pdl(karras_leaf_kernel<KeyT, true>, dim3(gl), dim3(256), 0, stream, prim, codes, perm, nodes, n, header);
+    e = launch_pdl(karras_leaf_kernel<KeyT, true>, dim3(gl), dim3(256), 0, stream, prim, codes, perm, nodes, n, header);
   else
-    launch_pdl(karras_leaf_kernel<KeyT, false>, dim3(gl), dim3(256), 0, stream, prim, codes, perm, nodes, n, header);
-  if (n < 2) return;
-  launch_pdl(karras_topdown_kernel<KeyT>, dim3((unsigned)((n - 1 + 255) / 256)), dim3(256), 0, stream, codes, n, v);
-  launch_pdl(karras_box_kernel, dim3(gl), dim3(256), 0, stream, nodes, n, is_box ? kLeafBoxes : kLeafPoints, v);
+    e = launch_pdl(karras_leaf_kernel<KeyT, false>, dim3(gl), dim3(256), 0, stream, prim, codes, perm, nodes, n, header);
+  if (e != cudaSuccess || n < 2) return e;
+  e = launch_pdl(karras_topdown_kernel<KeyT>, dim3((unsigned)((n - 1 + 255) / 256)), dim3(256), 0, stream, codes, n, v);
+  if (e != cudaSuccess) return e;
+  return launch_pdl(karras_box_kernel, dim3(gl), dim3(256), 0, stream, nodes, n, is_box ? kLeafBoxes : kLeafPoints, v);
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
@@ -377,13 +379,14 @@ int launch_variant_karras(const float* prim, bool is_box, const void* sorted_cod
                           void* nodes, int n, const Header* header, void* extra, cudaStream_t stream) {
   VariantScratch v = variant_scratch(static_cast<char*>(extra), n);
   if (n >= 2 && cudaMemsetAsync(v.flags, 0, sizeof(uint32_t) * (size_t)(n - 1), stream) != cudaSuccess) return -1;
+  cudaError_t e;
   if (key_bytes == 4)
-    launch_variant_keys<uint32_t>(prim, is_box, static_cast<const uint32_t*>(sorted_codes), perm, static_cast<char*>(nodes), n,
-                                  header, v, stream);
+    e = launch_variant_keys<uint32_t>(prim, is_box, static_cast<const uint32_t*>(sorted_codes), perm, static_cast<char*>(nodes), n,
+                                      header, v, stream);
   else
-    launch_variant_keys<uint64_t>(prim, is_box, static_cast<const uint64_t*>(sorted_codes), perm, static_cast<char*>(nodes), n,
-                                  header, v, stream);
-  return 0;
+    e = launch_variant_keys<uint64_t>(prim, is_box, static_cast<const uint64_t*>(sorted_codes), perm, static_cast<char*>(nodes), n,
+                                      header, v, stream);
+  return e == cudaSuccess ? 0 : -1;
 }
 
 }  // namespace bvh

@@ -999,3 +999,24 @@ def test_equal_codes_p4_goldens_through_the_cuda_path(B, bits):
         assert e["left_child"][: n - 1].tolist() == [int(t) for t in lc.split()], n
         assert e["rope"].tolist() == [int(t) for t in rp.split()], n
         assert e["perm"].tolist() == list(range(n))
+
+
+@pytest.mark.parametrize("cap", [128, 136, 1024])
+def test_rows_to_csr_wide_copy_every_alignment_and_length(B, cap):
+    """bvh_rows_to_csr on its own ("Store the result"): rows of 128 entries and more are copied by a warp with
+    128-bit accesses whose destination starts at any 4-byte offset.  Every row length 0 .. cap + 3 occurs, next to rows of
+    every other length, so every (alignment, length, head, tail) combination does; rows longer than cap are left alone."""
+    rng = np.random.default_rng(cap)
+    lengths = np.concatenate([np.arange(cap + 4), rng.integers(0, cap + 4, 3000), np.arange(cap + 4)[::-1], [cap] * 9])
+    rng.shuffle(lengths[cap + 4: -9])
+    q = len(lengths)
+    rows = rng.integers(0, 1 << 30, (q, cap)).astype(np.int32)
+    offsets = np.concatenate([[0], np.cumsum(lengths)]).astype(np.int64)
+    want = np.full(int(offsets[-1]) + 8, -5, np.int32)
+    for j in range(q):
+        if lengths[j] <= cap:
+            want[offsets[j]: offsets[j] + lengths[j]] = rows[j, : lengths[j]]
+    got = torch.full((len(want),), -5, dtype=torch.int32, device="cuda")
+    B.bvh_rows_to_csr(_dev(rows.reshape(-1)), cap, _dev(lengths.astype(np.int32)), _dev(offsets), q, got)
+    torch.cuda.synchronize()
+    assert np.array_equal(got.cpu().numpy(), want)
