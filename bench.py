@@ -494,7 +494,9 @@ def run_ours(args) -> dict | None:
                         "what": "whole build as one call, median of 5; last step = build minus the staged times of memset, "
                                 "bounds, Morton and sort (rank 0)"}
         for variant, label in ((1, "karras_topdown + algorithm2 ropes + separate box pass"),
-                               (2, "algorithm3 (apetrei numbering, global atomics) + separate rope pass")):
+                               (2, "algorithm3 (apetrei numbering, global atomics) + separate rope pass"),
+                               (3, "algorithm4 as written (one thread per leaf, global store + ATOMICCAS, ropes and boxes "
+                                   "in the same pass): the paper's modification without the windowed organisation")):
             vscratch = torch.empty(binding.bvh_variant_sizes(n, bits, variant), dtype=torch.uint8, device=device)
             vnodes = torch.empty_like(bvh.nodes)
             vt = []

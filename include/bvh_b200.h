@@ -233,7 +233,7 @@ int bvh_query_any_hit(const void* nodes, int64_t n, const float* queries, int qu
 
 /* NEXT-2: MEASUREMENT variants of the build, not product paths.  They replace the last step (the single
  * bottom-up pass of Algorithm 4) by what the paper compares itself with; bounds, Morton codes, sort and the record
- * layout are unchanged.
+ * layout are unchanged.  (variant = 3 below is the paper's own algorithm in unoptimised form, for the same purpose.)
  *   variant = 1  Karras' top-down construction, one thread per internal node searching its range and split on the
  *                common-prefix length of the augmented keys, skip-connections by Algorithm 2
  *                (PAPER.md:105-116), and a separate bottom-up pass for the boxes with atomic arrival counters in global
@@ -245,6 +245,11 @@ int bvh_query_any_hit(const void* nodes, int64_t n, const float* queries, int qu
  *                the buffer is marked and the query kernels refuse it) and is read back with bvh_variant_export:
  *                left, right: int32[n-1] by Apetrei index (unified child indices: internal p -> p, leaf i -> n-1+i);
  *                rope: int32[2n-1]; aabb: float[2n-1][6]; root: int32[1].  Any output may be NULL.
+ *   variant = 3  Algorithm 4 exactly as the paper writes it, in the plain form of variant 2: one
+ *                thread per leaf, `store` in global memory, ATOMICCAS, the second arrival numbers the parent (L20), writes
+ *                left child and skip-connection (L21-26) and the union of the two boxes, the sibling's read back through L2.
+ *                `nodes` comes out byte-identical to bvh_build_points / bvh_build_boxes.  Against variant 2 it measures what
+ *                the paper's modification saves; against the product, what the windowed organisation of hierarchy.cu adds.
  * scratch must hold bvh_variant_sizes bytes (the product's scratch plus parent / child / counter arrays).  stage_events
  * as in bvh_build_staged (may be NULL); event [12] closes the replaced step.  bvh_variant_sizes is a host call. */
 int bvh_variant_sizes(int64_t n, int morton_bits, int variant, size_t* scratch_bytes);

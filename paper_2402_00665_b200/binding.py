@@ -242,7 +242,8 @@ def bvh_variant_sizes(n: int, morton_bits: int, variant: int) -> int:
 def bvh_build_variant(prim, prim_is_box: int, n: int, morton_bits: int, nodes, scratch, variant: int) -> None:
     """NEXT-2 measurement variants: 1 = Karras top-down + Algorithm 2 + separate box pass (same `nodes` bytes as the
     product); 2 = unmodified Algorithm 3 (Apetrei numbering) + separate skip-connection pass (read with
-    bvh_variant_export)."""
+    bvh_variant_export); 3 = Algorithm 4 as the paper writes it, one thread per leaf with a global `store` (same `nodes`
+    bytes as the product)."""
     _check(load_library().bvh_build_variant(_ptr(prim), prim_is_box, n, morton_bits, _ptr(nodes), _ptr(scratch),
                                             scratch.numel() * scratch.element_size(), variant, _stream(), None),
            "bvh_build_variant")

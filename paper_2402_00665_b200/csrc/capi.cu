@@ -166,7 +166,7 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   if (misaligned(prim) || misaligned(nodes) || misaligned(scratch)) return BVH_ERR_INVALID_ARGUMENT;
   if ((reinterpret_cast<uintptr_t>(nodes) & 31u) != 0) return BVH_ERR_INVALID_ARGUMENT;
   const ScratchLayout L = scratch_layout(n, morton_bits);
-  if (variant < 0 || variant > 2) return BVH_ERR_INVALID_ARGUMENT;
+  if (variant < 0 || variant > 3) return BVH_ERR_INVALID_ARGUMENT;
   if (scratch_bytes < L.total + (variant != 0 ? variant_extra_bytes(n) : 0)) return BVH_ERR_SCRATCH;
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   char* base = static_cast<char*>(scratch);
@@ -225,6 +225,13 @@ static int build(const float* prim, bool is_box, int64_t n, int morton_bits, voi
   if (variant == 2) {
     if (launch_variant_apetrei(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
                                nodes, (int)n, header, base + L.total, stream) != 0)
+      return BVH_ERR_CUDA;
+    mark(12);
+    return check_launch();
+  }
+  if (variant == 3) {
+    if (launch_variant_alg4(prim, is_box, base + L.keys[0], L.key_bytes, reinterpret_cast<const uint32_t*>(base + L.vals[0]),
+                            nodes, (int)n, header, base + L.total, stream) != 0)
       return BVH_ERR_CUDA;
     mark(12);
     return check_launch();
@@ -357,7 +364,7 @@ int bvh_build_staged(const float* prim, int prim_is_box, int64_t n, int morton_b
 }
 
 int bvh_variant_sizes(int64_t n, int morton_bits, int variant, size_t* scratch_bytes) {
-  if (n < 0 || !scratch_bytes || (variant != 1 && variant != 2)) return BVH_ERR_INVALID_ARGUMENT;
+  if (n < 0 || !scratch_bytes || variant < 1 || variant > 3) return BVH_ERR_INVALID_ARGUMENT;
   if (morton_bits != 30 && morton_bits != 63) return BVH_ERR_MORTON_BITS;
   if (n >= ((int64_t)1 << 30)) return BVH_ERR_TOO_LARGE;
   *scratch_bytes = bvh::scratch_layout(n, morton_bits).total + bvh::variant_extra_bytes(n);

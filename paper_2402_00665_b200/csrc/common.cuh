@@ -214,6 +214,9 @@ int launch_variant_karras(const float* prim, bool is_box, const void* sorted_cod
 // ... and the unmodified Algorithm 3 (Apetrei numbering, stored root) followed by a separate skip-connection pass.
 int launch_variant_apetrei(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
                            void* nodes, int n, const Header* header, void* extra, cudaStream_t stream);
+// ... and Algorithm 4 in the same plain form (one thread per leaf, global `store`): byte-identical `nodes`.
+int launch_variant_alg4(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
+                        void* nodes, int n, const Header* header, void* extra, cudaStream_t stream);
 int launch_variant_apetrei_export(const void* nodes, void* extra, int n, int32_t* left, int32_t* right, int32_t* rope,
                                   float* aabb, int32_t* root, cudaStream_t stream);
 // K6/K8: stackless traversal.  kind 0 = spheres (xyzr), 1 = boxes (minmax), 2 = rays (o.xyz, d.xyz, tmin, tmax).

@@ -316,6 +316,98 @@ static cudaError_t launch_apetrei_keys(const float* prim, bool is_box, const Key
   return launch_pdl(apetrei_rope_kernel, dim3((unsigned)((2 * (int64_t)n - 1 + 255) / 256)), dim3(256), 0, stream, nodes, n, v);
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// variant 3: Algorithm 4 AS THE PAPER WRITES IT, in the same plain form as variant 2: one thread per
+// leaf, `store` in global memory initialised to the invalid value (L1), ATOMICCAS (L12 / L17), the first thread to arrive
+// at a parent stops (L13 / L18), the second extends its range by the sibling's (L14 / L19), numbers the parent with its
+// Karras index q (L20: the right end of the range if the parent is itself a left child, else the left end), writes the
+// left child (L21, reading G2: L_p if the left range is the single leaf p, else I_p) and the skip-connection (L22-26:
+// sentinel on the right-most path, else leaf or internal node r = range_right + 1 by comparing delta*(range_right) with
+// delta*(r)), and -- G10 -- the union of its own box with the sibling's, read back through L2 after a fence.  No shared
+// memory, no windows, no lock-step rounds: against variant 2 (Algorithm 3 + the extra skip-connection pass) this isolates
+// what the paper's MODIFICATION saves; against the product (hierarchy.cu) it shows what the windowed organisation adds.
+// The sibling needs no pointer exchange: with Karras numbering its index follows from the ranges (the left child of split
+// p is L_p / I_p, the right child L_{p+1} / I_{p+1}).  `nodes` comes out byte-identical to the product's.
+template <typename KeyT>
+__global__ void __launch_bounds__(256)
+alg4_plain_kernel(const KeyT* __restrict__ codes, char* nodes_base, int n, int leaf_kind, VariantScratch v) {
+  pdl_wait();
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n || n < 2) return;
+  const int leaf_base = n - 1;
+  Node* internal = reinterpret_cast<Node*>(nodes_base + kNodesHeaderBytes);
+  int* store = reinterpret_cast<int*>(v.flags);
+  auto sim = [&](int a) { return (a < 0 || a >= n - 1) ? -1 : prefix_len(codes, n, codes[a], a, a + 1); };   // larger = smaller delta*
+  int range_left = i, range_right = i;                       // L2
+  int sim_left = sim(i - 1), sim_right = sim(i);             // L3-4 (the leaf's own skip-connection, L5-8: karras_leaf_kernel)
+  float lo[3], hi[3];
+  load_box_any(nodes_base, n, leaf_kind, leaf_base + i, lo, hi);
+  while (true) {
+    const bool is_left = sim_right > sim_left;               // L10: delta_right < delta_left
+    const int p = is_left ? range_right : range_left - 1;    // L11 / L16: the split of the parent
+    __threadfence();                                         // this node's record before its arrival
+    const int other = atomicCAS(store + p, kInvalid, is_left ? range_left : range_right);   // L12 / L17
+    if (other == kInvalid) return;                           // L13 / L18
+    __threadfence();
+    int sib;
+    if (is_left) {
+      range_right = other;                                   // L14
+      sim_right = sim(range_right);
+      sib = (range_right == p + 1) ? leaf_base + p + 1 : p + 1;
+    } else {
+      range_left = other;                                    // L19
+      sim_left = sim(range_left - 1);
+      sib = (range_left == p) ? leaf_base + p : p;
+    }
+    const int q = (sim_right > sim_left) ? range_right : range_left;            // L20
+    const int left = (range_left == p) ? leaf_base + p : p;                     // L21
+    int rope = kSentinel;                                                       // L22-23
+    if (range_right != n - 1) {
+      const int r = range_right + 1;                                            // L25
+      rope = (sim_right > sim(r)) ? leaf_base + r : r;                          // L26: delta*(range_right) < delta*(r) -> leaf
+    }
+    float lo2[3], hi2[3];
+    load_box_any(nodes_base, n, leaf_kind, sib, lo2, hi2);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      lo[a] = fminf(lo[a], lo2[a]);
+      hi[a] = fmaxf(hi[a], hi2[a]);
+    }
+    Node rec;
+    rec.lo = make_float4(lo[0], lo[1], lo[2], __int_as_float(left));
+    rec.hi = make_float4(hi[0], hi[1], hi[2], __int_as_float(rope));
+    internal[q] = rec;
+    if (q == 0) return;                                      // L28: the root
+  }
+}
+
+template <typename KeyT>
+static cudaError_t launch_alg4_keys(const float* prim, bool is_box, const KeyT* codes, const uint32_t* perm, char* nodes, int n,
+                                    const Header* header, VariantScratch v, cudaStream_t stream) {
+  const unsigned gl = (unsigned)((n + 255) / 256);
+  cudaError_t e;
+  if (is_box)
+    e = launch_pdl(karras_leaf_kernel<KeyT, true>, dim3(gl), dim3(256), 0, stream, prim, codes, perm, nodes, n, header);
+  else
+    e = launch_pdl(karras_leaf_kernel<KeyT, false>, dim3(gl), dim3(256), 0, stream, prim, codes, perm, nodes, n, header);
+  if (e != cudaSuccess) return e;
+  return launch_pdl(alg4_plain_kernel<KeyT>, dim3(gl), dim3(256), 0, stream, codes, nodes, n, is_box ? kLeafBoxes : kLeafPoints, v);
+}
+
+int launch_variant_alg4(const float* prim, bool is_box, const void* sorted_codes, int key_bytes, const uint32_t* perm,
+                        void* nodes, int n, const Header* header, void* extra, cudaStream_t stream) {
+  VariantScratch v = variant_scratch(static_cast<char*>(extra), n);
+  if (n >= 2 && cudaMemsetAsync(v.flags, 0xFF, sizeof(uint32_t) * (size_t)(n - 1), stream) != cudaSuccess) return -1;   // store <- invalid (L1)
+  cudaError_t e;
+  if (key_bytes == 4)
+    e = launch_alg4_keys<uint32_t>(prim, is_box, static_cast<const uint32_t*>(sorted_codes), perm, static_cast<char*>(nodes), n,
+                                   header, v, stream);
+  else
+    e = launch_alg4_keys<uint64_t>(prim, is_box, static_cast<const uint64_t*>(sorted_codes), perm, static_cast<char*>(nodes), n,
+                                   header, v, stream);
+  return e == cudaSuccess ? 0 : -1;
+}
+
 // variant 2 export: the arrays of the Apetrei-numbered hierarchy in the unified index space (internal I_p -> p).
 __global__ void apetrei_export_kernel(const char* __restrict__ nodes, VariantScratch v, int n, int32_t* left, int32_t* right,
                                       int32_t* rope, float* aabb, int32_t* root) {

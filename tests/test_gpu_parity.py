@@ -1020,3 +1020,47 @@ def test_rows_to_csr_wide_copy_every_alignment_and_length(B, cap):
     B.bvh_rows_to_csr(_dev(rows.reshape(-1)), cap, _dev(lengths.astype(np.int32)), _dev(offsets), q, got)
     torch.cuda.synchronize()
     assert np.array_equal(got.cpu().numpy(), want)
+
+
+@pytest.mark.parametrize("name,n", [("C1", 4096), ("C2", 100_001), ("C3", 300_000), ("C4", 120_000), ("C5", 70_000)])
+def test_variant_algorithm4_as_written(B, oracle_lib, name, n):
+    """NEXT-2, third arm: Algorithm 4 in the plain form the paper gives it (one thread per leaf, global
+    `store`, ATOMICCAS) produces the same bytes as the product's windowed single pass, and both equal the oracle."""
+    w = W.make(name, n=n, q=0)
+    is_box = int(w.prims.shape[1] == 6)
+    a = B.Bvh(w.n, w.morton_bits)
+    a.nodes.zero_()
+    a.build(_dev(w.prims))
+    v = B.Bvh(w.n, w.morton_bits)
+    v.scratch = torch.empty(B.bvh_variant_sizes(w.n, w.morton_bits, 3), dtype=torch.uint8, device="cuda")
+    v.nodes.zero_()
+    for _ in range(2):                                  # twice into the same scratch: `store` is re-initialised per build
+        B.bvh_build_variant(_dev(w.prims), is_box, w.n, w.morton_bits, v.nodes, v.scratch, 3)
+        torch.cuda.synchronize()
+        assert torch.equal(a.nodes, v.nodes)
+    assert_build_equal(export_np(v), oracle_lib.build_bvh(w.prims, w.morton_bits), name)
+    for tiny in (1, 2, 3, 4, 5):
+        pts = W.uniform_cube(tiny, seed=tiny)
+        t = B.Bvh(tiny, 63)
+        t.scratch = torch.empty(B.bvh_variant_sizes(tiny, 63, 3), dtype=torch.uint8, device="cuda")
+        B.bvh_build_variant(_dev(pts), 0, tiny, 63, t.nodes, t.scratch, 3)
+        torch.cuda.synchronize()
+        assert_build_equal(export_np(t), oracle_lib.build_bvh(pts, 63), f"tiny {tiny}")
+    # the paper's worked example (PAPER.md:120) and the equal-codes case, against the hand-derived goldens
+    g = _gold_arrays("p1_worked_example.txt")
+    pts, perm = _p1_points()
+    t = B.Bvh(8, 30)
+    t.scratch = torch.empty(B.bvh_variant_sizes(8, 30, 3), dtype=torch.uint8, device="cuda")
+    B.bvh_build_variant(_dev(pts), 0, 8, 30, t.nodes, t.scratch, 3)
+    torch.cuda.synchronize()
+    e = export_np(t)
+    assert e["left_child"][:7].tolist() == g["left_child"] and e["rope"].tolist() == g["rope"] and e["perm"].tolist() == perm.tolist()
+    for line in _gold_rows("p4_equal_codes.txt"):
+        head, lc, rp = line.split("|")
+        m = int(head.split()[1])
+        t = B.Bvh(m, 30)
+        t.scratch = torch.empty(B.bvh_variant_sizes(m, 30, 3), dtype=torch.uint8, device="cuda")
+        B.bvh_build_variant(_dev(np.full((m, 3), 0.25, np.float32)), 0, m, 30, t.nodes, t.scratch, 3)
+        torch.cuda.synchronize()
+        e = export_np(t)
+        assert e["left_child"][: m - 1].tolist() == [int(x) for x in lc.split()] and e["rope"].tolist() == [int(x) for x in rp.split()]
