@@ -49,10 +49,14 @@ NOMINAL_HBM_GBS = 8000.0   # the denominator BASELINE.json north_star names
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of a kernel from the `ncu --set full` captures
 # summarised in profiles/, keyed by (workload, n, q): `roofline.traffic` is null for any other workload or size.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r02b_ncu.md: one step, rows 2 (collect), 6 (rows_to_csr), 14 (hierarchy, level 1); two-pass leg, rows 0 (count),
-    # 1 (fill): DRAM read + write
-    ("C3", 10_000_000, 1_000_000): {"collect": 3_180_800_000, "rows_to_csr": 4_995_000_000, "count": 241_363_000,
-                                    "fill": 3_220_800_000, "hierarchy": 1_335_100_000},
+    # profiles/r03_ncu.md, one step each: collect, rows_to_csr, level 1 of the hierarchy (DRAM read + write);
+    # profiles/r02b_ncu.md, two-pass leg, rows 0 (count), 1 (fill)
+    ("C3", 10_000_000, 1_000_000): {"collect": 3_180_537_000, "rows_to_csr": 4_829_984_000, "count": 241_363_000,
+                                    "fill": 3_220_800_000, "hierarchy": 1_333_382_000},
+    ("C4", 4_000_000, 4_000_000): {"collect": 948_331_008, "rows_to_csr": 313_999_616,
+                                   "hierarchy": 605_211_136},
+    ("C5", 1 << 24, 1 << 24): {"collect": 6_883_123_000, "rows_to_csr": 5_561_789_000,
+                               "hierarchy": 2_681_882_000},
 }
 
 

@@ -406,7 +406,7 @@ __device__ __forceinline__ void traverse_body(const TraverseArgs& A, TravSmem<Qu
     if (MODE == kModeFill && A.only_over) have = have && (int64_t)A.counts[j] > A.cap;
     if (MODE == kModeFill && A.out_limit != 0) have = have && A.offsets[j + 1] <= A.out_limit;
     Query query;
-    query.load(queries, j);
+    query.load(queries, have ? j : 0);                       // (the overflow pass serves few rows: no gather for the others)
     __syncwarp();                                            // the previous chunk's scans are over
     query.to_shared(s_query + threadIdx.x * Query::kSlotWords);
     int32_t* row = nullptr;
